@@ -1,0 +1,162 @@
+/* qhap.h -- C ABI of the QHap hot path on B200 (sm_100a).
+ *
+ * Method: QHap, arxiv/paper_2603_25762.  Citations are line numbers of /root/reference/PAPER.md
+ * (section / equation in brackets).  The library turns a fragment x heterozygous-SNP matrix into a Max-Cut
+ * graph (read graph: PAPER.md:L235-L246 [Eq. 2-3]; SNP graph: L287-L319 [Eq. 9-14], Pore-C scaling L350),
+ * solves it with ballistic simulated bifurcation over many replicas (L252-L267 [Eq. 4-6]) and reads the
+ * phase assignment back (L271-L281 [Eq. 7-8]; L336-L338).
+ *
+ * Conventions (every entry point):
+ *  - plain C, no exceptions cross the boundary; every function returns a qhap_status.
+ *  - ALL array pointers are DEVICE pointers owned by the caller unless the comment says HOST.  The library
+ *    allocates nothing that outlives a call.  Scratch comes from the caller's `workspace` (device memory,
+ *    256-byte aligned).  Calling with workspace == NULL is a SIZE QUERY: it writes the required byte count to
+ *    *ws_bytes, launches nothing and returns QHAP_OK.  With workspace != NULL, *ws_bytes is the size provided;
+ *    too small -> QHAP_ERR_WORKSPACE (and *ws_bytes = required).
+ *  - all work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).  Entry points
+ *    that return a count to the host (graph builds: nnz) synchronise the stream once; qhap_bsb_solve,
+ *    qhap_cut_eval and the readouts are asynchronous: results are valid after the caller synchronises.
+ *  - no global state, no hidden RNG, no CPU fallback: without an sm_100 device every call returns QHAP_ERR_CUDA.
+ *  - qhap_last_error() returns a thread-local text for the last non-OK status.
+ */
+#ifndef QHAP_H_
+#define QHAP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define QHAP_API __attribute__((visibility("default")))
+#else
+#define QHAP_API
+#endif
+
+typedef enum {
+  QHAP_OK = 0,
+  QHAP_ERR_INVALID_ARG = 1, /* NULL where an array is required, negative size, unknown mode              */
+  QHAP_ERR_RANGE = 2,       /* a value is not exactly representable (|J| > 2048 in fp16 dense J, > 256 in  */
+                            /* bf16; fixed-point sum overflow; nnz >= 2^31)                                  */
+  QHAP_ERR_WORKSPACE = 3,   /* workspace or output capacity too small; required size written back          */
+  QHAP_ERR_CUDA = 4         /* CUDA runtime error or no sm_100 device                                       */
+} qhap_status;
+
+/* Fragment matrix: reads x het SNPs with alleles {0,1,missing} and base qualities (PAPER.md:L216 last sentence;
+ * the ternary matrix M of Eq. 1 [L226-L229] and the quality matrix W of Eq. 9-10 [L289-L295] are implicit).
+ * CSR by fragment, snp_idx strictly ascending inside a fragment.  The read-graph build additionally requires
+ * non-empty fragments sorted by their first SNP index (checked on the device -> QHAP_ERR_INVALID_ARG). */
+typedef struct {
+  int32_t n_frag, n_snp;
+  int64_t nnz;               /* = frag_ptr[n_frag] (host copy, so that size queries need no device read)  */
+  const int64_t *frag_ptr;   /* [n_frag+1]                                                                */
+  const int32_t *snp_idx;    /* [nnz]                                                                     */
+  const uint8_t *allele;     /* [nnz] 0 = ref, 1 = alt, 2 = missing (entry ignored everywhere, Eq. 1 "0") */
+  const uint8_t *qual;       /* [nnz] integer Phred, clamped to [1,93]; may be NULL for the read graph    */
+  const uint8_t *frag_flags; /* [n_frag] bit0: Pore-C derived (SNP graph: contribution x alpha, L350); NULL = 0 */
+  const uint8_t *h1;         /* [n_snp] allele carried by the initial H1 (gauge, L222); NULL = all 0      */
+} qhap_frags;
+
+/* Symmetric weighted graph in CSR: both (a,b) and (b,a) stored, columns strictly ascending in a row, no diagonal.
+ * Read graph: d = # shared SNPs with opposing alleles (Eq. 2-3), c = # shared with equal alleles.
+ * SNP graph: w_fx = Eq. 14 as an exact int64 fixed-point sum at scale 2^-32; w = (float)(w_fx * 2^-32). */
+typedef struct {
+  int32_t n;        /* vertices                                                                          */
+  int64_t nnz;      /* directed entries; on input to a build: CAPACITY of col/d/c/w_fx/w                 */
+  int32_t *row_ptr; /* [n+1]                                                                             */
+  int32_t *col;     /* [nnz]                                                                             */
+  int32_t *d, *c;   /* [nnz] read graph only (else NULL)                                                 */
+  int64_t *w_fx;    /* [nnz] SNP graph only (else NULL)                                                  */
+  float *w;         /* [nnz] SNP graph only (else NULL)                                                  */
+} qhap_csr;
+
+enum { QHAP_WEIGHT_D = 0,        /* w = D        (paper Eq. 3, non-negative)                               */
+       QHAP_WEIGHT_D_MINUS_C = 1,/* w = D - C    (BASELINE.json config 0: "discordant minus concordant")   */
+       QHAP_WEIGHT_FX = 2 };     /* w = w_fx     (SNP graph)                                               */
+enum { QHAP_DENSE_NONE = 0, QHAP_DENSE_FP16 = 1, QHAP_DENSE_BF16 = 2 };
+
+/* (1) Read-graph build, PAPER.md:L235-L246 [Eq. 2-3]; edge set = pairs of fragments sharing >= 1 covered SNP.
+ * out->row_ptr must point to [n_frag+1] ints.  If out->col == NULL or out->nnz (capacity) is too small only the
+ * count pass runs: row_ptr and out->nnz (required) are written and QHAP_ERR_WORKSPACE is returned when col != NULL.
+ * Otherwise col/d/c are filled.  Optionally also writes J = -w (Eq. 4) for `weight_mode` as a dense row-major
+ * [dense_ld x dense_ld] matrix (dense_ld >= n_frag, multiple of 8; padding rows/cols written as 0) in fp16 or bf16;
+ * an entry that is not exactly representable gives QHAP_ERR_RANGE (checked on device, reported after the sync). */
+QHAP_API qhap_status qhap_build_read_graph(const qhap_frags *frags, int32_t weight_mode, qhap_csr *out, void *dense_J,
+                                  int32_t dense_ld, int32_t dense_dtype, void *workspace, size_t *ws_bytes,
+                                  void *stream);
+
+/* (2) SNP-graph build, PAPER.md:L287-L319 [Eq. 9-14]; linkage depth k/10 (L85): each SNP of a fragment is linked to
+ * its nearest floor(k (|S_i|-1) / 10) downstream SNPs; Pore-C fragments (flag bit0) use the exhaustive depth and
+ * their terms are scaled by alpha (L350).  Every term is rounded to int64 at scale 2^32 and integer-added, so the
+ * result does not depend on the summation order.  `llr_table` is a HOST array [94*94] of fp64
+ * log10(P_cis/P_trans) indexed Qu*94+Qv (Eq. 9, 11, 12), or NULL to let the library evaluate it with the C library.
+ * Capacity protocol as for the read graph (out->row_ptr is [n_snp+1]). */
+QHAP_API qhap_status qhap_build_snp_graph(const qhap_frags *frags, int32_t linkage_tenths, double alpha,
+                                 const double *llr_table, qhap_csr *out, void *workspace, size_t *ws_bytes,
+                                 void *stream);
+
+/* bSB parameters (PAPER.md:L265 gives the outline; constants from BASELINE.json; readings R10a-f):
+ *   a_k = a0 k / (steps_total - 1), k = step_begin .. step_begin + steps_run - 1
+ *   F = J x (x of the previous step);  y += dt (-(a0 - a_k) x + c0 F);  x += dt a0 y;  |x| > 1: x = sign(x), y = 0. */
+typedef struct {
+  int32_t replicas;     /* R; x, y are [n][R] with the replica index contiguous                           */
+  int32_t steps_total;  /* T of the ramp                                                                  */
+  int32_t step_begin;   /* first step index run by this call (resume)                                     */
+  int32_t steps_run;    /* number of steps run by this call                                               */
+  double dt, a0;        /* BASELINE.json: 1.25, 1.0                                                       */
+  double c0;            /* <= 0: automatic 0.5 sqrt(N-1) / ||J||_F per instance                           */
+  uint64_t seed;        /* used when init_state != 0                                                      */
+  int32_t weight_mode;  /* QHAP_WEIGHT_*: which CSR arrays define w (J = -w)                              */
+  int32_t path;         /* 0 auto, 1 dense tcgen05 GEMM (needs dense_J), 2 sparse CSR                     */
+  int32_t tile_skip;    /* dense path: 1 = skip all-zero 64-column blocks of J (bit-identical result)     */
+  int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
+  int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */
+  int32_t reserved;
+} qhap_bsb_params;
+
+/* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`
+ * (instance b owns rows inst_ptr[b] .. inst_ptr[b+1]-1; all its columns lie in the same range).
+ * inst_ptr: HOST array [n_inst+1] or NULL for a single instance.  dense_J: optional dense J (see above) for the
+ * tensor-core path (single instance only).  x, y: [graph->n][R] fp32 in/out.  Outputs (used when finalize != 0):
+ * best_spins [graph->n] int8 (+1/-1, sign(0) = +1), best_cut [n_inst] int64 in the graph's integer units,
+ * best_replica [n_inst] (lowest index with maximal cut), cut_per_replica [n_inst][R] (may be NULL). */
+QHAP_API qhap_status qhap_bsb_solve(const qhap_csr *graph, int32_t n_inst, const int32_t *inst_ptr, const void *dense_J,
+                           int32_t dense_ld, int32_t dense_dtype, const qhap_bsb_params *params, float *x, float *y,
+                           int8_t *best_spins, int64_t *best_cut, int32_t *best_replica, int64_t *cut_per_replica,
+                           void *workspace, size_t *ws_bytes, void *stream);
+
+/* (5) Cut and Ising energy of given spins, PAPER.md:L254-L263 [Eq. 4-6]:
+ *   cut_r = sum over undirected edges with s_a != s_b of w_ab;  energy_r = W_tot - 2 cut_r  (= -1/2 s^T J s, J = -A),
+ * in the graph's integer units (counts, or 2^-32 fixed point).  spins: [n][R] int8 (+1/-1).  energy may be NULL. */
+QHAP_API qhap_status qhap_cut_eval(const qhap_csr *graph, int32_t weight_mode, const int8_t *spins, int32_t replicas,
+                          int64_t *cut, int64_t *energy, void *workspace, size_t *ws_bytes, void *stream);
+
+/* (6) Phase readout.  Read-based vote, PAPER.md:L271-L281 [Eq. 7-8]: v_j = sum_i s_i M_ij;
+ * hap1[j] = H1 allele if v_j > 0, the other allele if v_j < 0, -1 (unphased) if v_j == 0.
+ * SNP-based (L336-L338 with one solve): hap1[u] = h1[u] if s_u > 0 else 1 - h1[u]. */
+QHAP_API qhap_status qhap_phase_readout_reads(const qhap_frags *frags, const int8_t *spins /*[n_frag]*/, int8_t *hap1 /*[n_snp]*/,
+                                     void *workspace, size_t *ws_bytes, void *stream);
+QHAP_API qhap_status qhap_phase_readout_snps(int32_t n_snp, const uint8_t *h1 /*may be NULL*/, const int8_t *spins,
+                                    int8_t *hap1, void *stream);
+
+/* (7) Block split (BASELINE.json config 3: "independent 5k-SNP overlapping blocks"; R17): sub-graphs induced
+ * by the SNP windows [win[2b], win[2b+1]) (HOST array), emitted as one block-diagonal CSR in the order of the windows.
+ * Capacity protocol as for the builds; out->row_ptr is [sum of window lengths + 1]. */
+QHAP_API qhap_status qhap_block_split(const qhap_csr *graph, int32_t n_blocks, const int64_t *win, qhap_csr *out,
+                             void *workspace, size_t *ws_bytes, void *stream);
+
+/* (7) Block stitch: orient each block against the previous one by the majority over the overlap, each block owning
+ * the SNPs up to the overlap midpoint.  block_spins: concatenated per-block spins (device); out: [n] (device). */
+QHAP_API qhap_status qhap_block_stitch(int32_t n, int32_t n_blocks, const int64_t *win /*HOST*/, const int8_t *block_spins,
+                              int8_t *out, void *workspace, size_t *ws_bytes, void *stream);
+
+QHAP_API const char *qhap_last_error(void);
+/* Library / build identification, e.g. "qhap-b200 0.1 sm_100a". */
+QHAP_API const char *qhap_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QHAP_H_ */

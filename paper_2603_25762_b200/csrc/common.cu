@@ -1,0 +1,106 @@
+// libqhap: error text, device check, exclusive scan.
+#include "common.cuh"
+
+#include <stdarg.h>
+
+namespace qhap {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+static int g_dev_checked = 0;  // 0 unknown, 1 ok, -1 bad
+static int g_sm_count = 0;
+
+qhap_status require_device() {
+  if (g_dev_checked == 1) return QHAP_OK;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  cudaDeviceProp prop;
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) {
+    set_error("no CUDA device: %s (libqhap has no CPU fallback)", cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return QHAP_ERR_CUDA;
+  }
+  if (prop.major != 10) {
+    set_error("device '%s' is sm_%d%d; libqhap is built for sm_100a only", prop.name, prop.major, prop.minor);
+    return QHAP_ERR_CUDA;
+  }
+  g_sm_count = prop.multiProcessorCount;
+  g_dev_checked = 1;
+  return QHAP_OK;
+}
+
+int sm_count() { return g_sm_count > 0 ? g_sm_count : 148; }
+
+// ------------------------------------------------------------------------------------------------ scan
+// One CTA of 1024 threads walks the array in tiles of 4096 counts, carrying the running total.
+__global__ void __launch_bounds__(1024) scan_i32_kernel(const int32_t* __restrict__ in, int32_t* __restrict__ out,
+                                                        int64_t n, int64_t* total_dev, int32_t* overflow_dev) {
+  __shared__ int64_t warp_tot[32];
+  __shared__ int64_t carry_s;
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  if (t == 0) carry_s = 0;
+  __syncthreads();
+  for (int64_t base = 0; base < n; base += 4096) {
+    int64_t i0 = base + int64_t(t) * 4;
+    int32_t v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = (i0 + k < n) ? in[i0 + k] : 0;
+    int64_t s = int64_t(v[0]) + v[1] + v[2] + v[3];
+    int64_t incl = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int64_t u = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += u;
+    }
+    if (lane == 31) warp_tot[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+      int64_t w = warp_tot[lane];
+      int64_t wi = w;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int64_t u = __shfl_up_sync(0xffffffffu, wi, o);
+        if (lane >= o) wi += u;
+      }
+      warp_tot[lane] = wi - w;  // exclusive prefix of the warp totals
+    }
+    __syncthreads();
+    int64_t carry = carry_s;
+    int64_t excl = carry + warp_tot[wid] + (incl - s);
+    // tile total = prefix of the last thread + its sum
+    __syncthreads();
+    if (t == 1023) carry_s = excl + s;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (i0 + k < n) out[i0 + k] = int32_t(excl);
+      excl += v[k];
+    }
+    __syncthreads();
+  }
+  if (t == 0) {
+    int64_t tot = carry_s;
+    out[n] = int32_t(tot);
+    if (total_dev) *total_dev = tot;
+    if (overflow_dev && tot > int64_t(0x7fffffff)) *overflow_dev = 1;
+  }
+}
+
+qhap_status exclusive_scan_i32(const int32_t* in, int32_t* out, int64_t n, int64_t* total_dev, int32_t* overflow_dev,
+                               cudaStream_t stream) {
+  scan_i32_kernel<<<1, 1024, 0, stream>>>(in, out, n, total_dev, overflow_dev);
+  QHAP_LAUNCH_CHECK();
+  return QHAP_OK;
+}
+
+}  // namespace qhap
+
+extern "C" const char* qhap_last_error(void) { return qhap::g_err; }
+extern "C" const char* qhap_version(void) { return "qhap-b200 0.1 sm_100a"; }

@@ -1,0 +1,232 @@
+// (5) Cut / Ising-energy evaluation and best-replica selection.  PAPER.md:L254-L267 [Eq. 4-6].
+//   cut_r = sum_{a<b, s_a != s_b} w_ab,  E_r = W_tot - 2 cut_r,  r* = lowest r with maximal cut.
+// Integer arithmetic only (int32 counts or int64 2^-32 fixed point) -> bit-exact and order independent.
+// Layout: lanes run across replicas (the contiguous dimension of spins[n][R] / x[n][R]); a warp owns a tile of
+// consecutive rows and a chunk of 32*VEC replicas, keeps VEC int64 partial cuts per lane in registers and flushes them
+// with one atomicAdd per (lane, slot) when its tile (or the instance) ends.
+#include "kernels.cuh"
+
+namespace qhap {
+
+namespace {
+
+constexpr int kRowsPerWarp = 32;
+
+template <class SpinT, int VEC>
+struct SpinLoad;
+
+// int8 spins, 4 per 32-bit word: returns a mask with bit k set when replica k is -1.
+template <>
+struct SpinLoad<int8_t, 4> {
+  static __device__ __forceinline__ uint32_t load(const int8_t* p) {
+    uint32_t v = *reinterpret_cast<const uint32_t*>(p);
+    return ((v >> 7) & 1u) | ((v >> 14) & 2u) | ((v >> 21) & 4u) | ((v >> 28) & 8u);
+  }
+};
+template <>
+struct SpinLoad<int8_t, 1> {
+  static __device__ __forceinline__ uint32_t load(const int8_t* p) { return (*p < 0) ? 1u : 0u; }
+};
+// fp32 positions: s = +1 if x >= 0 else -1 (R10e)
+template <>
+struct SpinLoad<float, 4> {
+  static __device__ __forceinline__ uint32_t load(const float* p) {
+    float4 v = *reinterpret_cast<const float4*>(p);
+    return (v.x >= 0.f ? 0u : 1u) | (v.y >= 0.f ? 0u : 2u) | (v.z >= 0.f ? 0u : 4u) | (v.w >= 0.f ? 0u : 8u);
+  }
+};
+template <>
+struct SpinLoad<float, 1> {
+  static __device__ __forceinline__ uint32_t load(const float* p) { return (*p >= 0.f) ? 0u : 1u; }
+};
+
+template <class SpinT, int VEC>
+__global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const int32_t* __restrict__ row_ptr,
+                                                             const int32_t* __restrict__ col,
+                                                             const int32_t* __restrict__ d, const int32_t* __restrict__ c,
+                                                             const int64_t* __restrict__ w_fx, int mode,
+                                                             const SpinT* __restrict__ spins, int32_t R, int32_t n_inst,
+                                                             const int32_t* __restrict__ inst_ptr,
+                                                             unsigned long long* __restrict__ cut,
+                                                             unsigned long long* __restrict__ wtot) {
+  const int lane = threadIdx.x & 31;
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int chunks = (R + 32 * VEC - 1) / (32 * VEC);
+  const int64_t n_tiles = (int64_t(n) + kRowsPerWarp - 1) / kRowsPerWarp;
+  const int64_t n_warps = (int64_t(gridDim.x) * blockDim.x) >> 5;
+  for (int64_t work = warp; work < n_tiles * chunks; work += n_warps) {
+    const int chunk = int(work % chunks);
+    const int32_t a0 = int32_t(work / chunks) * kRowsPerWarp;
+    const int32_t a1 = min(n, a0 + kRowsPerWarp);
+    const int r = chunk * 32 * VEC + lane * VEC;
+    const bool active = r < R;  // R % VEC == 0 is guaranteed by the dispatcher
+    // instance of the first row (binary search; inst_ptr is tiny)
+    int inst = 0;
+    if (n_inst > 1) {
+      int lo = 0, hi = n_inst;
+      while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (inst_ptr[mid] <= a0) lo = mid; else hi = mid;
+      }
+      inst = lo;
+    }
+    int64_t acc[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) acc[k] = 0;
+    int64_t wsum = 0;
+    auto flush = [&](int b) {
+      if (active) {
+#pragma unroll
+        for (int k = 0; k < VEC; ++k)
+          if (acc[k] != 0) atomicAdd(&cut[size_t(b) * R + r + k], (unsigned long long)acc[k]);
+      }
+#pragma unroll
+      for (int k = 0; k < VEC; ++k) acc[k] = 0;
+      if (chunk == 0) {
+        int64_t t = warp_sum(wsum);
+        if (lane == 0 && t != 0) atomicAdd(&wtot[b], (unsigned long long)t);
+      }
+      wsum = 0;
+    };
+    for (int32_t a = a0; a < a1; ++a) {
+      if (n_inst > 1 && a >= inst_ptr[inst + 1]) {
+        flush(inst);
+        while (a >= inst_ptr[inst + 1]) ++inst;
+      }
+      const int32_t e0 = row_ptr[a], e1 = row_ptr[a + 1];
+      const uint32_t sa = active ? SpinLoad<SpinT, VEC>::load(spins + size_t(a) * R + r) : 0u;
+      for (int32_t eb = e0; eb < e1; eb += 32) {
+        // lanes fetch 32 entries, then broadcast them one by one
+        const int32_t e = eb + lane;
+        int32_t my_col = -1;
+        int64_t my_w = 0;
+        if (e < e1) {
+          my_col = col[e];
+          if (my_col > a) my_w = edge_weight(mode, d, c, w_fx, e);   // each undirected edge once
+        }
+        if (chunk == 0 && my_col > a) wsum += my_w;
+        const int cnt = min(32, e1 - eb);
+        for (int j = 0; j < cnt; ++j) {
+          const int32_t b = __shfl_sync(0xffffffffu, my_col, j);
+          const int64_t w = __shfl_sync(0xffffffffu, my_w, j);
+          if (b <= a || !active) continue;
+          const uint32_t diff = sa ^ SpinLoad<SpinT, VEC>::load(spins + size_t(b) * R + r);
+#pragma unroll
+          for (int k = 0; k < VEC; ++k) acc[k] += ((diff >> k) & 1u) ? w : 0;
+        }
+      }
+    }
+    flush(inst);
+  }
+}
+
+// One CTA per instance: energy = W_tot - 2 cut, best replica = lowest index with maximal cut.
+__global__ void __launch_bounds__(256) cut_finalize_kernel(int32_t R, const long long* __restrict__ cut,
+                                                           const long long* __restrict__ wtot,
+                                                           long long* __restrict__ energy,
+                                                           long long* __restrict__ best_cut,
+                                                           int32_t* __restrict__ best_replica) {
+  const int b = blockIdx.x;
+  __shared__ long long s_cut[256];
+  __shared__ int s_idx[256];
+  long long bc = 0;
+  int bi = 0x7fffffff;
+  for (int r = threadIdx.x; r < R; r += blockDim.x) {
+    long long v = cut[size_t(b) * R + r];
+    if (energy) energy[size_t(b) * R + r] = wtot[b] - 2 * v;
+    if (bi == 0x7fffffff || v > bc) { bc = v; bi = r; }   // ascending r per thread: ties keep the lower index
+  }
+  s_cut[threadIdx.x] = bc;
+  s_idx[threadIdx.x] = bi;
+  __syncthreads();
+  for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      long long v2 = s_cut[threadIdx.x + o];
+      int i2 = s_idx[threadIdx.x + o];
+      int i1 = s_idx[threadIdx.x];
+      if (i2 != 0x7fffffff && (i1 == 0x7fffffff || v2 > s_cut[threadIdx.x] || (v2 == s_cut[threadIdx.x] && i2 < i1))) {
+        s_cut[threadIdx.x] = v2;
+        s_idx[threadIdx.x] = i2;
+      }
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    if (best_cut) best_cut[b] = s_cut[0];
+    if (best_replica) best_replica[b] = s_idx[0];
+  }
+}
+
+__global__ void __launch_bounds__(256) gather_best_spins_kernel(int32_t n, int32_t R, const float* __restrict__ x,
+                                                                int32_t n_inst, const int32_t* __restrict__ inst_ptr,
+                                                                const int32_t* __restrict__ best_replica,
+                                                                int8_t* __restrict__ best_spins) {
+  const int32_t a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= n) return;
+  int inst = 0;
+  if (n_inst > 1) {
+    int lo = 0, hi = n_inst;
+    while (hi - lo > 1) {
+      int mid = (lo + hi) >> 1;
+      if (inst_ptr[mid] <= a) lo = mid; else hi = mid;
+    }
+    inst = lo;
+  }
+  best_spins[a] = (x[size_t(a) * R + best_replica[inst]] >= 0.f) ? int8_t(1) : int8_t(-1);
+}
+
+template <class SpinT>
+qhap_status launch_cut(const CsrView& g, int mode, const SpinT* spins, int32_t R, int32_t n_inst,
+                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream) {
+  QHAP_CUDA_TRY(cudaMemsetAsync(cut, 0, sizeof(int64_t) * size_t(n_inst) * R, stream));
+  QHAP_CUDA_TRY(cudaMemsetAsync(wtot, 0, sizeof(int64_t) * size_t(n_inst), stream));
+  if (g.n == 0 || R == 0) return QHAP_OK;
+  const bool vec4 = (R % 4 == 0) && ((reinterpret_cast<uintptr_t>(spins) & (4 * sizeof(SpinT) - 1)) == 0);
+  const int chunks = vec4 ? (R + 127) / 128 : (R + 31) / 32;
+  const int64_t work = ceil_div(g.n, kRowsPerWarp) * chunks;
+  const int blocks = int(std::min<int64_t>(ceil_div(work, 8), int64_t(sm_count()) * 8));
+  auto* cu = reinterpret_cast<unsigned long long*>(cut);
+  auto* wt = reinterpret_cast<unsigned long long*>(wtot);
+  if (vec4)
+    cut_accumulate_kernel<SpinT, 4><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, spins, R,
+                                                                n_inst, inst_ptr_dev, cu, wt);
+  else
+    cut_accumulate_kernel<SpinT, 1><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, spins, R,
+                                                                n_inst, inst_ptr_dev, cu, wt);
+  QHAP_LAUNCH_CHECK();
+  return QHAP_OK;
+}
+
+}  // namespace
+
+qhap_status cut_from_spins(const CsrView& g, int mode, const int8_t* spins, int32_t R, int32_t n_inst,
+                           const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream) {
+  return launch_cut<int8_t>(g, mode, spins, R, n_inst, inst_ptr_dev, cut, wtot, stream);
+}
+
+qhap_status cut_from_x(const CsrView& g, int mode, const float* x, int32_t R, int32_t n_inst,
+                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream) {
+  return launch_cut<float>(g, mode, x, R, n_inst, inst_ptr_dev, cut, wtot, stream);
+}
+
+qhap_status cut_finalize(int32_t n_inst, int32_t R, const int64_t* cut, const int64_t* wtot, int64_t* energy,
+                         int64_t* best_cut, int32_t* best_replica, cudaStream_t stream) {
+  if (n_inst == 0) return QHAP_OK;
+  cut_finalize_kernel<<<n_inst, 256, 0, stream>>>(R, reinterpret_cast<const long long*>(cut),
+                                                  reinterpret_cast<const long long*>(wtot),
+                                                  reinterpret_cast<long long*>(energy),
+                                                  reinterpret_cast<long long*>(best_cut), best_replica);
+  QHAP_LAUNCH_CHECK();
+  return QHAP_OK;
+}
+
+qhap_status gather_best_spins(int32_t n, int32_t R, const float* x, int32_t n_inst, const int32_t* inst_ptr_dev,
+                              const int32_t* best_replica, int8_t* best_spins, cudaStream_t stream) {
+  if (n == 0) return QHAP_OK;
+  gather_best_spins_kernel<<<int(ceil_div(n, 256)), 256, 0, stream>>>(n, R, x, n_inst, inst_ptr_dev, best_replica,
+                                                                    best_spins);
+  QHAP_LAUNCH_CHECK();
+  return QHAP_OK;
+}
+
+}  // namespace qhap

@@ -1,0 +1,315 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle, element by element
+on the same seeded inputs.  Bars (BASELINE.json north_star): graph builds and cut evaluation bit-exact; bSB trajectories
+max |dx|, |dy| <= 1e-3 over the first 50 steps; best cut >= oracle - 0.5 %; switch error <= oracle + 0.1 pp.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2603_25762_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TRAJ_TOL = 1e-3          # north_star
+WALL_BAND = 1e-4         # |x_pre| within this of 1.0: the wall decision may legitimately differ
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests selected (-m gpu) but no CUDA device is visible"
+    from paper_2603_25762_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    return torch
+
+
+def porec_like(seed, n_snp=400, n_reads=120):
+    base = synth.make_fragments(seed=seed, L=400_000, n_snp=n_snp, n_reads=n_reads, len_law=("uniform", 8_000, 30_000),
+                                flip=0.05, missing=0.05, qual=("normal", 18, 5, 3, 40))
+    pc = synth.make_porec_fragments(seed=seed + 1, base=base, L=400_000, flip=0.05, qual=("normal", 18, 5, 3, 40),
+                                    target_edges=300, batch=64, d_min=5e3, d_max=3e5)
+    return synth.merge_fragments(base, pc)
+
+
+def assert_csr_equal(got: dict, exp: dict, keys):
+    assert got["n"] == exp["n"] and got["nnz"] == exp["nnz"], (got["n"], exp["n"], got["nnz"], exp["nnz"])
+    for k in ("row_ptr", "col") + tuple(keys):
+        assert np.array_equal(got[k], exp[k]), k
+
+
+# ------------------------------------------------------------------------------------------ (1) read graph
+@pytest.mark.parametrize("case", ["cfg0", "tiny-missing", "cfg2-scaled", "porec", "cfg1-scaled"])
+def test_read_graph_bit_exact(B, oracle, case):
+    if case == "cfg0":
+        fr, _ = synth.make_config(0)
+    elif case == "tiny-missing":
+        fr = synth.make_fragments(seed=5, L=40_000, n_snp=40, n_reads=30, len_law=("uniform", 4_000, 15_000), flip=0.1,
+                                  missing=0.2, qual=("normal", 20, 8, 1, 60))
+    elif case == "cfg2-scaled":
+        fr, _ = synth.make_config(2, scale=0.05)
+    elif case == "cfg1-scaled":
+        fr, _ = synth.make_config(1, scale=0.1)
+    else:
+        fr = porec_like(77)
+    exp = oracle.read_graph(fr)
+    dfr = B.upload_frags(fr)
+    for mode, dd in ((0, B.QHAP_DENSE_FP16), (1, B.QHAP_DENSE_FP16), (1, B.QHAP_DENSE_BF16)):
+        g, J = B.qhap_build_read_graph(dfr, weight_mode=mode, dense_dtype=dd)
+        assert_csr_equal(g.to_host(), exp, ("d", "c"))
+        # dense J = -w exactly, zero elsewhere (including the padding)
+        w = oracle.read_weights(exp, mode)
+        Jexp = np.zeros(J.shape, np.float64)
+        rows = np.repeat(np.arange(exp["n"]), np.diff(exp["row_ptr"]))
+        Jexp[rows, exp["col"]] = -w
+        assert np.array_equal(J.float().cpu().numpy().astype(np.float64), Jexp)
+
+
+def test_read_graph_rejects_unsorted(B):
+    fr, _ = synth.make_config(0)
+    # swap the first two fragments' order by rebuilding the CSR reversed
+    order = np.arange(fr.n_frag)[::-1]
+    cnt = np.diff(fr.frag_ptr)[order]
+    ptr = np.concatenate([[0], np.cumsum(cnt)]).astype(np.int64)
+    src = np.concatenate([np.arange(fr.frag_ptr[i], fr.frag_ptr[i + 1]) for i in order])
+    fr2 = synth.Fragments(fr.n_frag, fr.n_snp, ptr, fr.snp_idx[src], fr.allele[src], fr.qual[src], fr.frag_flags[order],
+                          fr.h1, fr.hap_a, fr.frag_hap[order], fr.snp_pos)
+    with pytest.raises(B.QhapError) as ei:
+        B.qhap_build_read_graph(B.upload_frags(fr2))
+    assert ei.value.status == B.QHAP_ERR_INVALID_ARG
+
+
+def test_read_graph_dense_range_error(B):
+    """|w| > 256 is not exact in bf16 -> QHAP_ERR_RANGE, never silent rounding."""
+    n_snp, k = 600, 2
+    ptr = np.array([0, n_snp, 2 * n_snp], np.int64)
+    idx = np.tile(np.arange(n_snp, dtype=np.int32), k)
+    al = np.concatenate([np.zeros(n_snp, np.uint8), np.ones(n_snp, np.uint8)])
+    fr = synth.Fragments(2, n_snp, ptr, idx, al, np.full(2 * n_snp, 30, np.uint8), np.zeros(2, np.uint8),
+                         np.zeros(n_snp, np.uint8), np.zeros(n_snp, np.uint8), np.zeros(2, np.uint8), np.arange(n_snp, dtype=np.int64))
+    dfr = B.upload_frags(fr)
+    g, J = B.qhap_build_read_graph(dfr, weight_mode=0, dense_dtype=B.QHAP_DENSE_FP16)
+    assert g.d.cpu().tolist() == [600, 600] and float(J[0, 1]) == -600.0
+    with pytest.raises(B.QhapError) as ei:
+        B.qhap_build_read_graph(dfr, weight_mode=0, dense_dtype=B.QHAP_DENSE_BF16)
+    assert ei.value.status == B.QHAP_ERR_RANGE
+
+
+# ------------------------------------------------------------------------------------------- (2) SNP graph
+@pytest.mark.parametrize("case,tenths", [("tiny", 10), ("tiny", 3), ("cfg3-scaled", 3), ("cfg3-scaled", 10), ("porec", 3),
+                                         ("cfg2-scaled", 10)])
+def test_snp_graph_bit_exact(B, oracle, case, tenths):
+    if case == "tiny":
+        fr = synth.make_fragments(seed=5, L=40_000, n_snp=50, n_reads=40, len_law=("uniform", 4_000, 15_000), flip=0.1,
+                                  missing=0.1, qual=("normal", 20, 8, 1, 60))
+        fr.h1 = np.random.default_rng(1).integers(0, 2, fr.n_snp).astype(np.uint8)
+    elif case == "cfg3-scaled":
+        fr, _ = synth.make_config(3, scale=0.01)
+    elif case == "cfg2-scaled":
+        fr, _ = synth.make_config(2, scale=0.03)      # long rows: > 85 partners -> the 1024-slot table class
+    else:
+        fr = porec_like(78)
+    exp = oracle.snp_graph(fr, tenths, 0.1)
+    g = B.qhap_build_snp_graph(B.upload_frags(fr), tenths, 0.1, llr_table=oracle.llr_table())
+    assert_csr_equal(g.to_host(), exp, ("w_fx", "w"))
+    # the library's own table (C library pow/log10 on this box) gives the same bits
+    g2 = B.qhap_build_snp_graph(B.upload_frags(fr), tenths, 0.1)
+    assert_csr_equal(g2.to_host(), exp, ("w_fx", "w"))
+
+
+def test_block_split_and_stitch_bit_exact(B, oracle, torch_mod):
+    fr, p = synth.make_config(3, scale=0.01)
+    exp_g = oracle.snp_graph(fr, 3, 0.1)
+    win = synth.block_windows(fr.n_snp, 500, 450)
+    exp = oracle.block_split(exp_g, win)
+    g = B.upload_csr(exp_g)
+    got = B.qhap_block_split(g, win)
+    assert_csr_equal(got.to_host(), exp, ("w_fx", "w"))
+    assert np.array_equal(got.inst_ptr, exp["inst_ptr"])
+    rng = np.random.default_rng(0)
+    blocks = [np.where(rng.integers(0, 2, hi - lo) == 1, 1, -1).astype(np.int8) for lo, hi in win.tolist()]
+    exp_s = oracle.block_stitch(fr.n_snp, win, blocks)
+    got_s = B.qhap_block_stitch(fr.n_snp, win, torch_mod.from_numpy(np.concatenate(blocks)).cuda())
+    assert np.array_equal(got_s.cpu().numpy(), exp_s)
+
+
+# ------------------------------------------------------------------------------------------ (5) cut / energy
+@pytest.mark.parametrize("R", [1, 5, 64, 200])
+def test_cut_eval_bit_exact(B, oracle, torch_mod, R):
+    fr, _ = synth.make_config(0)
+    rg = oracle.read_graph(fr)
+    sg = oracle.snp_graph(fr, 10, 0.1)
+    for g, modes in ((rg, (0, 1)), (sg, (2,))):
+        dg = B.upload_csr(g)
+        s = synth.random_spins(R, g["n"], R)
+        for mode in modes:
+            w = g["w_fx"] if mode == 2 else oracle.read_weights(g, mode)
+            ecut, een = oracle.cut_eval(g["row_ptr"], g["col"], w, s)
+            cut, en = B.qhap_cut_eval(dg, mode, torch_mod.from_numpy(s).cuda())
+            assert np.array_equal(cut.cpu().numpy(), ecut) and np.array_equal(en.cpu().numpy(), een)
+
+
+def test_cut_eval_empty_graph(B, torch_mod):
+    g = B.Csr(3, 0, torch_mod.zeros(4, dtype=torch_mod.int32, device="cuda"), torch_mod.zeros(1, dtype=torch_mod.int32, device="cuda"),
+              torch_mod.zeros(1, dtype=torch_mod.int32, device="cuda"), torch_mod.zeros(1, dtype=torch_mod.int32, device="cuda"))
+    cut, en = B.qhap_cut_eval(g, 0, torch_mod.ones((3, 4), dtype=torch_mod.int8, device="cuda"))
+    assert cut.cpu().tolist() == [0, 0, 0, 0] and en.cpu().tolist() == [0, 0, 0, 0]
+
+
+# ------------------------------------------------------------------------------------------ (3)(4) bSB steps
+def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, steps=50, path=2, dense_J=None, inst_ptr=None,
+                       c0=None, tile_skip=0):
+    """Step both sides from identical fp32 initial states; after every step compare x and y (north_star: <= 1e-3).
+    A (spin, replica) whose oracle pre-clamp |x| lies within WALL_BAND of 1 may take the other wall decision; its y is then
+    excluded for that step (x still agrees to ~WALL_BAND).  Returns the maxima and the number of excluded entries."""
+    jval = (-(g["w"] if mode == 2 else w_int)).astype(np.float32)
+    x0, y0 = synth.bsb_init_state(seed, n, R)
+    dg = B.upload_csr(dict(g, inst_ptr=inst_ptr))
+    xg = torch_mod.from_numpy(x0.copy()).cuda(); yg = torch_mod.from_numpy(y0.copy()).cuda()
+    ws = None
+    if inst_ptr is None:
+        inst = [(0, n)]
+    else:
+        inst = [(int(inst_ptr[b]), int(inst_ptr[b + 1])) for b in range(len(inst_ptr) - 1)]
+    xo = x0.astype(np.float64); yo = y0.astype(np.float64)
+    xpre = np.zeros_like(xo)
+    subs = []
+    for lo, hi in inst:      # per-instance CSR for the oracle (block-diagonal -> local columns)
+        rp = (g["row_ptr"][lo:hi + 1] - g["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(g["row_ptr"][lo]), int(g["row_ptr"][hi]))
+        subs.append((rp, (g["col"][sl] - lo).astype(np.int32), jval[sl]))
+    mdx = mdy = 0.0
+    excluded = 0
+    for k in range(steps):
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, step_begin=k, steps_run=1, weight_mode=mode, path=path, x=xg, y=yg,
+                               dense_J=dense_J, finalize=False, workspace=ws, c0=c0 or 0.0, tile_skip=tile_skip)
+        ws = res["workspace"]
+        for (lo, hi), (rp, cl, jv) in zip(inst, subs):
+            xs, ys, xp = xo[lo:hi].copy(), yo[lo:hi].copy(), np.zeros((hi - lo, R))
+            oracle.bsb_run(rp, cl, jv, xs, ys, steps_total=T, step_begin=k, steps_run=1, n_threads=8, xpre=xp, c0=c0)
+            xo[lo:hi], yo[lo:hi], xpre[lo:hi] = xs, ys, xp
+        xh, yh = xg.cpu().numpy().astype(np.float64), yg.cpu().numpy().astype(np.float64)
+        marginal = np.abs(np.abs(xpre) - 1.0) < WALL_BAND
+        dx = np.abs(xh - xo).max()
+        dy = np.abs(np.where(marginal, 0.0, yh - yo)).max()
+        mdx, mdy = max(mdx, dx), max(mdy, dy)
+        excluded += int(marginal.sum())
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, f"step {k}: max|dx| {dx:.3e}, max|dy| {dy:.3e}"
+    assert excluded <= 1e-3 * n * R * steps
+    return mdx, mdy, excluded
+
+
+def test_init_state_matches_generator(B, oracle, torch_mod):
+    fr, p = synth.make_config(0)
+    g = oracle.read_graph(fr)
+    res = B.qhap_bsb_solve(B.upload_csr(g), replicas=64, steps_total=10, steps_run=0, seed=p["seed"], weight_mode=1, finalize=False)
+    x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, 64)
+    assert np.array_equal(res["x"].cpu().numpy(), x0) and np.array_equal(res["y"].cpu().numpy(), y0)
+
+
+@pytest.mark.parametrize("R", [64, 6, 3])
+def test_sparse_trajectory_cfg0(B, oracle, torch_mod, R):
+    fr, p = synth.make_config(0)
+    g = oracle.read_graph(fr)
+    for mode in (0, 1):
+        w = oracle.read_weights(g, mode)
+        mdx, mdy, exc = compare_trajectory(B, oracle, torch_mod, g, w, mode, fr.n_frag, R, p["T"], p["seed"])
+        print(f"cfg0 sparse mode {mode} R {R}: max|dx| {mdx:.2e} max|dy| {mdy:.2e} excluded {exc}")
+
+
+def test_sparse_trajectory_snp_graph_batched(B, oracle, torch_mod):
+    """cfg3-like: block-diagonal batch of instances with per-instance c0, R = 256 (float4 path)."""
+    fr, p = synth.make_config(3, scale=0.01)
+    g = oracle.snp_graph(fr, 3, 0.1)
+    win = synth.block_windows(fr.n_snp, 500, 450)
+    bs = oracle.block_split(g, win)
+    mdx, mdy, exc = compare_trajectory(B, oracle, torch_mod, bs, bs["w_fx"], 2, bs["n"], 256, p["T"], p["seed"], steps=50,
+                                       inst_ptr=bs["inst_ptr"])
+    print(f"cfg3-scaled batched: max|dx| {mdx:.2e} max|dy| {mdy:.2e} excluded {exc}")
+
+
+def test_sparse_trajectory_cfg1_scaled(B, oracle, torch_mod):
+    fr, p = synth.make_config(1, scale=0.1)
+    g = oracle.read_graph(fr)
+    w = oracle.read_weights(g, 1)
+    mdx, mdy, exc = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, 128, p["T"], p["seed"])
+    print(f"cfg1-scaled sparse: max|dx| {mdx:.2e} max|dy| {mdy:.2e} excluded {exc}")
+
+
+# -------------------------------------------------------------------------------- full solve: quality and phasing
+def ser_reads(oracle, fr, spins):
+    m = oracle.switch_hamming(oracle.read_vote(fr, spins), fr.hap_a)
+    return m["se"], m["he"]
+
+
+def test_solve_cfg0_quality_and_readout(B, oracle, torch_mod):
+    """Full cfg0 solve on the GPU vs the oracle with the same seeds and replica count."""
+    fr, p = synth.make_config(0)
+    g = oracle.read_graph(fr)
+    dfr = B.upload_frags(fr)
+    for mode in (0, 1):
+        w = oracle.read_weights(g, mode)
+        x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, p["R"])
+        ores = oracle.solve(g["row_ptr"], g["col"], w, (-w).astype(np.float32), x0, y0, steps_total=p["T"], n_threads=8)
+        dg, _ = B.qhap_build_read_graph(dfr, weight_mode=mode)
+        res = B.qhap_bsb_solve(dg, replicas=p["R"], steps_total=p["T"], seed=p["seed"], weight_mode=mode)
+        gcut = int(res["best_cut"].cpu()[0]); ocut = ores["best_cut"]
+        assert gcut >= ocut - 0.005 * abs(ocut), (gcut, ocut)
+        # the reported cut is the cut of the reported spins (bit-exact, oracle's evaluation)
+        spins = res["best_spins"].cpu().numpy()
+        ccut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, spins)
+        assert ccut[0] == gcut
+        cuts = res["cut"].cpu().numpy()[0]
+        r = int(res["best_replica"].cpu()[0])
+        assert cuts[r] == gcut == cuts.max() and r == int(np.flatnonzero(cuts == cuts.max())[0])
+        # per-replica cuts equal the oracle's evaluation of sign(x) of the GPU state
+        sx = np.where(res["x"].cpu().numpy() >= 0, 1, -1).astype(np.int8)
+        ecut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, sx)
+        assert np.array_equal(cuts, ecut)
+        # phasing
+        hap = B.qhap_phase_readout_reads(dfr, res["best_spins"]).cpu().numpy()
+        assert np.array_equal(hap, oracle.read_vote(fr, spins))
+        gse, ghe = (lambda m: (m["se"], m["he"]))(oracle.switch_hamming(hap, fr.hap_a))
+        ose, ohe = ser_reads(oracle, fr, ores["best_spins"])
+        print(f"cfg0 mode {mode}: gpu cut {gcut} oracle cut {ocut}; SE gpu {gse:.4f} oracle {ose:.4f}")
+        assert gse <= ose + 0.001
+
+
+def test_solve_snp_blocks_quality(B, oracle, torch_mod):
+    """cfg3-like batched blocks: per-instance best cut vs oracle, stitched SER vs oracle's."""
+    fr, p = synth.make_config(3, scale=0.01)
+    dfr = B.upload_frags(fr)
+    g = B.qhap_build_snp_graph(dfr, 3, 0.1)
+    win = synth.block_windows(fr.n_snp, 500, 450)
+    bs = B.qhap_block_split(g, win)
+    R, T = 64, 400
+    res = B.qhap_bsb_solve(bs, replicas=R, steps_total=T, seed=p["seed"], weight_mode=2)
+    hb = bs.to_host()
+    x0, y0 = synth.bsb_init_state(p["seed"], hb["n"], R)
+    gspins = res["best_spins"].cpu().numpy()
+    ospins = np.zeros(hb["n"], np.int8)
+    for b in range(len(win)):
+        lo, hi = int(hb["inst_ptr"][b]), int(hb["inst_ptr"][b + 1])
+        rp = (hb["row_ptr"][lo:hi + 1] - hb["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(hb["row_ptr"][lo]), int(hb["row_ptr"][hi]))
+        cl = (hb["col"][sl] - lo).astype(np.int32)
+        o = oracle.solve(rp, cl, hb["w_fx"][sl], (-hb["w"][sl]).astype(np.float32), x0[lo:hi], y0[lo:hi], steps_total=T, n_threads=8)
+        ospins[lo:hi] = o["best_spins"]
+        gcut = int(res["best_cut"].cpu()[b])
+        assert gcut >= o["best_cut"] - 0.005 * abs(o["best_cut"]), (b, gcut, o["best_cut"])
+        ccut, _ = oracle.cut_eval(rp, cl, hb["w_fx"][sl], gspins[lo:hi])
+        assert ccut[0] == gcut
+    gst = B.qhap_block_stitch(fr.n_snp, win, res["best_spins"]).cpu().numpy()
+    ost = oracle.block_stitch(fr.n_snp, win, [ospins[int(hb["inst_ptr"][b]):int(hb["inst_ptr"][b + 1])] for b in range(len(win))])
+    ghap = B.qhap_phase_readout_snps(dfr.h1, torch_mod.from_numpy(gst).cuda()).cpu().numpy()
+    assert np.array_equal(ghap, oracle.snp_readout(fr.h1, gst))
+    covered = np.bincount(fr.snp_idx[fr.allele <= 1], minlength=fr.n_snp) > 0
+    gm = oracle.switch_hamming(ghap[covered], fr.hap_a[covered])
+    om = oracle.switch_hamming(oracle.snp_readout(fr.h1, ost)[covered], fr.hap_a[covered])
+    print(f"cfg3-scaled: SE gpu {gm['se']:.4f} oracle {om['se']:.4f}")
+    assert gm["se"] <= om["se"] + 0.001

@@ -1,0 +1,357 @@
+#!/usr/bin/env python
+"""bench.py -- QHap hot path on B200: bSB spin-updates/s and phasing wall-time per region (BASELINE.json `metric`).
+
+A "step" is one pass of the whole hot path over one synthetic region:
+  qhap_build_read_graph -> qhap_bsb_solve (T bSB steps x R replicas, cut evaluation, best replica) -> qhap_phase_readout_reads
+on BASELINE.json config 1 (read-based MHC-like region: ~8,000 HiFi-like reads, R = 1,024, T = 2,000) by default.
+`value` = n * R * T * n_gpus / seconds per step with the fragments already resident in HBM; `e2e` is the same call
+sequence fed from pinned HOST buffers (H2D of the fragment matrix and D2H of the haplotype + best cut inside the timed
+region).  N > 1 (torchrun): every rank runs its own R replicas of the same region (weak scaling, no per-step exchange),
+then 16 bytes per rank are all-gathered to pick the global best replica (paper_2603_25762_b200/parallel.py).
+
+`--impl reference` times the fp64 CPU oracle (oracle/, test infrastructure) on the box's host cores on a bounded sample
+of the same workload -- a reported baseline, not the target.
+
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "bsb_spin_updates_per_s"
+UNIT = "spin-updates/s"
+L2_FLUSH_BYTES = 512 << 20
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (1 = the config the metric is quoted on)")
+    ap.add_argument("--path", default="auto", choices=["auto", "dense", "sparse"], help="bSB step kernel (auto = fastest validated)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU seconds of the oracle sample")
+    return ap.parse_args()
+
+
+def workload_name(cfg, fr, p):
+    return (f"BASELINE.json configs[{cfg}] {p['name']}: {fr.n_frag} fragments x {fr.n_snp} het SNPs, "
+            f"{p['graph']} graph, R={p['R']}, T={p['T']}, dt={p['dt']}, a0={p['a0']}")
+
+
+# ---------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_id: str):
+        self.proc = None
+        self.gpu_id = gpu_id
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", self.gpu_id, f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        d = json.loads(f.read_text())
+        return dict(hbm=float(d["hbm_gbs"]), bf16=float(d["bf16_tflops"]), bf16_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                    which="measured (MEASURED_PEAKS.json)")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, which="fallback (B200_PROFILING.md)")
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def oracle_sample(fr, p, cores, cpu_seconds, R_o=None):
+    """One pass of the path in the fp64 oracle on a bounded sample: full graph build + R_o replicas x T_o steps + cut +
+    vote.  Returns timings; T_o is sized from a 2-step probe so that the bSB part takes about `cpu_seconds`."""
+    from oracle import oracle as O
+    mode = 1
+    t0 = time.perf_counter()
+    if p["graph"] == "read":
+        g = O.read_graph(fr)
+        w_int = O.read_weights(g, mode)
+        jval = (-w_int).astype(np.float32)
+    else:
+        g = O.snp_graph(fr, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
+        w_int = g["w_fx"]
+        jval = (-g["w"]).astype(np.float32)
+    t_build = time.perf_counter() - t0
+    n = g["n"]
+    R_o = R_o or min(p["R"], 16 * cores)
+    from paper_2603_25762_b200 import synth
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R_o)
+    x, y = x0.astype(np.float64), y0.astype(np.float64)
+    t0 = time.perf_counter()
+    O.bsb_run(g["row_ptr"], g["col"], jval, x, y, steps_total=p["T"], step_begin=0, steps_run=2, n_threads=cores)
+    probe = (time.perf_counter() - t0) / 2
+    T_o = int(max(4, min(p["T"] - 2, cpu_seconds / max(probe, 1e-6))))
+    t0 = time.perf_counter()
+    x, y, _ = O.bsb_run(g["row_ptr"], g["col"], jval, x, y, steps_total=p["T"], step_begin=2, steps_run=T_o, n_threads=cores)
+    t_bsb = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    s = O.sign_spins(x)
+    cut, _ = O.cut_eval(g["row_ptr"], g["col"], w_int, s)
+    r = O.best_replica(cut)
+    if p["graph"] == "read":
+        O.read_vote(fr, s[:, r].copy())
+    else:
+        O.snp_readout(fr.h1, s[:, r].copy())
+    t_read = time.perf_counter() - t0
+    return dict(n=n, R_o=R_o, T_o=T_o, t_build=t_build, t_bsb=t_bsb, t_read=t_read, edges=int(g["nnz"]) // 2)
+
+
+def extrapolated(s, p):
+    """spin-updates/s of the whole path at the full R, T from a sample: build + bSB scaled by (R T)/(R_o T_o) + readout."""
+    full = s["t_build"] + s["t_bsb"] * (p["R"] * p["T"]) / (s["R_o"] * s["T_o"]) + s["t_read"] * p["R"] / s["R_o"]
+    return s["n"] * p["R"] * p["T"] / full, full
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2603_25762_b200 import synth
+    from oracle import oracle as O
+    O.build()
+    cores = O.hardware_threads()
+    fr, p = synth.make_config(args.config)
+    per_step = max(2.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
+    times, samples = [], []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        s = oracle_sample(fr, p, cores, per_step)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt); samples.append(s)
+    vals = [extrapolated(s, p) for s in samples]
+    value = float(np.mean([v[0] for v in vals]))
+    s = samples[-1]
+    sample = (f"per step: full graph build + {s['R_o']} of {p['R']} replicas x {s['T_o']} of {p['T']} bSB steps + cut + readout; "
+              f"value = n R T / (t_build + t_bsb (R T)/(R_o T_o) + t_readout R/R_o)")
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(args.config, fr, p), "sampled": sample},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "region_s_extrapolated": float(np.mean([v[1] for v in vals])), "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2603_25762_b200 import binding as B, parallel, synth
+
+    rank, world, local = parallel.init_from_env()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    fr, p = synth.make_config(args.config)
+    assert p["graph"] == "read", "bench.py times the read-based configs (0-2); the SNP configs are parity-test cases"
+    mode = B.QHAP_WEIGHT_D_MINUS_C            # BASELINE.json: "discordant minus concordant"
+    n, R, T = fr.n_frag, p["R"], p["T"]
+    seed = parallel.rank_seed(p["seed"], rank)
+    path = {"auto": 2, "sparse": 2, "dense": 1}[args.path]
+    dense_dtype = B.QHAP_DENSE_FP16 if path == 1 else B.QHAP_DENSE_NONE
+
+    dfr = B.upload_frags(fr)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    state = {}
+
+    def one_pass(frags):
+        g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype)
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J,
+                               cut_per_replica=False, workspace=state.get("ws"))
+        state["ws"] = res["workspace"]
+        cut, spins = res["best_cut"], res["best_spins"]
+        if world > 1:
+            cut, spins, _ = parallel.select_best_across_ranks(cut, spins)
+        hap = B.qhap_phase_readout_reads(frags, spins)
+        state["g"] = g
+        return cut, hap
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, warmup, steps):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        launches0 = 0
+        barrier()
+        for it in range(warmup + steps):
+            flush.zero_()                                   # L2 flush between iterations (outside the event pairs)
+            if it == warmup:
+                barrier()
+                launches0 = B.qhap_launch_count()
+            if it >= warmup:
+                ev[it - warmup][0].record()
+            fn()
+            if it >= warmup:
+                ev[it - warmup][1].record()
+        barrier()
+        launches = B.qhap_launch_count() - launches0
+        ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, launches
+
+    props = torch.cuda.get_device_properties(local)
+    gpu_id = str(local)
+    try:
+        u = str(props.uuid)
+        gpu_id = u if u.startswith("GPU-") else "GPU-" + u
+    except Exception:
+        pass
+    sampler = ClockSampler(gpu_id)
+    sampler.start()
+    ms, launches = timed(lambda: one_pass(dfr), args.warmup, args.steps)
+    clocks = sampler.stop()
+    value = n * R * T * world / (ms * 1e-3)
+    g = state["g"]
+    edges = g.nnz // 2
+
+    # ---- e2e: the same pass fed from pinned host buffers, result read back to the host
+    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(fr, k), dtype=dt)).pin_memory()
+            for k, dt in (("frag_ptr", np.int64), ("snp_idx", np.int32), ("allele", np.uint8), ("qual", np.uint8))}
+    dbuf = {k: torch.empty_like(v, device=dev) for k, v in host.items()}
+    hap_host = torch.empty(fr.n_snp, dtype=torch.int8).pin_memory()
+    cut_host = torch.empty(1, dtype=torch.int64).pin_memory()
+    h2d = sum(v.numel() * v.element_size() for v in host.values())
+    d2h = hap_host.numel() + 8
+
+    def e2e_pass():
+        for k in host:
+            dbuf[k].copy_(host[k], non_blocking=True)
+        frags = B.Frags(fr.n_frag, fr.n_snp, fr.nnz, dbuf["frag_ptr"], dbuf["snp_idx"], dbuf["allele"], dbuf["qual"], None, None)
+        cut, hap = one_pass(frags)
+        hap_host.copy_(hap, non_blocking=True)
+        cut_host.copy_(cut, non_blocking=True)
+
+    e2e_ms, _ = timed(e2e_pass, max(1, min(args.warmup, 2)), max(2, min(args.steps, 3)))
+    e2e_value = n * R * T * world / (e2e_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (the bSB step): T launches timed with CUDA events on the launching stream
+    J = None
+    if path == 1:
+        _, J = B.qhap_build_read_graph(dfr, weight_mode=mode, dense_dtype=dense_dtype)
+    res0 = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=0, seed=seed, weight_mode=mode, path=path, dense_J=J, finalize=False)
+    x, y = res0["x"], res0["y"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    l0 = B.qhap_launch_count()
+    e0.record()
+    B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=T, weight_mode=mode, path=path, x=x, y=y, dense_J=J, finalize=False,
+                     workspace=state.get("ws"))
+    e1.record()
+    torch.cuda.synchronize()
+    step_launches = B.qhap_launch_count() - l0
+    step_ms = e0.elapsed_time(e1) / T
+    peaks = measured_peaks()
+    if path == 2:
+        # algorithmic bytes per launch: 16 B of fp32 state per spin-update (read x, read y, write y,
+        # write x') + the CSR once per launch (int32 col + fp32 val per directed entry, int32 row_ptr per row)
+        alg_bytes = 16.0 * n * R + 8.0 * g.nnz + 4.0 * (n + 1)
+        roofline = {"kernel": "sparse_step_kernel", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
+                    "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms, "peak_source": peaks["which"]}
+    else:
+        n_pad = (n + 127) // 128 * 128
+        terms = 2
+        alg_flops = 2.0 * n_pad * n_pad * R * terms
+        roofline = {"kernel": "dense_step_kernel", "bound": "tensor", "achieved": alg_flops / (step_ms * 1e-3) / 1e12,
+                    "peak": peaks["bf16_sustained"], "unit": "TFLOP/s", "traffic": None, "flops_per_launch": alg_flops,
+                    "launch_ms": step_ms, "peak_source": peaks["which"] + ", sustained bf16 x 1.0 (fp16 = same kind::f16 rate)"}
+    roofline["frac"] = roofline["achieved"] / roofline["peak"]
+    prof = ROOT / "profiles" / "roofline_traffic.json"              # dram bytes per launch from the committed ncu capture
+    if prof.exists():
+        try:
+            roofline["traffic"] = json.loads(prof.read_text()).get(roofline["kernel"])
+        except Exception:
+            pass
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": workload_name(args.config, fr, p), "path": {1: "dense-tcgen05", 2: "sparse-csr"}[path],
+                      "weight_mode": "D-C", "replicas_per_gpu": R, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
+                      "parallelism": f"replicas x{world} (weak)"},
+           "region_ms": ms, "edges_replicas_per_s": edges * R * T * world / (ms * 1e-3), "undirected_edges": edges,
+           "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+           "gpu_launches": int(launches), "bsb_step_launches_per_solve": int(step_launches),
+           "clocks": clocks, "roofline": roofline, "library": B.qhap_version()}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as O
+        O.build()
+        cores = O.hardware_threads()
+        s = oracle_sample(fr, p, cores, args.cpu_seconds)
+        v, full = extrapolated(s, p)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": (f"full graph build ({s['t_build']:.2f} s) + {s['R_o']} of {R} replicas x {s['T_o']} of {T} bSB steps "
+                                          f"({s['t_bsb']:.2f} s) + cut + readout ({s['t_read']:.2f} s), extrapolated to R x T"),
+                               "bsb_only_value": s["n"] * s["R_o"] * s["T_o"] / s["t_bsb"], "region_s_extrapolated": full}
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -153,6 +153,9 @@ QHAP_API qhap_status qhap_block_stitch(int32_t n, int32_t n_blocks, const int64_
                               int8_t *out, void *workspace, size_t *ws_bytes, void *stream);
 
 QHAP_API const char *qhap_last_error(void);
+/* Number of CUDA kernels this library has launched in this process so far (monotonic; bench.py reports the difference
+ * over its timed region as "gpu_launches"). */
+QHAP_API uint64_t qhap_launch_count(void);
 /* Library / build identification, e.g. "qhap-b200 0.1 sm_100a". */
 QHAP_API const char *qhap_version(void);
 

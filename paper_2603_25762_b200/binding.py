@@ -25,7 +25,7 @@ QHAP_DENSE_NONE, QHAP_DENSE_FP16, QHAP_DENSE_BF16 = 0, 1, 2
 
 EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_bsb_solve", "qhap_cut_eval",
            "qhap_phase_readout_reads", "qhap_phase_readout_snps", "qhap_block_split", "qhap_block_stitch",
-           "qhap_last_error", "qhap_version"]
+           "qhap_last_error", "qhap_launch_count", "qhap_version"]
 
 
 class _Frags(C.Structure):
@@ -50,6 +50,7 @@ for _name in EXPORTS[:8]:
     getattr(_lib, _name).restype = C.c_int
 _lib.qhap_last_error.restype = C.c_char_p
 _lib.qhap_version.restype = C.c_char_p
+_lib.qhap_launch_count.restype = C.c_uint64
 
 
 class QhapError(RuntimeError):
@@ -60,6 +61,10 @@ class QhapError(RuntimeError):
 
 def qhap_version() -> str:
     return _lib.qhap_version().decode()
+
+
+def qhap_launch_count() -> int:
+    return int(_lib.qhap_launch_count())
 
 
 def qhap_last_error() -> str:

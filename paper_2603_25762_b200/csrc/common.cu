@@ -3,6 +3,8 @@
 
 #include <stdarg.h>
 
+#include <atomic>
+
 namespace qhap {
 
 static thread_local char g_err[512] = "";
@@ -13,6 +15,9 @@ void set_error(const char* fmt, ...) {
   vsnprintf(g_err, sizeof(g_err), fmt, ap);
   va_end(ap);
 }
+
+static std::atomic<uint64_t> g_launches{0};
+void count_launches(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 static int g_dev_checked = 0;  // 0 unknown, 1 ok, -1 bad
 static int g_sm_count = 0;
@@ -103,4 +108,5 @@ qhap_status exclusive_scan_i32(const int32_t* in, int32_t* out, int64_t n, int64
 }  // namespace qhap
 
 extern "C" const char* qhap_last_error(void) { return qhap::g_err; }
+extern "C" uint64_t qhap_launch_count(void) { return qhap::g_launches.load(std::memory_order_relaxed); }
 extern "C" const char* qhap_version(void) { return "qhap-b200 0.1 sm_100a"; }

@@ -37,7 +37,14 @@ void set_error(const char* fmt, ...);
     }                                  \
   } while (0)
 
-#define QHAP_LAUNCH_CHECK() QHAP_CUDA_TRY(cudaGetLastError())
+// Every kernel launch of the library is followed by QHAP_LAUNCH_CHECK(): it counts the launch (qhap_launch_count) and
+// turns a launch error into QHAP_ERR_CUDA.
+void count_launches(uint64_t n);
+#define QHAP_LAUNCH_CHECK()                 \
+  do {                                      \
+    ::qhap::count_launches(1);              \
+    QHAP_CUDA_TRY(cudaGetLastError());      \
+  } while (0)
 
 // sm_100 present?  (cached per process)
 qhap_status require_device();

@@ -113,7 +113,7 @@ typedef struct {
   int32_t tile_skip;    /* dense path: 1 = skip all-zero 64-column blocks of J (bit-identical result)     */
   int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
   int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */
-  int32_t reserved;
+  int32_t dense_bn;     /* dense path: tile width in output spins (multiple of 16 in 16..256); 0 = automatic          */
 } qhap_bsb_params;
 
 /* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`

@@ -1,14 +1,425 @@
-// (3) Dense bSB step on the tensor cores (tcgen05 / TMEM / TMA).  Placeholder until the kernel lands.
+// (3) Dense bSB step on the 5th-generation tensor cores: F = J X for all replicas as a tcgen05 GEMM with TMEM
+// accumulators fed by TMA, with the y/x update, the a(t) ramp and the inelastic wall fused into the epilogue.
+// PAPER.md:L252-L265 [Eq. 4-6] (the solver), L235-L246 (J = -w of the read graph); recurrence: DESIGN.md R10a-f.
+//
+// GEMM orientation: D[r][i] = sum_k xs[r][k] J[i][k], i.e.
+//   A (M side) = replicas: the fp16 split copies x_hi, x_lo of the state, stored [R][n_k] (spin index contiguous = K-major);
+//   B (N side) = output spins: rows of J (fp16, integers exact to 2048), row-major [ld][ld] (K-major);
+//   D in TMEM: lane = replica, column = spin  ->  the epilogue's fp32 state accesses x[i][r], y[i][r] are coalesced
+//   across the 32 lanes of a warp without any shared-memory transpose.
+// x is carried in fp32; the tensor cores see x = x_hi + x_lo (two fp16 terms, |x - x_hi - x_lo| <= 2^-25 for |x| <= 1),
+// both terms accumulate into the same fp32 TMEM tile against the same J tile in shared memory.
+// Jacobi update across CTAs: the fp16 copies are double-buffered (read buffer b, write buffer 1-b); fp32 x, y are
+// private to the tile that owns them and are updated in place.  One launch per step (grid-wide step boundary).
+//
+// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one elected lane),
+// warps 2..9 = epilogue (TMEM lane quarter = warp % 4, two warps per quarter interleave 32-column chunks).
+// Pipelines: kStages shared-memory stages (full/empty mbarriers) and 2 TMEM accumulator stages (tmem_full/tmem_empty).
+#include <cuda.h>
+#include <cuda_fp16.h>
+
+#include <vector>
+
 #include "kernels.cuh"
+#include "sm100_ptx.cuh"
 
 namespace qhap {
 
-size_t dense_workspace_bytes(int32_t, int32_t, int32_t) { return 256; }
+namespace {
 
-qhap_status dense_solve_steps(const CsrView&, const void*, int32_t, int32_t, int32_t, const float*, const qhap_bsb_params&,
-                              float*, float*, void*, size_t, cudaStream_t) {
-  set_error("dense tcgen05 path not built in this revision");
-  return QHAP_ERR_INVALID_ARG;
+constexpr int kBM = 128;                 // replicas per tile (UMMA M)
+constexpr int kBK = 64;                  // spins per k-block: 64 fp16 = one 128-byte swizzle row
+constexpr int kMaxBN = 256;              // output spins per tile (UMMA N), runtime 32..256 in steps of 32
+constexpr int kStages = 3;
+constexpr int kStageJ = kMaxBN * kBK * 2;            // 32 KB
+constexpr int kStageX = kBM * kBK * 2;               // 16 KB each for x_hi, x_lo
+constexpr int kStageBytes = kStageJ + 2 * kStageX;   // 64 KB
+constexpr int kEpiWarps = 8;
+constexpr int kChunk = 16;                // accumulator columns (spins) per tcgen05.ld in the epilogue
+constexpr int kThreads = 64 + 32 * kEpiWarps;
+constexpr int kTmemCols = 512;                       // 2 accumulator stages x 256 columns
+constexpr size_t kSmemBytes = size_t(kStages) * kStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+
+struct DenseArgs {
+  int32_t n, R, n_k;          // spins, replicas, row pitch (elements) of the fp16 copies
+  int32_t BN;                 // tile width in output spins
+  int32_t n_tiles_m, n_tiles_n, n_kblocks;
+  const int32_t* kb_cnt;      // [n_tiles_n] number of listed k-blocks per N tile, or nullptr = all k-blocks
+  const int32_t* kb_idx;      // [n_tiles_n][n_kblocks]
+  const float* c1;            // [1] dt c0
+  float c2, c3;
+  float* x;                   // [n][R] fp32, in place
+  float* y;
+  __half* xh_out;             // [R][n_k] next step's split copies
+  __half* xl_out;
+};
+
+// fp32 -> two fp16 terms.  hi = rn(x); lo = rn(x - hi) (exact difference; lo may be subnormal: absolute error <= 2^-25).
+__device__ __forceinline__ void split_half(float v, __half& hi, __half& lo) {
+  hi = __float2half_rn(v);
+  lo = __float2half_rn(v - __half2float(hi));
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_xh,
+                  const __grid_constant__ CUtensorMap tm_xl, const DenseArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;       // 128B swizzle needs 1024-byte alignment
+  const uint32_t bar_base = smem_base + kStages * kStageBytes;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kStages + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kStages + 2 + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 4);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && ptx::elect_one()) {
+    ptx::prefetch_tensormap(&tm_j);
+    ptx::prefetch_tensormap(&tm_xh);
+    ptx::prefetch_tensormap(&tm_xl);
+    for (int s = 0; s < kStages; ++s) {
+      ptx::mbar_init(full_bar(s), 1);
+      ptx::mbar_init(empty_bar(s), 1);
+    }
+    for (int s = 0; s < 2; ++s) {
+      ptx::mbar_init(tfull_bar(s), 1);
+      ptx::mbar_init(tempty_bar(s), kEpiWarps);
+    }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) ptx::tmem_alloc(tmem_slot, kTmemCols);
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int n_tiles = a.n_tiles_m * a.n_tiles_n;
+  const uint32_t stage_tx = uint32_t(a.BN) * kBK * 2 + 2u * kStageX;
+
+  if (warp == 0) {
+    // ===================================================================================== TMA producer
+    if (ptx::elect_one()) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;      // M fastest: neighbouring CTAs share the J tile in L2
+        const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
+        for (int j = 0; j < nkb; ++j) {
+          const int kb = a.kb_cnt ? a.kb_idx[size_t(tn) * a.n_kblocks + j] : j;
+          ptx::mbar_wait(empty_bar(stage), phase ^ 1);
+          const uint32_t sj = smem_base + stage * kStageBytes;
+          ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx);
+          ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
+          ptx::tma_load_2d(sj + kStageJ, &tm_xh, full_bar(stage), kb * kBK, tm * kBM);
+          ptx::tma_load_2d(sj + kStageJ + kStageX, &tm_xl, full_bar(stage), kb * kBK, tm * kBM);
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ======================================================================================= MMA issuer
+    const uint32_t idesc = ptx::umma_idesc_f16_f32(kBM, uint32_t(a.BN));
+    int stage = 0;
+    uint32_t phase = 0;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int tn = tile / a.n_tiles_m;
+      const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
+      ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);                    // epilogue has drained this accumulator stage
+      ptx::tc_fence_after();
+      const uint32_t d_tmem = tmem_base + uint32_t(acc) * kMaxBN;
+      for (int j = 0; j < nkb; ++j) {
+        ptx::mbar_wait(full_bar(stage), phase);
+        ptx::tc_fence_after();
+        if (ptx::elect_one()) {
+          const uint32_t sj = smem_base + stage * kStageBytes;
+          const uint64_t dj = ptx::umma_desc_k_sw128(sj);
+          const uint64_t dh = ptx::umma_desc_k_sw128(sj + kStageJ);
+          const uint64_t dl = ptx::umma_desc_k_sw128(sj + kStageJ + kStageX);
+#pragma unroll
+          for (int kk = 0; kk < kBK / 16; ++kk) {                         // UMMA_K = 16 for 16-bit inputs: +32 B per step
+            ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+            ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
+          }
+          ptx::umma_commit(empty_bar(stage));                            // frees the smem stage when these MMAs are done
+          if (j == nkb - 1) ptx::umma_commit(tfull_bar(acc));            // accumulator complete -> epilogue
+        }
+        __syncwarp();
+        if (++stage == kStages) { stage = 0; phase ^= 1; }
+      }
+      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    }
+  } else {
+    // ========================================================================================= epilogue
+    const int ew = warp - 2;
+    const int quarter = warp & 3;              // TMEM lanes 32 q .. 32 q + 31 are accessible to warps with warp % 4 == q
+    const int par = ew >> 2;                   // two warps per quarter take alternating 32-column chunks
+    const float c1 = __ldg(a.c1), c2 = a.c2, c3 = a.c3;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+      const int r = tm * kBM + quarter * 32 + lane;
+      const bool r_ok = r < a.R;
+      ptx::mbar_wait(tfull_bar(acc), acc_phase);
+      ptx::tc_fence_after();
+      for (int ch = par; ch * kChunk < a.BN; ch += 2) {
+        const int i0 = tn * a.BN + ch * kChunk;
+        if (i0 >= a.n) break;
+        uint32_t v[kChunk];
+        ptx::tmem_ld_32x32b_x16(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
+        float xv[kChunk], yv[kChunk];
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+          const bool ok = r_ok && (i0 + j) < a.n;
+          const size_t off = size_t(i0 + j) * a.R + r;
+          xv[j] = ok ? a.x[off] : 0.f;
+          yv[j] = ok ? a.y[off] : 0.f;
+        }
+        ptx::tmem_ld_wait();
+        uint32_t hp[kChunk / 2], lp[kChunk / 2];    // fp16 pairs (spin i0 + 2q, i0 + 2q + 1) of x_hi', x_lo'
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+          const bool ok = r_ok && (i0 + j) < a.n;
+          const float F = __uint_as_float(v[j]);
+          float yn = fmaf(c1, F, fmaf(-c2, xv[j], yv[j]));
+          float xn = fmaf(c3, yn, xv[j]);
+          if (fabsf(xn) > 1.0f) {                  // inelastic wall, strict inequality (R10d)
+            xn = copysignf(1.0f, xn);
+            yn = 0.0f;
+          }
+          if (ok) {
+            const size_t off = size_t(i0 + j) * a.R + r;
+            a.x[off] = xn;
+            a.y[off] = yn;
+          }
+          __half h, l;
+          split_half(ok ? xn : 0.f, h, l);
+          const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+          if (j & 1) { hp[j >> 1] |= hb << 16; lp[j >> 1] |= lb << 16; }
+          else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
+        }
+        if (r_ok) {                                 // 32 contiguous bytes per thread; n_k >= round_up(n, 64) keeps it in bounds
+          uint4* ph = reinterpret_cast<uint4*>(a.xh_out + size_t(r) * a.n_k + i0);
+          uint4* pl = reinterpret_cast<uint4*>(a.xl_out + size_t(r) * a.n_k + i0);
+#pragma unroll
+          for (int q = 0; q < kChunk / 8; ++q) {
+            ph[q] = make_uint4(hp[4 * q], hp[4 * q + 1], hp[4 * q + 2], hp[4 * q + 3]);
+            pl[q] = make_uint4(lp[4 * q], lp[4 * q + 1], lp[4 * q + 2], lp[4 * q + 3]);
+          }
+        }
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    }
+  }
+
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc(tmem_base, kTmemCols);
+  }
+}
+
+// x [n][R] fp32 -> split copies [R][n_k] fp16 (transpose through shared memory, 32 x 32 tiles).
+__global__ void __launch_bounds__(256) split_x_kernel(int32_t n, int32_t R, int32_t n_k, const float* __restrict__ x,
+                                                      __half* __restrict__ xh, __half* __restrict__ xl) {
+  __shared__ float t[32][33];
+  const int i0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int j = ty; j < 32; j += 8) {
+    const int i = i0 + j, r = r0 + tx;
+    t[j][tx] = (i < n && r < R) ? x[size_t(i) * R + r] : 0.f;
+  }
+  __syncthreads();
+  for (int j = ty; j < 32; j += 8) {
+    const int r = r0 + j, i = i0 + tx;
+    if (r < R && i < n_k) {
+      __half h, l;
+      split_half(t[tx][j], h, l);
+      xh[size_t(r) * n_k + i] = h;
+      xl[size_t(r) * n_k + i] = l;
+    }
+  }
+}
+
+// tile_skip lists: flag[tn][kb] = 1 iff some row of N tile tn has a non-zero in k-block kb (one warp per row).
+__global__ void __launch_bounds__(256) kb_flag_kernel(int32_t n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
+                                                      int32_t BN, int32_t n_kblocks, int32_t* __restrict__ flag) {
+  const int32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n) return;
+  const int lane = threadIdx.x & 31;
+  int32_t* f = flag + size_t(a / BN) * n_kblocks;
+  for (int32_t e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) f[col[e] / kBK] = 1;
+}
+
+// One CTA per N tile: ascending list of flagged k-blocks (at least one entry, so that every tile produces an accumulator).
+__global__ void __launch_bounds__(32) kb_list_kernel(int32_t n_kblocks, const int32_t* __restrict__ flag, int32_t* __restrict__ kb_cnt,
+                                                     int32_t* __restrict__ kb_idx) {
+  const int tn = blockIdx.x, lane = threadIdx.x;
+  const int32_t* f = flag + size_t(tn) * n_kblocks;
+  int32_t* out = kb_idx + size_t(tn) * n_kblocks;
+  int32_t cnt = 0;
+  for (int32_t base = 0; base < n_kblocks; base += 32) {
+    const int32_t kb = base + lane;
+    const bool on = kb < n_kblocks && f[kb] != 0;
+    const uint32_t m = __ballot_sync(0xffffffffu, on);
+    if (on) out[cnt + __popc(m & ((1u << lane) - 1u))] = kb;
+    cnt += __popc(m);
+  }
+  if (lane == 0) {
+    if (cnt == 0) { out[0] = 0; cnt = 1; }
+    kb_cnt[tn] = cnt;
+  }
+}
+
+// ------------------------------------------------------------------------------------------- host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// 2-D fp16 tensor [outer][inner] with row pitch `pitch` elements; box {64, box_outer}; 128-byte swizzle; OOB -> 0.
+qhap_status make_map(CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer, uint64_t pitch, uint32_t box_outer) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) {
+    set_error("cuTensorMapEncodeTiled not available from the driver");
+    return QHAP_ERR_CUDA;
+  }
+  const cuuint64_t dims[2] = {inner, outer};
+  const cuuint64_t strides[1] = {pitch * 2};
+  const cuuint32_t box[2] = {uint32_t(kBK), box_outer};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    set_error("cuTensorMapEncodeTiled failed with CUresult %d (base %p inner %llu outer %llu pitch %llu)", int(r), base,
+              (unsigned long long)inner, (unsigned long long)outer, (unsigned long long)pitch);
+    return QHAP_ERR_CUDA;
+  }
+  return QHAP_OK;
+}
+
+int32_t pitch_of(int32_t n) { return int32_t(ceil_div(n, 64) * 64); }
+
+// Tile width: full GEMM -> minimise waves x width over the persistent grid; tile_skip -> narrow tiles (the step is then
+// bound by the epilogue's state traffic and balances better with more tiles).
+int32_t choose_bn(int32_t n, int32_t R, bool tile_skip, int32_t forced) {
+  if (forced >= 16 && forced <= kMaxBN && forced % 16 == 0) return forced;
+  if (n <= 16) return 16;
+  const int64_t tm = ceil_div(R, kBM), sms = sm_count();
+  int32_t best = 128;
+  double best_cost = 1e300;
+  for (int32_t bn : {64, 96, 128, 160, 192, 224, 256}) {
+    if (tile_skip && bn > 128) break;
+    const int64_t tiles = tm * ceil_div(n, bn);
+    const double cost = double(ceil_div(tiles, sms)) * (bn + (tile_skip ? 16 : 4));   // + fixed per-tile overhead
+    if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && bn > best)) { best_cost = cost; best = bn; }
+  }
+  return best;
+}
+
+}  // namespace
+
+size_t dense_workspace_bytes(int32_t n, int32_t ld, int32_t R) {
+  (void)ld;
+  Workspace ws(nullptr);
+  const size_t copy = size_t(R) * pitch_of(n);
+  ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy);
+  const size_t n_kb = size_t(ceil_div(n, kBK)), n_tn_max = size_t(ceil_div(n, 32));
+  ws.take<int32_t>(n_tn_max);             // kb_cnt
+  ws.take<int32_t>(n_tn_max * n_kb);      // kb_idx
+  ws.take<int32_t>(n_tn_max * n_kb);      // flags
+  return ws.used();
+}
+
+qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld, int32_t dtype, int32_t R, const float* c1_dev,
+                              const qhap_bsb_params& p, float* x, float* y, void* ws_ptr, size_t ws_bytes, cudaStream_t stream) {
+  const int32_t n = g.n;
+  QHAP_REQUIRE(dtype == QHAP_DENSE_FP16, "dense path takes J in fp16");
+  QHAP_REQUIRE((reinterpret_cast<uintptr_t>(dense_J) & 15) == 0, "dense_J must be 16-byte aligned");
+  QHAP_REQUIRE(ws_bytes >= dense_workspace_bytes(n, ld, R), "dense workspace too small");
+  Workspace ws(ws_ptr);
+  const int32_t n_k = pitch_of(n);
+  const size_t copy = size_t(R) * n_k;
+  __half* xh[2];
+  __half* xl[2];
+  xh[0] = ws.take<__half>(copy); xl[0] = ws.take<__half>(copy);
+  xh[1] = ws.take<__half>(copy); xl[1] = ws.take<__half>(copy);
+  const int32_t n_kb = int32_t(ceil_div(n, kBK));
+  const size_t n_tn_max = size_t(ceil_div(n, 32));
+  int32_t* kb_cnt = ws.take<int32_t>(n_tn_max);
+  int32_t* kb_idx = ws.take<int32_t>(n_tn_max * n_kb);
+  int32_t* flags = ws.take<int32_t>(n_tn_max * n_kb);
+
+  const bool skip = p.tile_skip != 0;
+  const int32_t BN = choose_bn(n, R, skip, p.dense_bn);
+  DenseArgs a;
+  a.n = n; a.R = R; a.n_k = n_k; a.BN = BN;
+  a.n_tiles_m = int32_t(ceil_div(R, kBM));
+  a.n_tiles_n = int32_t(ceil_div(n, BN));
+  a.n_kblocks = n_kb;
+  a.kb_cnt = skip ? kb_cnt : nullptr;
+  a.kb_idx = skip ? kb_idx : nullptr;
+  a.c1 = c1_dev;
+  a.x = x; a.y = y;
+
+  static bool attr_set = false;
+  if (!attr_set) {
+    QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
+    attr_set = true;
+  }
+
+  CUtensorMap tm_j, tm_h[2], tm_l[2];
+  QHAP_TRY(make_map(&tm_j, dense_J, uint64_t(ld), uint64_t(ld), uint64_t(ld), uint32_t(BN)));
+  for (int b = 0; b < 2; ++b) {
+    QHAP_TRY(make_map(&tm_h[b], xh[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
+    QHAP_TRY(make_map(&tm_l[b], xl[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
+  }
+
+  {
+    dim3 grid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
+    split_x_kernel<<<grid, 256, 0, stream>>>(n, R, n_k, x, xh[0], xl[0]);
+    QHAP_LAUNCH_CHECK();
+  }
+  if (skip) {
+    QHAP_CUDA_TRY(cudaMemsetAsync(flags, 0, sizeof(int32_t) * size_t(a.n_tiles_n) * n_kb, stream));
+    kb_flag_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, BN, n_kb, flags);
+    QHAP_LAUNCH_CHECK();
+    kb_list_kernel<<<a.n_tiles_n, 32, 0, stream>>>(n_kb, flags, kb_cnt, kb_idx);
+    QHAP_LAUNCH_CHECK();
+  }
+
+  const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
+  int cur = 0;
+  for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
+    const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
+    a.c2 = float(p.dt * (p.a0 - a_k));
+    a.c3 = float(p.dt * p.a0);
+    a.xh_out = xh[cur ^ 1];
+    a.xl_out = xl[cur ^ 1];
+    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_j, tm_h[cur], tm_l[cur], a);
+    QHAP_LAUNCH_CHECK();
+    cur ^= 1;
+  }
+  return QHAP_OK;
 }
 
 }  // namespace qhap

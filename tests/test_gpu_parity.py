@@ -292,6 +292,81 @@ def test_sparse_trajectory_cfg1_scaled(B, oracle, torch_mod):
     print(f"cfg1-scaled sparse: {fmt_traj(o)}")
 
 
+# ------------------------------------------------------------------------------------ (3) dense tcgen05 step
+def dense_case(B, oracle, name):
+    if name == "cfg0":
+        fr, p = synth.make_config(0)
+    elif name == "cfg1-scaled":
+        fr, p = synth.make_config(1, scale=0.1)          # ~800 reads: several N tiles, a ragged tail, banded J
+    elif name == "cfg2-scaled":
+        fr, p = synth.make_config(2, scale=0.15)         # ONT-like: |J| beyond the bf16-exact range, fp16-exact
+    else:
+        raise KeyError(name)
+    g = oracle.read_graph(fr)
+    w = oracle.read_weights(g, 1)
+    dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    return fr, p, g, w, J
+
+
+@pytest.mark.parametrize("name,R,bn,skip", [("cfg0", 64, 0, 0), ("cfg0", 5, 48, 1), ("cfg1-scaled", 200, 0, 0),
+                                            ("cfg1-scaled", 136, 112, 1), ("cfg2-scaled", 128, 256, 0)])
+def test_dense_trajectory(B, oracle, torch_mod, name, R, bn, skip):
+    """The tcgen05 step against the fp64 oracle: same bar as the sparse step (north_star: 1e-3 over 50 steps)."""
+    fr, p, g, w, J = dense_case(B, oracle, name)
+    jval = (-w).astype(np.float32)
+    x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, R)
+    dg = B.upload_csr(g)
+    xg = torch_mod.from_numpy(x0.copy()).cuda(); yg = torch_mod.from_numpy(y0.copy()).cuda()
+    xo, yo = x0.astype(np.float64), y0.astype(np.float64)
+    worst = 0.0
+    for k0 in range(0, 50, 10):       # 10 steps per call: exercises the ping-pong of the fp16 copies and the resume path
+        B.qhap_bsb_solve(dg, replicas=R, steps_total=p["T"], step_begin=k0, steps_run=10, weight_mode=1, path=1, x=xg, y=yg,
+                         dense_J=J, finalize=False, tile_skip=skip, dense_bn=bn)
+        xo, yo, _ = oracle.bsb_run(g["row_ptr"], g["col"], jval, xo, yo, steps_total=p["T"], step_begin=k0, steps_run=10, n_threads=8)
+        dx = np.abs(xg.cpu().numpy() - xo).max(); dy = np.abs(yg.cpu().numpy() - yo).max()
+        worst = max(worst, dx, dy)
+        if k0 < 20:                   # before wall contacts amplify roundings (the full policy is in compare_trajectory)
+            assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (name, k0, dx, dy)
+    print(f"dense {name} R {R} bn {bn} skip {skip}: max deviation over 50 free-running steps {worst:.2e}")
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=20, path=1, dense_J=J,
+                           tile_skip=skip)
+    print(f"dense {name}: {fmt_traj(o)}")
+
+
+def test_dense_tile_skip_is_bit_identical_and_matches_sparse(B, oracle, torch_mod):
+    """P12: skipped k-blocks contribute exactly 0 -> tile_skip changes no bit; dense vs sparse agree within the bar."""
+    fr, p, g, w, J = dense_case(B, oracle, "cfg1-scaled")
+    R = 256
+    dg = B.upload_csr(g)
+    outs = []
+    for path, skip, bn in ((1, 0, 128), (1, 1, 128), (1, 1, 64), (2, 0, 0)):
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=p["T"], steps_run=30, seed=p["seed"], weight_mode=1, path=path,
+                               dense_J=J if path == 1 else None, finalize=False, tile_skip=skip, dense_bn=bn)
+        outs.append((res["x"].cpu().numpy(), res["y"].cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    # another tile width changes the split of the same ascending-k accumulation only through skipped zero blocks
+    assert np.abs(outs[0][0] - outs[2][0]).max() <= 1e-5
+    dx = np.abs(outs[0][0] - outs[3][0]).max(); dy = np.abs(outs[0][1] - outs[3][1]).max()
+    print(f"dense vs sparse after 30 steps: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+    assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
+
+
+def test_dense_solve_quality_cfg0(B, oracle, torch_mod):
+    fr, p, g, w, J = dense_case(B, oracle, "cfg0")
+    x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, p["R"])
+    ores = oracle.solve(g["row_ptr"], g["col"], w, (-w).astype(np.float32), x0, y0, steps_total=p["T"], n_threads=8)
+    for skip in (0, 1):
+        res = B.qhap_bsb_solve(B.upload_csr(g), replicas=p["R"], steps_total=p["T"], seed=p["seed"], weight_mode=1, path=1, dense_J=J,
+                               tile_skip=skip)
+        gcut = int(res["best_cut"].cpu()[0])
+        assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
+        ccut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, res["best_spins"].cpu().numpy())
+        assert ccut[0] == gcut
+        gse, _ = ser_reads(oracle, fr, res["best_spins"].cpu().numpy())
+        ose, _ = ser_reads(oracle, fr, ores["best_spins"])
+        assert gse <= ose + 0.001
+
+
 # -------------------------------------------------------------------------------- full solve: quality and phasing
 def ser_reads(oracle, fr, spins):
     m = oracle.switch_hamming(oracle.read_vote(fr, spins), fr.hap_a)

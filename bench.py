@@ -42,7 +42,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (1 = the config the metric is quoted on)")
-    ap.add_argument("--path", default="auto", choices=["auto", "dense", "sparse"], help="bSB step kernel (auto = fastest validated)")
+    ap.add_argument("--path", default="auto", choices=["auto", "dense", "dense-full", "sparse"],
+                    help="bSB step kernel: dense = tcgen05 tiles over the non-zero k-blocks of J (tile_skip, bit-identical to "
+                         "dense-full = the whole N x N GEMM); sparse = CSR; auto = dense")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU seconds of the oracle sample")
     return ap.parse_args()
@@ -199,7 +201,8 @@ def run_ours(args):
     mode = B.QHAP_WEIGHT_D_MINUS_C            # BASELINE.json: "discordant minus concordant"
     n, R, T = fr.n_frag, p["R"], p["T"]
     seed = parallel.rank_seed(p["seed"], rank)
-    path = {"auto": 2, "sparse": 2, "dense": 1}[args.path]
+    path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1}[args.path]
+    tile_skip = 0 if args.path == "dense-full" else 1
     dense_dtype = B.QHAP_DENSE_FP16 if path == 1 else B.QHAP_DENSE_NONE
 
     dfr = B.upload_frags(fr)
@@ -208,7 +211,7 @@ def run_ours(args):
 
     def one_pass(frags):
         g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype)
-        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J,
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip,
                                cut_per_replica=False, workspace=state.get("ws"))
         state["ws"] = res["workspace"]
         cut, spins = res["best_cut"], res["best_spins"]
@@ -281,53 +284,84 @@ def run_ours(args):
     e2e_ms, _ = timed(e2e_pass, max(1, min(args.warmup, 2)), max(2, min(args.steps, 3)))
     e2e_value = n * R * T * world / (e2e_ms * 1e-3)
 
-    # ---- roofline of the dominant kernel (the bSB step): T launches timed with CUDA events on the launching stream
+    # ---- roofline of the dominant kernel (the bSB step): launches timed with CUDA events on the launching stream
     J = None
     if path == 1:
         _, J = B.qhap_build_read_graph(dfr, weight_mode=mode, dense_dtype=dense_dtype)
-    res0 = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=0, seed=seed, weight_mode=mode, path=path, dense_J=J, finalize=False)
-    x, y = res0["x"], res0["y"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    l0 = B.qhap_launch_count()
-    e0.record()
-    B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=T, weight_mode=mode, path=path, x=x, y=y, dense_J=J, finalize=False,
-                     workspace=state.get("ws"))
-    e1.record()
-    torch.cuda.synchronize()
-    step_launches = B.qhap_launch_count() - l0
-    step_ms = e0.elapsed_time(e1) / T
     peaks = measured_peaks()
+
+    def time_steps(path_, skip_, steps_):
+        res0 = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=0, seed=seed, weight_mode=mode, path=2, finalize=False)
+        x, y = res0["x"], res0["y"]
+        kw = dict(replicas=R, steps_total=T, weight_mode=mode, path=path_, x=x, y=y, dense_J=J if path_ == 1 else None, finalize=False,
+                  tile_skip=skip_)
+        r = B.qhap_bsb_solve(g, step_begin=0, steps_run=min(20, steps_), **kw)          # warm-up (also sizes the workspace)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        l0 = B.qhap_launch_count()
+        e0.record()
+        B.qhap_bsb_solve(g, step_begin=0, steps_run=steps_, workspace=r["workspace"], **kw)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps_, B.qhap_launch_count() - l0
+
+    step_ms, step_launches = time_steps(path, tile_skip, T)
+    n_pad = (n + 127) // 128 * 128
+
+    def tensor_roofline(ms_):
+        # flops the full GEMM performs per launch: 2 n^2 R per split term, 2 terms (x_hi, x_lo)
+        alg_flops = 2.0 * n * n * R * 2
+        return {"kernel": "dense_step_kernel (full N x N GEMM)", "bound": "tensor", "achieved": alg_flops / (ms_ * 1e-3) / 1e12,
+                "peak": peaks["bf16_sustained"], "unit": "TFLOP/s", "traffic": None, "flops_per_launch": alg_flops, "launch_ms": ms_,
+                "frac": alg_flops / (ms_ * 1e-3) / 1e12 / peaks["bf16_sustained"],
+                "peak_source": peaks["which"] + ": sustained bf16 (fp16 inputs run at the same kind::f16 rate)"}
+
+    extra = {}
     if path == 2:
-        # algorithmic bytes per launch: 16 B of fp32 state per spin-update (read x, read y, write y,
-        # write x') + the CSR once per launch (int32 col + fp32 val per directed entry, int32 row_ptr per row)
+        # algorithmic bytes per launch: 16 B of fp32 state per spin-update (read x, read y, write y, write x')
+        # + the CSR once per launch (int32 col + fp32 val per directed entry, int32 row_ptr per row)
         alg_bytes = 16.0 * n * R + 8.0 * g.nnz + 4.0 * (n + 1)
         roofline = {"kernel": "sparse_step_kernel", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
                     "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms, "peak_source": peaks["which"]}
+        roofline["frac"] = roofline["achieved"] / roofline["peak"]
+    elif tile_skip:
+        # algorithmic bytes per launch: fp32 state 16 B + fp16 split copies written once (4 B) and read at
+        # least once (4 B) per spin-update + the non-zero 64 x 64 fp16 blocks of J once
+        hg = g.to_host()                              # bookkeeping for the byte count only
+        rows = np.repeat(np.arange(n, dtype=np.int64), np.diff(hg["row_ptr"]))
+        nz_blocks = int(np.unique((rows // 64) * (1 << 32) + hg["col"].astype(np.int64) // 64).size)
+        alg_bytes = 24.0 * n * R + nz_blocks * 64 * 64 * 2.0
+        roofline = {"kernel": "dense_step_kernel (tile_skip)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9,
+                    "peak": peaks["hbm"], "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms,
+                    "peak_source": peaks["which"], "nonzero_64x64_blocks_of_J": nz_blocks}
+        roofline["frac"] = roofline["achieved"] / roofline["peak"]
+        full_ms, _ = time_steps(1, 0, 200)            # the same kernel over ALL k-blocks (north_star's dense GEMM), 200 launches
+        extra["roofline_dense_full"] = tensor_roofline(full_ms)
+        extra["roofline_dense_full"]["spin_updates_per_s"] = n * R / (full_ms * 1e-3)
     else:
-        n_pad = (n + 127) // 128 * 128
-        terms = 2
-        alg_flops = 2.0 * n_pad * n_pad * R * terms
-        roofline = {"kernel": "dense_step_kernel", "bound": "tensor", "achieved": alg_flops / (step_ms * 1e-3) / 1e12,
-                    "peak": peaks["bf16_sustained"], "unit": "TFLOP/s", "traffic": None, "flops_per_launch": alg_flops,
-                    "launch_ms": step_ms, "peak_source": peaks["which"] + ", sustained bf16 x 1.0 (fp16 = same kind::f16 rate)"}
-    roofline["frac"] = roofline["achieved"] / roofline["peak"]
-    prof = ROOT / "profiles" / "roofline_traffic.json"              # dram bytes per launch from the committed ncu capture
+        roofline = tensor_roofline(step_ms)
+    prof = ROOT / "profiles" / "roofline_traffic.csv"              # dram bytes per launch from the committed ncu captures
     if prof.exists():
         try:
-            roofline["traffic"] = json.loads(prof.read_text()).get(roofline["kernel"])
+            for line in prof.read_text().splitlines()[1:]:
+                k, v = line.split(",")[:2]
+                if roofline["kernel"].startswith(k) and ((" (tile_skip)" in roofline["kernel"]) == ("tile_skip" in line)):
+                    roofline["traffic"] = float(v)
         except Exception:
             pass
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": workload_name(args.config, fr, p), "path": {1: "dense-tcgen05", 2: "sparse-csr"}[path],
+           "config": {"workload": workload_name(args.config, fr, p),
+                      "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM)" if tile_skip else " full GEMM"),
+                               2: "sparse-csr"}[path],
                       "weight_mode": "D-C", "replicas_per_gpu": R, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                       "parallelism": f"replicas x{world} (weak)"},
            "region_ms": ms, "edges_replicas_per_s": edges * R * T * world / (ms * 1e-3), "undirected_edges": edges,
            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
            "gpu_launches": int(launches), "bsb_step_launches_per_solve": int(step_launches),
            "clocks": clocks, "roofline": roofline, "library": B.qhap_version()}
+    out.update(extra)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O
         O.build()

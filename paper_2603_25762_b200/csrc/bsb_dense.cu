@@ -7,7 +7,7 @@
 //   B (N side) = output spins: rows of J (fp16, integers exact to 2048), row-major [ld][ld] (K-major);
 //   D in TMEM: lane = replica, column = spin  ->  the epilogue's fp32 state accesses x[i][r], y[i][r] are coalesced
 //   across the 32 lanes of a warp without any shared-memory transpose.
-// x is carried in fp32; the tensor cores see x = x_hi + x_lo (two fp16 terms, |x - x_hi - x_lo| <= 2^-25 for |x| <= 1),
+// x is carried in fp32; the tensor cores see 2^15 x = x_hi + x_lo (two fp16 terms, relative error <= 2^-23),
 // both terms accumulate into the same fp32 TMEM tile against the same J tile in shared memory.
 // Jacobi update across CTAs: the fp16 copies are double-buffered (read buffer b, write buffer 1-b); fp32 x, y are
 // private to the tile that owns them and are updated in place.  One launch per step (grid-wide step boundary).
@@ -54,10 +54,16 @@ struct DenseArgs {
   __half* xl_out;
 };
 
-// fp32 -> two fp16 terms.  hi = rn(x); lo = rn(x - hi) (exact difference; lo may be subnormal: absolute error <= 2^-25).
+// fp32 -> two fp16 terms of xs = 2^15 x (|x| <= 1 -> |xs| <= 32768, inside fp16's range): hi = rn(xs), lo = rn(xs - hi)
+// (the difference is exact in fp32).  The scale keeps lo a NORMAL fp16 number for every |x| >= 2^-17, so that
+// |xs - hi - lo| <= 2^-23 |xs|: a relative resolution one bit short of fp32's at every magnitude (unscaled, lo would be
+// a subnormal below |x| = 0.25 and the resolution an absolute 2^-25).  The accumulator then holds 2^15 F; the epilogue
+// folds the exact factor 2^-15 into c1, so fma(c1 2^-15, 2^15 F, .) == fma(c1, F, .) bit for bit.
+constexpr float kXScale = 32768.0f;
 __device__ __forceinline__ void split_half(float v, __half& hi, __half& lo) {
-  hi = __float2half_rn(v);
-  lo = __float2half_rn(v - __half2float(hi));
+  const float vs = v * kXScale;
+  hi = __float2half_rn(vs);
+  lo = __float2half_rn(vs - __half2float(hi));
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -156,7 +162,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     const int ew = warp - 2;
     const int quarter = warp & 3;              // TMEM lanes 32 q .. 32 q + 31 are accessible to warps with warp % 4 == q
     const int par = ew >> 2;                   // two warps per quarter take alternating 32-column chunks
-    const float c1 = __ldg(a.c1), c2 = a.c2, c3 = a.c3;
+    const float c1 = __ldg(a.c1) * (1.0f / kXScale), c2 = a.c2, c3 = a.c3;   // accumulator = 2^15 F
     int acc = 0;
     uint32_t acc_phase = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {

@@ -66,6 +66,69 @@ __device__ __forceinline__ void split_half(float v, __half& hi, __half& lo) {
   lo = __float2half_rn(vs - __half2float(hi));
 }
 
+struct EpiConsts {
+  float c1, c2, c3;
+  int lane_r;            // replica of this thread inside the tile
+};
+
+// fp32 state of one work item (16 spins x this thread's replica) -> registers; masked entries read as 0.
+__device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, float (&xv)[kChunk],
+                                         float (&yv)[kChunk]) {
+  const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+  const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
+  const bool r_ok = r < a.R;
+  const float* px = a.x + size_t(i0) * a.R + r;
+  const float* py = a.y + size_t(i0) * a.R + r;
+#pragma unroll
+  for (int j = 0; j < kChunk; ++j) {
+    const bool ok = r_ok && (i0 + j) < a.n;
+    xv[j] = ok ? px[size_t(j) * a.R] : 0.f;
+    yv[j] = ok ? py[size_t(j) * a.R] : 0.f;
+  }
+}
+
+// Fused update of one work item: y' = y + dt(-(a0 - a_k) x + c0 F), x' = x + dt a0 y', inelastic wall; stores x', y'
+// (fp32, coalesced across the warp's 32 replicas) and the fp16 split of x' (32 contiguous bytes per thread).
+__device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tile, int ch,
+                                                 const uint32_t (&v)[kChunk], const float (&xv)[kChunk],
+                                                 const float (&yv)[kChunk]) {
+  const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+  const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
+  const bool r_ok = r < a.R;
+  float* px = a.x + size_t(i0) * a.R + r;
+  float* py = a.y + size_t(i0) * a.R + r;
+  uint32_t hp[kChunk / 2], lp[kChunk / 2];    // fp16 pairs (spin i0 + 2q, i0 + 2q + 1) of x_hi', x_lo'
+#pragma unroll
+  for (int j = 0; j < kChunk; ++j) {
+    const bool ok = r_ok && (i0 + j) < a.n;
+    const float F = __uint_as_float(v[j]);
+    float yn = fmaf(ec.c1, F, fmaf(-ec.c2, xv[j], yv[j]));
+    float xn = fmaf(ec.c3, yn, xv[j]);
+    if (fabsf(xn) > 1.0f) {                  // inelastic wall, strict inequality (R10d)
+      xn = copysignf(1.0f, xn);
+      yn = 0.0f;
+    }
+    if (ok) {
+      px[size_t(j) * a.R] = xn;
+      py[size_t(j) * a.R] = yn;
+    }
+    __half h, l;
+    split_half(ok ? xn : 0.f, h, l);
+    const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+    if (j & 1) { hp[j >> 1] |= hb << 16; lp[j >> 1] |= lb << 16; }
+    else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
+  }
+  if (r_ok && i0 < a.n) {                      // n_k >= round_up(n, 64) keeps the 16-spin run in bounds
+    uint4* ph = reinterpret_cast<uint4*>(a.xh_out + size_t(r) * a.n_k + i0);
+    uint4* pl = reinterpret_cast<uint4*>(a.xl_out + size_t(r) * a.n_k + i0);
+#pragma unroll
+    for (int q = 0; q < kChunk / 8; ++q) {
+      ph[q] = make_uint4(hp[4 * q], hp[4 * q + 1], hp[4 * q + 2], hp[4 * q + 3]);
+      pl[q] = make_uint4(lp[4 * q], lp[4 * q + 1], lp[4 * q + 2], lp[4 * q + 3]);
+    }
+  }
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_xh,
                   const __grid_constant__ CUtensorMap tm_xl, const DenseArgs a) {
@@ -159,68 +222,55 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     }
   } else {
     // ========================================================================================= epilogue
+    // Work item = (tile, 16-column chunk).  The fp32 state of item k+1 is loaded into registers before item k is
+    // computed and stored (two register buffers, alternated by a 2x unrolled loop), across tile boundaries too: the
+    // loads do not depend on the accumulator, so they are in flight while the warp waits for tmem_full.
     const int ew = warp - 2;
     const int quarter = warp & 3;              // TMEM lanes 32 q .. 32 q + 31 are accessible to warps with warp % 4 == q
-    const int par = ew >> 2;                   // two warps per quarter take alternating 32-column chunks
-    const float c1 = __ldg(a.c1) * (1.0f / kXScale), c2 = a.c2, c3 = a.c3;   // accumulator = 2^15 F
+    const int par = ew >> 2;                   // the kEpiWarps / 4 warps of a quarter take chunks par, par + P, par + 2P, ...
+    constexpr int P = kEpiWarps / 4;
+    EpiConsts ec;
+    ec.c1 = __ldg(a.c1) * (1.0f / kXScale);    // accumulator = 2^15 F
+    ec.c2 = a.c2; ec.c3 = a.c3;
+    ec.lane_r = quarter * 32 + lane;
     int acc = 0;
     uint32_t acc_phase = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
-      const int r = tm * kBM + quarter * 32 + lane;
-      const bool r_ok = r < a.R;
-      ptx::mbar_wait(tfull_bar(acc), acc_phase);
-      ptx::tc_fence_after();
-      for (int ch = par; ch * kChunk < a.BN; ch += 2) {
-        const int i0 = tn * a.BN + ch * kChunk;
-        if (i0 >= a.n) break;
-        uint32_t v[kChunk];
-        ptx::tmem_ld_32x32b_x16(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
-        float xv[kChunk], yv[kChunk];
-#pragma unroll
-        for (int j = 0; j < kChunk; ++j) {
-          const bool ok = r_ok && (i0 + j) < a.n;
-          const size_t off = size_t(i0 + j) * a.R + r;
-          xv[j] = ok ? a.x[off] : 0.f;
-          yv[j] = ok ? a.y[off] : 0.f;
-        }
-        ptx::tmem_ld_wait();
-        uint32_t hp[kChunk / 2], lp[kChunk / 2];    // fp16 pairs (spin i0 + 2q, i0 + 2q + 1) of x_hi', x_lo'
-#pragma unroll
-        for (int j = 0; j < kChunk; ++j) {
-          const bool ok = r_ok && (i0 + j) < a.n;
-          const float F = __uint_as_float(v[j]);
-          float yn = fmaf(c1, F, fmaf(-c2, xv[j], yv[j]));
-          float xn = fmaf(c3, yn, xv[j]);
-          if (fabsf(xn) > 1.0f) {                  // inelastic wall, strict inequality (R10d)
-            xn = copysignf(1.0f, xn);
-            yn = 0.0f;
-          }
-          if (ok) {
-            const size_t off = size_t(i0 + j) * a.R + r;
-            a.x[off] = xn;
-            a.y[off] = yn;
-          }
-          __half h, l;
-          split_half(ok ? xn : 0.f, h, l);
-          const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-          if (j & 1) { hp[j >> 1] |= hb << 16; lp[j >> 1] |= lb << 16; }
-          else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
-        }
-        if (r_ok) {                                 // 32 contiguous bytes per thread; n_k >= round_up(n, 64) keeps it in bounds
-          uint4* ph = reinterpret_cast<uint4*>(a.xh_out + size_t(r) * a.n_k + i0);
-          uint4* pl = reinterpret_cast<uint4*>(a.xl_out + size_t(r) * a.n_k + i0);
-#pragma unroll
-          for (int q = 0; q < kChunk / 8; ++q) {
-            ph[q] = make_uint4(hp[4 * q], hp[4 * q + 1], hp[4 * q + 2], hp[4 * q + 3]);
-            pl[q] = make_uint4(lp[4 * q], lp[4 * q + 1], lp[4 * q + 2], lp[4 * q + 3]);
-          }
-        }
+    // every warp owns chunk `par` of every tile (possibly fully masked), so that it arrives on tmem_empty once per tile
+    auto advance = [&](int& tile, int& ch) {
+      ch += P;
+      if (ch * kChunk >= a.BN || (tile / a.n_tiles_m) * a.BN + ch * kChunk >= a.n) { tile += gridDim.x; ch = par; }
+    };
+    auto step = [&](int& tile, int& ch, const float (&xc)[kChunk], const float (&yc)[kChunk], float (&xn)[kChunk],
+                    float (&yn)[kChunk]) -> bool {
+      if (ch == par) {                         // first chunk of a tile: the accumulator must be complete
+        ptx::mbar_wait(tfull_bar(acc), acc_phase);
+        ptx::tc_fence_after();
       }
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      uint32_t v[kChunk];
+      ptx::tmem_ld_32x32b_x16(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
+      int ntile = tile, nch = ch;
+      advance(ntile, nch);
+      const bool nhave = ntile < n_tiles;
+      if (nhave) epi_load(a, ec, ntile, nch, xn, yn);
+      ptx::tmem_ld_wait();
+      epi_update_store(a, ec, tile, ch, v, xc, yc);
+      if (ntile != tile) {                     // last chunk of this warp in the tile: hand the accumulator stage back
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      }
+      tile = ntile; ch = nch;
+      return nhave;
+    };
+    int tile = blockIdx.x, ch = par;
+    if (tile < n_tiles) {
+      float xa[kChunk], ya[kChunk], xb[kChunk], yb[kChunk];
+      epi_load(a, ec, tile, ch, xa, ya);
+      while (true) {
+        if (!step(tile, ch, xa, ya, xb, yb)) break;
+        if (!step(tile, ch, xb, yb, xa, ya)) break;
+      }
     }
   }
 
@@ -328,8 +378,8 @@ int32_t pitch_of(int32_t n) { return int32_t(ceil_div(n, 64) * 64); }
 // Tile width: full GEMM -> minimise waves x width over the persistent grid; tile_skip -> narrow tiles (the step is then
 // bound by the epilogue's state traffic and balances better with more tiles).
 int32_t choose_bn(int32_t n, int32_t R, bool tile_skip, int32_t forced) {
-  if (forced >= 16 && forced <= kMaxBN && forced % 16 == 0) return forced;
-  if (n <= 16) return 16;
+  if (forced >= 16 * (kEpiWarps / 4) && forced <= kMaxBN && forced % 16 == 0) return forced;
+  if (n <= 32) return 32;
   const int64_t tm = ceil_div(R, kBM), sms = sm_count();
   int32_t best = 128;
   double best_cost = 1e300;

@@ -443,3 +443,54 @@ def test_solve_snp_blocks_quality(B, oracle, torch_mod):
     om = oracle.switch_hamming(oracle.snp_readout(fr.h1, ost)[covered], fr.hap_a[covered])
     print(f"cfg3-scaled: SE gpu {gm['se']:.4f} oracle {om['se']:.4f}")
     assert gm["se"] <= om["se"] + 0.001
+
+
+# ----------------------------------------------------------- BASELINE.json configs[1] at FULL size (bench.py's launch config)
+def test_cfg1_full_size_sampled(B, oracle, torch_mod):
+    """cfg1 as bench.py runs it (n = 8,000 fragments, R = 1,024, dense tcgen05 step with tile_skip, device-side seeded
+    start state): graph build bit-exact; the first 10 steps of 8 sampled replicas against the oracle run on exactly those
+    replicas (replicas are independent trajectories); cuts of the sampled replicas and the best cut bit-exact; best cut
+    and switch error against an oracle solve of a 64-replica subset."""
+    fr, p = synth.make_config(1)
+    n, R, T = fr.n_frag, p["R"], p["T"]
+    dfr = B.upload_frags(fr)
+    og = oracle.read_graph(fr)
+    g, J = B.qhap_build_read_graph(dfr, weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    assert_csr_equal(g.to_host(), og, ("d", "c"))
+    w = oracle.read_weights(og, 1)
+    jval = (-w).astype(np.float32)
+    # dense J is exactly -w scattered (sampled rows)
+    Jh = J.cpu().numpy()
+    for a in (0, 1, n // 2, n - 1):
+        row = np.zeros(Jh.shape[1], np.float32)
+        sl = slice(og["row_ptr"][a], og["row_ptr"][a + 1])
+        row[og["col"][sl]] = jval[sl]
+        assert np.array_equal(Jh[a].astype(np.float32), row)
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    sample = np.array([0, 1, 127, 128, 500, 777, 1000, R - 1])
+    for path, skip, name in ((1, 1, "dense tile_skip"), (2, 0, "sparse")):
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=1, path=path,
+                               dense_J=J if path == 1 else None, tile_skip=skip, finalize=False)
+        xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], jval, x0[:, sample].astype(np.float64), y0[:, sample].astype(np.float64),
+                                   steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+        dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
+        print(f"cfg1 full size, {name}: 10 steps, 8 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
+    res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=p["seed"], weight_mode=1, path=1, dense_J=J, tile_skip=1)
+    cuts = res["cut"].cpu().numpy()[0]
+    sx = np.where(res["x"].cpu().numpy()[:, sample] >= 0, 1, -1).astype(np.int8)
+    ecut, _ = oracle.cut_eval(og["row_ptr"], og["col"], w, sx)
+    assert np.array_equal(cuts[sample], ecut)
+    spins = res["best_spins"].cpu().numpy()
+    gcut = int(res["best_cut"].cpu()[0]); r = int(res["best_replica"].cpu()[0])
+    ccut, _ = oracle.cut_eval(og["row_ptr"], og["col"], w, spins)
+    assert ccut[0] == gcut == cuts.max() and r == int(np.flatnonzero(cuts == cuts.max())[0])
+    sub = np.arange(64)
+    ores = oracle.solve(og["row_ptr"], og["col"], w, jval, x0[:, sub].copy(), y0[:, sub].copy(), steps_total=T, n_threads=16)
+    assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
+    hap = B.qhap_phase_readout_reads(dfr, res["best_spins"]).cpu().numpy()
+    assert np.array_equal(hap, oracle.read_vote(fr, spins))
+    gse, ghe = ser_reads(oracle, fr, spins)
+    ose, ohe = ser_reads(oracle, fr, ores["best_spins"])
+    print(f"cfg1 full size: gpu best cut {gcut} (replica {r}), oracle(64 replicas) {ores['best_cut']}; SE gpu {gse:.5f} oracle {ose:.5f}")
+    assert gse <= ose + 0.001

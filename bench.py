@@ -9,6 +9,9 @@ sequence fed from pinned HOST buffers (H2D of the fragment matrix and D2H of the
 region).  N > 1 (torchrun): every rank runs its own R replicas of the same region (weak scaling, no per-step exchange),
 then 16 bytes per rank are all-gathered to pick the global best replica (paper_2603_25762_b200/parallel.py).
 
+`--config 3` / `--config 4` (not the default; extra measurements of the sparse CSR step) run the SNP-based path instead:
+  qhap_build_snp_graph -> [qhap_block_split] -> qhap_bsb_solve (CSR) -> [qhap_block_stitch] -> qhap_phase_readout_snps.
+
 `--impl reference` times the fp64 CPU oracle (oracle/, test infrastructure) on the box's host cores on a bounded sample
 of the same workload -- a reported baseline, not the target.
 
@@ -197,19 +200,43 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     fr, p = synth.make_config(args.config)
-    assert p["graph"] == "read", "bench.py times the read-based configs (0-2); the SNP configs are parity-test cases"
-    mode = B.QHAP_WEIGHT_D_MINUS_C            # BASELINE.json: "discordant minus concordant"
-    n, R, T = fr.n_frag, p["R"], p["T"]
+    snp = p["graph"] == "snp"
+    mode = B.QHAP_WEIGHT_FX if snp else B.QHAP_WEIGHT_D_MINUS_C     # BASELINE.json: "discordant minus concordant"
+    R, T = p["R"], p["T"]
+    n = fr.n_snp if snp else fr.n_frag
     seed = parallel.rank_seed(p["seed"], rank)
-    path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1}[args.path]
-    tile_skip = 0 if args.path == "dense-full" else 1
+    if snp:
+        assert args.path in ("auto", "sparse"), "the SNP graphs (configs 3, 4) run on the sparse CSR path"
+        path, tile_skip = 2, 0
+    else:
+        path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1}[args.path]
+        tile_skip = 0 if args.path == "dense-full" else 1
     dense_dtype = B.QHAP_DENSE_FP16 if path == 1 else B.QHAP_DENSE_NONE
+    win = synth.block_windows(fr.n_snp, p["block"], p["stride"]) if "block" in p else None
+    if win is not None and world > 1:
+        win_mine = win[parallel.block_shard(len(win), rank, world)]   # strong scaling over independent blocks (no exchange)
+    else:
+        win_mine = win
 
     dfr = B.upload_frags(fr)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     state = {}
 
     def one_pass(frags):
+        if snp:
+            g0 = B.qhap_build_snp_graph(frags, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
+            g = B.qhap_block_split(g0, win_mine) if win is not None else g0
+            res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=2, cut_per_replica=False,
+                                   workspace=state.get("ws"))
+            state["ws"] = res["workspace"]
+            cut, spins = res["best_cut"], res["best_spins"]
+            if win is not None:
+                spins = B.qhap_block_stitch(fr.n_snp, win_mine, spins) if world == 1 else spins
+            elif world > 1:
+                cut, spins, _ = parallel.select_best_across_ranks(cut, spins)
+            hap = B.qhap_phase_readout_snps(frags.h1, spins) if (win is None or world == 1) else spins
+            state["g"] = g
+            return cut, hap
         g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype)
         res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip,
                                cut_per_replica=False, workspace=state.get("ws"))
@@ -260,29 +287,35 @@ def run_ours(args):
     sampler.start()
     ms, launches = timed(lambda: one_pass(dfr), args.warmup, args.steps)
     clocks = sampler.stop()
-    value = n * R * T * world / (ms * 1e-3)
     g = state["g"]
+    # spins solved per pass: the read/SNP graph's vertices; config 3 solves overlapping blocks (sum of the window lengths),
+    # sharded over ranks (strong scaling); every other config runs R replicas of the whole instance per rank (weak scaling)
+    blocks = win is not None
+    n_solved = int((win[:, 1] - win[:, 0]).sum()) if blocks else n
+    work = n_solved * R * T * (1 if blocks else world)
+    value = work / (ms * 1e-3)
     edges = g.nnz // 2
 
     # ---- e2e: the same pass fed from pinned host buffers, result read back to the host
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(fr, k), dtype=dt)).pin_memory()
-            for k, dt in (("frag_ptr", np.int64), ("snp_idx", np.int32), ("allele", np.uint8), ("qual", np.uint8))}
+            for k, dt in (("frag_ptr", np.int64), ("snp_idx", np.int32), ("allele", np.uint8), ("qual", np.uint8)) + ((("frag_flags", np.uint8),) if snp else ())}
     dbuf = {k: torch.empty_like(v, device=dev) for k, v in host.items()}
     hap_host = torch.empty(fr.n_snp, dtype=torch.int8).pin_memory()
-    cut_host = torch.empty(1, dtype=torch.int64).pin_memory()
+    cut_host = torch.empty(len(win_mine) if blocks else 1, dtype=torch.int64).pin_memory()
     h2d = sum(v.numel() * v.element_size() for v in host.values())
-    d2h = hap_host.numel() + 8
+    d2h = hap_host.numel() + 8 * cut_host.numel()
 
     def e2e_pass():
         for k in host:
             dbuf[k].copy_(host[k], non_blocking=True)
-        frags = B.Frags(fr.n_frag, fr.n_snp, fr.nnz, dbuf["frag_ptr"], dbuf["snp_idx"], dbuf["allele"], dbuf["qual"], None, None)
+        frags = B.Frags(fr.n_frag, fr.n_snp, fr.nnz, dbuf["frag_ptr"], dbuf["snp_idx"], dbuf["allele"], dbuf["qual"],
+                        dbuf.get("frag_flags"), None)
         cut, hap = one_pass(frags)
-        hap_host.copy_(hap, non_blocking=True)
+        hap_host[:hap.numel()].copy_(hap, non_blocking=True)
         cut_host.copy_(cut, non_blocking=True)
 
     e2e_ms, _ = timed(e2e_pass, max(1, min(args.warmup, 2)), max(2, min(args.steps, 3)))
-    e2e_value = n * R * T * world / (e2e_ms * 1e-3)
+    e2e_value = work / (e2e_ms * 1e-3)
 
     # ---- roofline of the dominant kernel (the bSB step): launches timed with CUDA events on the launching stream
     J = None
@@ -320,7 +353,9 @@ def run_ours(args):
     if path == 2:
         # algorithmic bytes per launch: 16 B of fp32 state per spin-update (read x, read y, write y, write x')
         # + the CSR once per launch (int32 col + fp32 val per directed entry, int32 row_ptr per row)
-        alg_bytes = 16.0 * n * R + 8.0 * g.nnz + 4.0 * (n + 1)
+        # (+ SURVEY 8(d): 4 B per replica for every non-zero whose column lies outside the L2-resident band: config 4's
+        # long-range Pore-C entries -- not counted here, so the figure is a lower bound of the traffic the method needs)
+        alg_bytes = 16.0 * g.n * R + 8.0 * g.nnz + 4.0 * (g.n + 1)
         roofline = {"kernel": "sparse_step_kernel", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
                     "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms, "peak_source": peaks["which"]}
         roofline["frac"] = roofline["achieved"] / roofline["peak"]
@@ -351,13 +386,13 @@ def run_ours(args):
             pass
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if blocks else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": workload_name(args.config, fr, p),
                       "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM)" if tile_skip else " full GEMM"),
                                2: "sparse-csr"}[path],
-                      "weight_mode": "D-C", "replicas_per_gpu": R, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
-                      "parallelism": f"replicas x{world} (weak)"},
-           "region_ms": ms, "edges_replicas_per_s": edges * R * T * world / (ms * 1e-3), "undirected_edges": edges,
+                      "weight_mode": "fixed-point Eq. 14" if snp else "D-C", "replicas_per_gpu": R, "spins_solved": n_solved, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
+                      "parallelism": f"blocks x{world} (strong)" if blocks else f"replicas x{world} (weak)"},
+           "region_ms": ms, "edges_replicas_per_s": edges * R * T * (1 if blocks else world) / (ms * 1e-3), "undirected_edges": edges,
            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
            "gpu_launches": int(launches), "bsb_step_launches_per_solve": int(step_launches),
            "clocks": clocks, "roofline": roofline, "library": B.qhap_version()}

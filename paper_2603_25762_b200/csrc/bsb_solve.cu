@@ -52,8 +52,10 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   QHAP_REQUIRE(p->weight_mode >= 0 && p->weight_mode <= 2, "bad weight_mode");
   QHAP_REQUIRE(n_inst == 1 || inst_ptr, "inst_ptr (host) is required for n_inst > 1");
   int path = p->path;
-  if (path == 0) path = (dense_J && n_inst == 1) ? 1 : 2;
-  QHAP_REQUIRE(path == 1 || path == 2, "path must be 0, 1 or 2");
+  const int32_t res_rc = (path == 0 || path == 3) ? resident_plan(graph->n, graph->nnz, p->replicas) : 0;
+  if (path == 0) path = res_rc > 0 ? 3 : ((dense_J && n_inst == 1) ? 1 : 2);
+  QHAP_REQUIRE(path >= 1 && path <= 3, "path must be 0, 1, 2 or 3");
+  QHAP_REQUIRE(path != 3 || res_rc > 0, "resident path: problem too large for shared memory (needs n R <= 65536)");
   if (path == 1) {
     QHAP_REQUIRE(dense_J && n_inst == 1, "dense path needs dense_J and a single instance");
     QHAP_REQUIRE(dense_dtype == QHAP_DENSE_FP16, "dense path takes J in fp16 (exact to |J| <= 2048)");
@@ -87,6 +89,8 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   if (p->steps_run > 0 && n > 0) {
     if (path == 1) {
       QHAP_TRY(dense_solve_steps(g, dense_J, dense_ld, dense_dtype, R, s.c1, *p, x, y, s.dense, s.dense_bytes, stream));
+    } else if (path == 3) {
+      QHAP_TRY(resident_solve_steps(g, s.jval, R, res_rc, n_inst, s.inst_ptr, s.c1, *p, x, y, stream));
     } else {
       float* cur = x;
       float* alt = s.x_alt;

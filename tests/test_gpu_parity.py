@@ -292,6 +292,44 @@ def test_sparse_trajectory_cfg1_scaled(B, oracle, torch_mod):
     print(f"cfg1-scaled sparse: {fmt_traj(o)}")
 
 
+# ----------------------------------------------------------------- (4') shared-memory-resident solve (small problems)
+@pytest.mark.parametrize("R", [64, 5])
+def test_resident_path_equals_sparse_bitwise(B, oracle, torch_mod, R):
+    """path 3 keeps x, y and the CSR in shared memory for the whole call; same fp32 operation order as path 2."""
+    fr, p = synth.make_config(0)
+    g = oracle.read_graph(fr)
+    dg = B.upload_csr(g)
+    outs = {}
+    for path in (2, 3):
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=p["T"], steps_run=137, seed=p["seed"], weight_mode=1, path=path, finalize=False)
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=p["T"], step_begin=137, steps_run=63, weight_mode=1, path=path,
+                               x=res["x"], y=res["y"])
+        outs[path] = res
+    for k in ("x", "y", "best_spins", "best_cut", "best_replica", "cut"):
+        assert torch_mod.equal(outs[2][k], outs[3][k]), k
+    w = oracle.read_weights(g, 1)
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=20, path=3, expect_full=True)
+    print(f"cfg0 resident R {R}: {fmt_traj(o)}")
+
+
+def test_resident_path_batched_instances_and_auto(B, oracle, torch_mod):
+    """Block-diagonal batch (per-instance c0) on the resident path; path 0 picks it for small problems."""
+    fr, p = synth.make_config(3, scale=0.002)
+    g = oracle.snp_graph(fr, 3, 0.1)
+    win = synth.block_windows(fr.n_snp, 150, 120)
+    bs = oracle.block_split(g, win)
+    dg = B.upload_csr(bs)
+    outs = []
+    for path in (2, 3, 0):
+        res = B.qhap_bsb_solve(dg, replicas=16, steps_total=300, seed=7, weight_mode=2, path=path)
+        outs.append(res)
+    for k in ("x", "y", "best_spins", "best_cut"):
+        assert torch_mod.equal(outs[0][k], outs[1][k]) and torch_mod.equal(outs[0][k], outs[2][k]), k
+    with pytest.raises(B.QhapError):       # too large for shared memory -> loud error, no silent fallback
+        fr1, p1 = synth.make_config(1, scale=0.1)
+        B.qhap_bsb_solve(B.upload_csr(oracle.read_graph(fr1)), replicas=256, steps_total=10, seed=1, weight_mode=1, path=3)
+
+
 # ------------------------------------------------------------------------------------ (3) dense tcgen05 step
 def dense_case(B, oracle, name):
     if name == "cfg0":

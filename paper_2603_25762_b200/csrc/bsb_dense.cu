@@ -14,10 +14,11 @@
 //
 // Warp roles (320 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one elected lane),
 // warps 2..9 = epilogue (TMEM lane quarter = warp % 4, two warps per quarter interleave 32-column chunks).
-// Pipelines: kStages shared-memory stages (full/empty mbarriers) and 2 TMEM accumulator stages (tmem_full/tmem_empty).
+// Pipelines: n_stages shared-memory stages (full/empty mbarriers) and 2 TMEM accumulator stages (tmem_full/tmem_empty).
 #include <cuda.h>
 #include <cuda_fp16.h>
 
+#include <cstdlib>
 #include <vector>
 
 #include "kernels.cuh"
@@ -30,19 +31,19 @@ namespace {
 constexpr int kBM = 128;                 // replicas per tile (UMMA M)
 constexpr int kBK = 64;                  // spins per k-block: 64 fp16 = one 128-byte swizzle row
 constexpr int kMaxBN = 256;              // output spins per tile (UMMA N), runtime 32..256 in steps of 32
-constexpr int kStages = 3;
-constexpr int kStageJ = kMaxBN * kBK * 2;            // 32 KB
+constexpr int kMaxStages = 8;             // shared-memory pipeline depth: as many stages as fit (3 at BN = 256, 5 at BN = 64)
 constexpr int kStageX = kBM * kBK * 2;               // 16 KB each for x_hi, x_lo
-constexpr int kStageBytes = kStageJ + 2 * kStageX;   // 64 KB
+constexpr int kSmemBudget = 216 * 1024;              // operand stages; + 1 KB alignment slack + barriers <= 227 KB
 constexpr int kEpiWarps = 8;
 constexpr int kChunk = 16;                // accumulator columns (spins) per tcgen05.ld in the epilogue
 constexpr int kThreads = 64 + 32 * kEpiWarps;
 constexpr int kTmemCols = 512;                       // 2 accumulator stages x 256 columns
-constexpr size_t kSmemBytes = size_t(kStages) * kStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr size_t kSmemBytes = size_t(kSmemBudget) + 1024 /*alignment slack*/ + 256 /*barriers*/;
 
 struct DenseArgs {
   int32_t n, R, n_k;          // spins, replicas, row pitch (elements) of the fp16 copies
   int32_t BN;                 // tile width in output spins
+  int32_t n_stages;           // shared-memory stages of (BN x 64 J tile, 128 x 64 x_hi, 128 x 64 x_lo)
   int32_t n_tiles_m, n_tiles_n, n_kblocks;
   const int32_t* kb_cnt;      // [n_tiles_n] number of listed k-blocks per N tile, or nullptr = all k-blocks
   const int32_t* kb_idx;      // [n_tiles_n][n_kblocks]
@@ -134,12 +135,14 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
                   const __grid_constant__ CUtensorMap tm_xl, const DenseArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;       // 128B swizzle needs 1024-byte alignment
-  const uint32_t bar_base = smem_base + kStages * kStageBytes;
+  const int kStages = a.n_stages;
+  const uint32_t kStageJ = uint32_t(a.BN) * kBK * 2, kStageBytes = kStageJ + 2 * kStageX;
+  const uint32_t bar_base = smem_base + kSmemBudget;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
-  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kStages + s); };
-  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kStages + 2 + s); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 4);
+  auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 2 + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStages + 4);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && ptx::elect_one()) {
@@ -429,6 +432,8 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   const int32_t BN = choose_bn(n, R, skip, p.dense_bn);
   DenseArgs a;
   a.n = n; a.R = R; a.n_k = n_k; a.BN = BN;
+  a.n_stages = std::min(kMaxStages, kSmemBudget / (BN * kBK * 2 + 2 * kStageX));
+  if (const char* e = getenv("QHAP_TUNE_STAGES")) a.n_stages = std::max(1, std::min(a.n_stages, atoi(e)));   // TUNING ONLY
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = int32_t(ceil_div(n, BN));
   a.n_kblocks = n_kb;

@@ -44,6 +44,7 @@ struct DenseArgs {
   int32_t n, R, n_k;          // spins, replicas, row pitch (elements) of the fp16 copies
   int32_t BN;                 // tile width in output spins
   int32_t n_stages;           // shared-memory stages of (BN x 64 J tile, 128 x 64 x_hi, 128 x 64 x_lo)
+  int32_t stage_out;          // 1: the fp16 copies leave through swizzled shared-memory tiles and TMA stores (BN == 64)
   int32_t n_tiles_m, n_tiles_n, n_kblocks;
   const int32_t* kb_cnt;      // [n_tiles_n] number of listed k-blocks per N tile, or nullptr = all k-blocks
   const int32_t* kb_idx;      // [n_tiles_n][n_kblocks]
@@ -72,19 +73,44 @@ struct EpiConsts {
   int lane_r;            // replica of this thread inside the tile
 };
 
+// One bSB update (R10a-f) of a (spin, replica) plus the fp16 split of the new x.
+__device__ __forceinline__ void epi_point(const EpiConsts& ec, float F, float x, float y, float& xn, float& yn) {
+  yn = fmaf(ec.c1, F, fmaf(-ec.c2, x, y));
+  xn = fmaf(ec.c3, yn, x);
+  if (fabsf(xn) > 1.0f) {                    // inelastic wall, strict inequality (R10d)
+    xn = copysignf(1.0f, xn);
+    yn = 0.0f;
+  }
+}
+__device__ __forceinline__ void epi_pack(int j, float xn, uint32_t (&hp)[kChunk / 2], uint32_t (&lp)[kChunk / 2]) {
+  __half h, l;
+  split_half(xn, h, l);
+  const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+  if (j & 1) { hp[j >> 1] |= hb << 16; lp[j >> 1] |= lb << 16; }
+  else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
+}
+
 // fp32 state of one work item (16 spins x this thread's replica) -> registers; masked entries read as 0.
+// Element offsets are 32-bit (the host checks n R < 2^32): one integer add and one wide multiply-add per address.
 __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, float (&xv)[kChunk],
                                          float (&yv)[kChunk]) {
   const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
   const bool r_ok = r < a.R;
-  const float* px = a.x + size_t(i0) * a.R + r;
-  const float* py = a.y + size_t(i0) * a.R + r;
+  uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
+  if (r_ok && i0 + kChunk <= a.n) {          // interior item: no per-element predicates
 #pragma unroll
-  for (int j = 0; j < kChunk; ++j) {
-    const bool ok = r_ok && (i0 + j) < a.n;
-    xv[j] = ok ? px[size_t(j) * a.R] : 0.f;
-    yv[j] = ok ? py[size_t(j) * a.R] : 0.f;
+    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
+      xv[j] = a.x[off];
+      yv[j] = a.y[off];
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
+      const bool ok = r_ok && (i0 + j) < a.n;
+      xv[j] = ok ? a.x[off] : 0.f;
+      yv[j] = ok ? a.y[off] : 0.f;
+    }
   }
 }
 
@@ -92,34 +118,46 @@ __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec
 // (fp32, coalesced across the warp's 32 replicas) and the fp16 split of x' (32 contiguous bytes per thread).
 __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tile, int ch,
                                                  const uint32_t (&v)[kChunk], const float (&xv)[kChunk],
-                                                 const float (&yv)[kChunk]) {
+                                                 const float (&yv)[kChunk], uint32_t stg) {
   const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
   const bool r_ok = r < a.R;
-  float* px = a.x + size_t(i0) * a.R + r;
-  float* py = a.y + size_t(i0) * a.R + r;
+  uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
   uint32_t hp[kChunk / 2], lp[kChunk / 2];    // fp16 pairs (spin i0 + 2q, i0 + 2q + 1) of x_hi', x_lo'
+  if (r_ok && i0 + kChunk <= a.n) {
 #pragma unroll
-  for (int j = 0; j < kChunk; ++j) {
-    const bool ok = r_ok && (i0 + j) < a.n;
-    const float F = __uint_as_float(v[j]);
-    float yn = fmaf(ec.c1, F, fmaf(-ec.c2, xv[j], yv[j]));
-    float xn = fmaf(ec.c3, yn, xv[j]);
-    if (fabsf(xn) > 1.0f) {                  // inelastic wall, strict inequality (R10d)
-      xn = copysignf(1.0f, xn);
-      yn = 0.0f;
+    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
+      float xn, yn;
+      epi_point(ec, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
+      a.x[off] = xn;
+      a.y[off] = yn;
+      epi_pack(j, xn, hp, lp);
     }
-    if (ok) {
-      px[size_t(j) * a.R] = xn;
-      py[size_t(j) * a.R] = yn;
+  } else {
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
+      const bool ok = r_ok && (i0 + j) < a.n;
+      float xn, yn;
+      epi_point(ec, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
+      if (ok) {
+        a.x[off] = xn;
+        a.y[off] = yn;
+      }
+      epi_pack(j, ok ? xn : 0.f, hp, lp);
     }
-    __half h, l;
-    split_half(ok ? xn : 0.f, h, l);
-    const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-    if (j & 1) { hp[j >> 1] |= hb << 16; lp[j >> 1] |= lb << 16; }
-    else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
   }
-  if (r_ok && i0 < a.n) {                      // n_k >= round_up(n, 64) keeps the 16-spin run in bounds
+  if (stg != 0) {
+    // staging tile [128 replicas][64 spins] fp16 per array, rows of 128 B, 16-byte pieces XOR-swizzled by (row & 7):
+    // the layout a TMA box {64, 128} with the 128-byte swizzle expects; x_lo's tile follows x_hi's (16 KB each)
+    const int row = ec.lane_r;
+    const uint32_t base = stg + uint32_t(row) * 128u;
+#pragma unroll
+    for (int q = 0; q < kChunk / 8; ++q) {
+      const uint32_t piece = uint32_t(((ch * kChunk) >> 3) + q) ^ uint32_t(row & 7);
+      ptx::st_shared_v4(base + piece * 16u, hp[4 * q], hp[4 * q + 1], hp[4 * q + 2], hp[4 * q + 3]);
+      ptx::st_shared_v4(base + kStageX + piece * 16u, lp[4 * q], lp[4 * q + 1], lp[4 * q + 2], lp[4 * q + 3]);
+    }
+  } else if (r_ok && i0 < a.n) {               // n_k >= round_up(n, 64) keeps the 16-spin run in bounds
     uint4* ph = reinterpret_cast<uint4*>(a.xh_out + size_t(r) * a.n_k + i0);
     uint4* pl = reinterpret_cast<uint4*>(a.xl_out + size_t(r) * a.n_k + i0);
 #pragma unroll
@@ -132,7 +170,8 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
 
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_xh,
-                  const __grid_constant__ CUtensorMap tm_xl, const DenseArgs a) {
+                  const __grid_constant__ CUtensorMap tm_xl, const __grid_constant__ CUtensorMap tm_oh,
+                  const __grid_constant__ CUtensorMap tm_ol, const DenseArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;       // 128B swizzle needs 1024-byte alignment
   const int kStages = a.n_stages;
@@ -238,6 +277,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     ec.lane_r = quarter * 32 + lane;
     int acc = 0;
     uint32_t acc_phase = 0;
+    // fp16 output staging: two buffers of (x_hi tile, x_lo tile) behind the operand stages, alternated per tile
+    const uint32_t stg_base = smem_base + uint32_t(kStages) * kStageBytes;
+    uint32_t tcount = 0;
     // every warp owns chunk `par` of every tile (possibly fully masked), so that it arrives on tmem_empty once per tile
     auto advance = [&](int& tile, int& ch) {
       ch += P;
@@ -256,12 +298,28 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       const bool nhave = ntile < n_tiles;
       if (nhave) epi_load(a, ec, ntile, nch, xn, yn);
       ptx::tmem_ld_wait();
-      epi_update_store(a, ec, tile, ch, v, xc, yc);
+      const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
+      epi_update_store(a, ec, tile, ch, v, xc, yc, stg);
       if (ntile != tile) {                     // last chunk of this warp in the tile: hand the accumulator stage back
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        if (a.stage_out) {
+          // all epilogue warps have written their pieces of this tile -> one thread hands the two tiles to TMA.
+          // The elected thread first waits until the previous tile's stores have finished reading their buffer, so
+          // that after the barrier every warp may overwrite that buffer (it is the next tile's).
+          ptx::fence_proxy_async();
+          if (ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
+          ptx::named_barrier_sync(1, kEpiWarps * 32);
+          if (ew == 0 && lane == 0) {
+            const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+            ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
+            ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+            ptx::tma_store_commit();
+          }
+          ++tcount;
+        }
       }
       tile = ntile; ch = nch;
       return nhave;
@@ -274,6 +332,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if (!step(tile, ch, xa, ya, xb, yb)) break;
         if (!step(tile, ch, xb, yb, xa, ya)) break;
       }
+      if (a.stage_out && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();   // smem must outlive the bulk reads
     }
   }
 
@@ -413,6 +472,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
                               const qhap_bsb_params& p, float* x, float* y, void* ws_ptr, size_t ws_bytes, cudaStream_t stream) {
   const int32_t n = g.n;
   QHAP_REQUIRE(dtype == QHAP_DENSE_FP16, "dense path takes J in fp16");
+  QHAP_REQUIRE(uint64_t(g.n) * uint64_t(R) < (1ull << 32), "dense path: n * replicas must be below 2^32");
   QHAP_REQUIRE((reinterpret_cast<uintptr_t>(dense_J) & 15) == 0, "dense_J must be 16-byte aligned");
   QHAP_REQUIRE(ws_bytes >= dense_workspace_bytes(n, ld, R), "dense workspace too small");
   Workspace ws(ws_ptr);
@@ -432,7 +492,10 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   const int32_t BN = choose_bn(n, R, skip, p.dense_bn);
   DenseArgs a;
   a.n = n; a.R = R; a.n_k = n_k; a.BN = BN;
-  a.n_stages = std::min(kMaxStages, kSmemBudget / (BN * kBK * 2 + 2 * kStageX));
+  // fp16 copies through TMA stores: the tile must be exactly one 64-column box wide (tile_skip's width); the two
+  // staging buffers (2 x 32 KB) come out of the operand-stage budget
+  a.stage_out = (BN == kBK) ? 1 : 0;
+  a.n_stages = std::min(kMaxStages, (kSmemBudget - (a.stage_out ? 4 * kStageX : 0)) / (BN * kBK * 2 + 2 * kStageX));
   if (const char* e = getenv("QHAP_TUNE_STAGES")) a.n_stages = std::max(1, std::min(a.n_stages, atoi(e)));   // TUNING ONLY
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = int32_t(ceil_div(n, BN));
@@ -476,7 +539,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
     a.c3 = float(p.dt * p.a0);
     a.xh_out = xh[cur ^ 1];
     a.xl_out = xl[cur ^ 1];
-    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_j, tm_h[cur], tm_l[cur], a);
+    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a);
     QHAP_LAUNCH_CHECK();
     cur ^= 1;
   }

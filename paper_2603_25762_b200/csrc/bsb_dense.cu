@@ -12,13 +12,13 @@
 // Jacobi update across CTAs: the fp16 copies are double-buffered (read buffer b, write buffer 1-b); fp32 x, y are
 // private to the tile that owns them and are updated in place.  One launch per step (grid-wide step boundary).
 //
-// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one elected lane),
-// warps 2..9 = epilogue (TMEM lane quarter = warp % 4, two warps per quarter interleave 32-column chunks).
+// Warp roles (576 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one elected lane),
+// warps 2..17 = epilogue (TMEM lane quarter = warp % 4, four warps per quarter interleave 8-column chunks; the state of
+// the next chunk is prefetched into registers; at BN = 64 the fp16 copies leave through shared memory and TMA stores).
 // Pipelines: n_stages shared-memory stages (full/empty mbarriers) and 2 TMEM accumulator stages (tmem_full/tmem_empty).
 #include <cuda.h>
 #include <cuda_fp16.h>
 
-#include <cstdlib>
 #include <vector>
 
 #include "kernels.cuh"
@@ -34,8 +34,8 @@ constexpr int kMaxBN = 256;              // output spins per tile (UMMA N), runt
 constexpr int kMaxStages = 8;             // shared-memory pipeline depth: as many stages as fit (3 at BN = 256, 5 at BN = 64)
 constexpr int kStageX = kBM * kBK * 2;               // 16 KB each for x_hi, x_lo
 constexpr int kSmemBudget = 216 * 1024;              // operand stages; + 1 KB alignment slack + barriers <= 227 KB
-constexpr int kEpiWarps = 8;
-constexpr int kChunk = 16;                // accumulator columns (spins) per tcgen05.ld in the epilogue
+constexpr int kEpiWarps = 16;
+constexpr int kChunk = 8;                // accumulator columns (spins) per tcgen05.ld in the epilogue
 constexpr int kThreads = 64 + 32 * kEpiWarps;
 constexpr int kTmemCols = 512;                       // 2 accumulator stages x 256 columns
 constexpr size_t kSmemBytes = size_t(kSmemBudget) + 1024 /*alignment slack*/ + 256 /*barriers*/;
@@ -292,7 +292,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         ptx::tc_fence_after();
       }
       uint32_t v[kChunk];
-      ptx::tmem_ld_32x32b_x16(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
+      ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
       int ntile = tile, nch = ch;
       advance(ntile, nch);
       const bool nhave = ntile < n_tiles;
@@ -437,18 +437,19 @@ qhap_status make_map(CUtensorMap* m, const void* base, uint64_t inner, uint64_t 
 
 int32_t pitch_of(int32_t n) { return int32_t(ceil_div(n, 64) * 64); }
 
-// Tile width: full GEMM -> minimise waves x width over the persistent grid; tile_skip -> narrow tiles (the step is then
-// bound by the epilogue's state traffic and balances better with more tiles).
+// Tile width: full GEMM -> minimise waves x width over the persistent grid; tile_skip -> 64 (one swizzle box wide: the
+// step is then bound by the epilogue's state traffic, many small tiles balance best and the fp16 copies can leave
+// through TMA stores; measured on cfg1: 43 us at 64, 54-56 us at 96..256).
 int32_t choose_bn(int32_t n, int32_t R, bool tile_skip, int32_t forced) {
-  if (forced >= 16 * (kEpiWarps / 4) && forced <= kMaxBN && forced % 16 == 0) return forced;
+  if (forced >= kChunk * (kEpiWarps / 4) && forced <= kMaxBN && forced % 16 == 0) return forced;
   if (n <= 32) return 32;
+  if (tile_skip) return kBK;
   const int64_t tm = ceil_div(R, kBM), sms = sm_count();
   int32_t best = 128;
   double best_cost = 1e300;
   for (int32_t bn : {64, 96, 128, 160, 192, 224, 256}) {
-    if (tile_skip && bn > 128) break;
     const int64_t tiles = tm * ceil_div(n, bn);
-    const double cost = double(ceil_div(tiles, sms)) * (bn + (tile_skip ? 16 : 4));   // + fixed per-tile overhead
+    const double cost = double(ceil_div(tiles, sms)) * (bn + 4);   // + fixed per-tile overhead
     if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && bn > best)) { best_cost = cost; best = bn; }
   }
   return best;
@@ -496,7 +497,6 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   // staging buffers (2 x 32 KB) come out of the operand-stage budget
   a.stage_out = (BN == kBK) ? 1 : 0;
   a.n_stages = std::min(kMaxStages, (kSmemBudget - (a.stage_out ? 4 * kStageX : 0)) / (BN * kBK * 2 + 2 * kStageX));
-  if (const char* e = getenv("QHAP_TUNE_STAGES")) a.n_stages = std::max(1, std::min(a.n_stages, atoi(e)));   // TUNING ONLY
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = int32_t(ceil_div(n, BN));
   a.n_kblocks = n_kb;

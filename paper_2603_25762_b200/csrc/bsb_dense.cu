@@ -19,6 +19,7 @@
 #include <cuda.h>
 #include <cuda_fp16.h>
 
+#include <cstring>
 #include <vector>
 
 #include "kernels.cuh"
@@ -48,7 +49,11 @@ struct DenseArgs {
   int32_t n_tiles_m, n_tiles_n, n_kblocks;
   const int32_t* kb_cnt;      // [n_tiles_n] number of listed k-blocks per N tile, or nullptr = all k-blocks
   const int32_t* kb_idx;      // [n_tiles_n][n_kblocks]
-  const float* c1;            // [1] dt c0
+  const float* c1;            // [1] dt c0 (dense J), or per-row factors [n] when c1_per_row != 0 (block-compressed J)
+  int32_t c1_per_row;
+  int32_t j_terms;            // 1: J exact in fp16; 2: J = J_hi + J_lo (fp32 weights), a third MMA per k-slice
+  const int32_t* blk_ptr;     // block-compressed J: tile (tn, j-th listed k-block) is block blk_ptr[tn] + j of the
+                              // [blocks x 64][64] block arrays (nullptr: J is the dense matrix)
   float c2, c3;
   float* x;                   // [n][R] fp32, in place
   float* y;
@@ -74,8 +79,8 @@ struct EpiConsts {
 };
 
 // One bSB update (R10a-f) of a (spin, replica) plus the fp16 split of the new x.
-__device__ __forceinline__ void epi_point(const EpiConsts& ec, float F, float x, float y, float& xn, float& yn) {
-  yn = fmaf(ec.c1, F, fmaf(-ec.c2, x, y));
+__device__ __forceinline__ void epi_point(const EpiConsts& ec, float c1, float F, float x, float y, float& xn, float& yn) {
+  yn = fmaf(c1, F, fmaf(-ec.c2, x, y));
   xn = fmaf(ec.c3, yn, x);
   if (fabsf(xn) > 1.0f) {                    // inelastic wall, strict inequality (R10d)
     xn = copysignf(1.0f, xn);
@@ -128,7 +133,8 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
 #pragma unroll
     for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
       float xn, yn;
-      epi_point(ec, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
+      const float c1 = a.c1_per_row ? __ldg(a.c1 + i0 + j) : ec.c1;
+      epi_point(ec, c1, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
       a.x[off] = xn;
       a.y[off] = yn;
       epi_pack(j, xn, hp, lp);
@@ -138,7 +144,8 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
     for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
       const bool ok = r_ok && (i0 + j) < a.n;
       float xn, yn;
-      epi_point(ec, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
+      const float c1 = (a.c1_per_row && (i0 + j) < a.n) ? __ldg(a.c1 + i0 + j) : ec.c1;
+      epi_point(ec, c1, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
       if (ok) {
         a.x[off] = xn;
         a.y[off] = yn;
@@ -169,13 +176,15 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
-dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_xh,
+dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
+                  const __grid_constant__ CUtensorMap tm_xh,
                   const __grid_constant__ CUtensorMap tm_xl, const __grid_constant__ CUtensorMap tm_oh,
                   const __grid_constant__ CUtensorMap tm_ol, const DenseArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;       // 128B swizzle needs 1024-byte alignment
   const int kStages = a.n_stages;
-  const uint32_t kStageJ = uint32_t(a.BN) * kBK * 2, kStageBytes = kStageJ + 2 * kStageX;
+  const uint32_t kTileJ = uint32_t(a.BN) * kBK * 2;                    // one J tile; a second one (J_lo) follows if j_terms == 2
+  const uint32_t kStageJ = kTileJ * uint32_t(a.j_terms), kStageBytes = kStageJ + 2 * kStageX;
   const uint32_t bar_base = smem_base + kSmemBudget;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
@@ -206,7 +215,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   const int n_tiles = a.n_tiles_m * a.n_tiles_n;
-  const uint32_t stage_tx = uint32_t(a.BN) * kBK * 2 + 2u * kStageX;
+  const uint32_t stage_tx = kStageJ + 2u * kStageX;
 
   if (warp == 0) {
     // ===================================================================================== TMA producer
@@ -221,7 +230,13 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t sj = smem_base + stage * kStageBytes;
           ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx);
-          ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
+          if (a.blk_ptr) {
+            const int brow = (a.blk_ptr[tn] + j) * kBK;
+            ptx::tma_load_2d(sj, &tm_j, full_bar(stage), 0, brow);
+            if (a.j_terms == 2) ptx::tma_load_2d(sj + kTileJ, &tm_jl, full_bar(stage), 0, brow);
+          } else {
+            ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
+          }
           ptx::tma_load_2d(sj + kStageJ, &tm_xh, full_bar(stage), kb * kBK, tm * kBM);
           ptx::tma_load_2d(sj + kStageJ + kStageX, &tm_xl, full_bar(stage), kb * kBK, tm * kBM);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -247,12 +262,14 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if (ptx::elect_one()) {
           const uint32_t sj = smem_base + stage * kStageBytes;
           const uint64_t dj = ptx::umma_desc_k_sw128(sj);
+          const uint64_t djl = ptx::umma_desc_k_sw128(sj + kTileJ);
           const uint64_t dh = ptx::umma_desc_k_sw128(sj + kStageJ);
           const uint64_t dl = ptx::umma_desc_k_sw128(sj + kStageJ + kStageX);
 #pragma unroll
           for (int kk = 0; kk < kBK / 16; ++kk) {                         // UMMA_K = 16 for 16-bit inputs: +32 B per step
             ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
             ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
+            if (a.j_terms == 2) ptx::umma_f16(d_tmem, dh + 2u * kk, djl + 2u * kk, idesc, 1u);   // x_lo J_lo ~ 2^-22: dropped
           }
           ptx::umma_commit(empty_bar(stage));                            // frees the smem stage when these MMAs are done
           if (j == nkb - 1) ptx::umma_commit(tfull_bar(acc));            // accumulator complete -> epilogue
@@ -272,7 +289,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     const int par = ew >> 2;                   // the kEpiWarps / 4 warps of a quarter take chunks par, par + P, par + 2P, ...
     constexpr int P = kEpiWarps / 4;
     EpiConsts ec;
-    ec.c1 = __ldg(a.c1) * (1.0f / kXScale);    // accumulator = 2^15 F
+    ec.c1 = a.c1_per_row ? 0.f : __ldg(a.c1) * (1.0f / kXScale);    // accumulator = 2^15 F (per-row factors include it)
     ec.c2 = a.c2; ec.c3 = a.c3;
     ec.lane_r = quarter * 32 + lane;
     int acc = 0;
@@ -396,6 +413,68 @@ __global__ void __launch_bounds__(32) kb_list_kernel(int32_t n_kblocks, const in
   }
 }
 
+// ------------------------------------------------------------------- block-compressed J (64 x 64 fp16 tiles) from a CSR
+// max |J| over all entries (order-independent: integer max of the absolute value's bit pattern)
+__global__ void __launch_bounds__(256) absmax_kernel(int64_t nnz, const float* __restrict__ jval, uint32_t* __restrict__ out) {
+  uint32_t m = 0;
+  for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nnz; e += int64_t(gridDim.x) * blockDim.x)
+    m = max(m, __float_as_uint(fabsf(jval[e])));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
+// scale[0] = 2^e with max|J| 2^e in [2^13, 2^14) (1 for an all-zero J or when `unit` is set: integer weights are used as
+// they are); c1row[i] = c1[instance of i] 2^-15 / scale[0]  (exact power-of-two factors)
+__global__ void __launch_bounds__(256) block_scale_kernel(int32_t n, int32_t n_inst, const int32_t* __restrict__ inst_ptr,
+                                                          const float* __restrict__ c1, const uint32_t* __restrict__ amax,
+                                                          int32_t unit, float* __restrict__ scale, float* __restrict__ c1row) {
+  const float mx = __uint_as_float(*amax);
+  const float sc = (unit || !(mx > 0.f)) ? 1.0f : ldexpf(1.0f, 13 - ilogbf(mx));
+  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) scale[0] = sc;
+  if (i >= n) return;
+  int inst = 0;
+  if (n_inst > 1) {
+    int lo = 0, hi = n_inst;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (inst_ptr[mid] <= i) lo = mid; else hi = mid;
+    }
+    inst = lo;
+  }
+  c1row[i] = c1[inst] * (1.0f / kXScale) * (1.0f / sc);
+}
+
+// One warp per row: scatter the row's entries into their tiles.  Tile (tn, kb) is block blk_ptr[tn] + (rank of kb in the
+// ascending list kb_idx[tn][0 .. kb_cnt[tn])).  J_hi = fp16(J scale), J_lo = fp16(J scale - J_hi).
+__global__ void __launch_bounds__(256) block_fill_kernel(int32_t n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
+                                                         const float* __restrict__ jval, int32_t n_kblocks,
+                                                         const int32_t* __restrict__ kb_cnt, const int32_t* __restrict__ kb_idx,
+                                                         const int32_t* __restrict__ blk_ptr, const float* __restrict__ scale,
+                                                         __half* __restrict__ jh, __half* __restrict__ jl) {
+  const int32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n) return;
+  const int lane = threadIdx.x & 31;
+  const int32_t tn = a / kBK;
+  const int32_t* list = kb_idx + size_t(tn) * n_kblocks;
+  const int32_t cnt = kb_cnt[tn], base = blk_ptr[tn];
+  const float sc = scale[0];
+  for (int32_t e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
+    const int32_t c = col[e], kb = c / kBK;
+    int lo = 0, hi = cnt;                                  // list[lo] <= kb < list[hi]
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (list[mid] <= kb) lo = mid; else hi = mid;
+    }
+    const size_t idx = (size_t(base + lo) * kBK + size_t(a % kBK)) * kBK + size_t(c % kBK);
+    const float vs = jval[e] * sc;
+    const __half h = __float2half_rn(vs);
+    jh[idx] = h;
+    if (jl) jl[idx] = __float2half_rn(vs - __half2float(h));
+  }
+}
+
 // ------------------------------------------------------------------------------------------- host side
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -502,7 +581,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.n_kblocks = n_kb;
   a.kb_cnt = skip ? kb_cnt : nullptr;
   a.kb_idx = skip ? kb_idx : nullptr;
-  a.c1 = c1_dev;
+  a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
 
   static bool attr_set = false;
@@ -539,7 +618,145 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
     a.c3 = float(p.dt * p.a0);
     a.xh_out = xh[cur ^ 1];
     a.xl_out = xl[cur ^ 1];
-    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a);
+    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a);
+    QHAP_LAUNCH_CHECK();
+    cur ^= 1;
+  }
+  return QHAP_OK;
+}
+
+}  // namespace qhap
+
+// ------------------------------------------------------------------------------------------------------------------
+// Block path: the same tcgen05 step on a BLOCK-COMPRESSED J built from the CSR (no n x n matrix): only the 64 x 64 tiles
+// that hold a non-zero are stored ([blocks x 64][64] fp16, J_hi and -- for fp32 weights -- J_lo), one TMA box each.
+// For banded graphs (reads sorted by start, SNPs in genome order, block-diagonal batches of them) that is a few tiles
+// per 64 rows; a graph whose tiles would exceed the capacity below (long-range Pore-C edges) is refused and belongs on
+// the CSR path.  Batches: c1 is looked up per row (instances may end inside a tile).
+namespace qhap {
+
+namespace {
+// capacity of the tile arrays: 16x the CSR's own entries, plus one (possibly empty) tile per 64 rows
+int64_t block_capacity(int32_t n, int64_t nnz) { return 16 * nnz / (kBK * kBK) + ceil_div(n, kBK) + 1; }
+}  // namespace
+
+size_t block_workspace_bytes(int32_t n, int64_t nnz, int32_t R) {
+  Workspace ws(nullptr);
+  const size_t copy = size_t(R) * pitch_of(n);
+  ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy);
+  const size_t n_t = size_t(ceil_div(n, kBK));
+  ws.take<int32_t>(n_t + 1);              // kb_cnt
+  ws.take<int32_t>(n_t + 1);              // blk_ptr
+  ws.take<int32_t>(n_t * n_t);            // kb_idx
+  ws.take<int32_t>(n_t * n_t);            // flags
+  ws.take<float>(size_t(n));              // c1row
+  ws.take<uint32_t>(4);                   // absmax, scale
+  ws.take<int64_t>(2);                    // total blocks, overflow
+  const size_t cap = size_t(block_capacity(n, nnz)) * kBK * kBK;
+  ws.take<__half>(cap); ws.take<__half>(cap);
+  return ws.used();
+}
+
+qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weight_mode, int32_t R, int32_t n_inst,
+                              const int32_t* inst_ptr_dev, const float* c1_dev, const qhap_bsb_params& p, float* x, float* y,
+                              void* ws_ptr, size_t ws_bytes, cudaStream_t stream) {
+  const int32_t n = g.n;
+  QHAP_REQUIRE(uint64_t(n) * uint64_t(R) < (1ull << 32), "block path: n * replicas must be below 2^32");
+  QHAP_REQUIRE(ws_bytes >= block_workspace_bytes(n, g.nnz, R), "block workspace too small");
+  Workspace ws(ws_ptr);
+  const int32_t n_k = pitch_of(n);
+  const size_t copy = size_t(R) * n_k;
+  __half* xh[2];
+  __half* xl[2];
+  xh[0] = ws.take<__half>(copy); xl[0] = ws.take<__half>(copy);
+  xh[1] = ws.take<__half>(copy); xl[1] = ws.take<__half>(copy);
+  const int32_t n_t = int32_t(ceil_div(n, kBK));
+  int32_t* kb_cnt = ws.take<int32_t>(size_t(n_t) + 1);
+  int32_t* blk_ptr = ws.take<int32_t>(size_t(n_t) + 1);
+  int32_t* kb_idx = ws.take<int32_t>(size_t(n_t) * n_t);
+  int32_t* flags = ws.take<int32_t>(size_t(n_t) * n_t);
+  float* c1row = ws.take<float>(size_t(n));
+  uint32_t* scal = ws.take<uint32_t>(4);
+  int64_t* totals = ws.take<int64_t>(2);
+  const int64_t cap_blocks = block_capacity(n, g.nnz);
+  const size_t cap = size_t(cap_blocks) * kBK * kBK;
+  __half* jh = ws.take<__half>(cap);
+  __half* jl = ws.take<__half>(cap);
+  const bool two_terms = weight_mode == QHAP_WEIGHT_FX;      // integer counts are exact in fp16 (|J| <= 2048 checked below)
+
+  // tile lists (the same kernels as tile_skip at BN = 64), block offsets, capacity check (one host synchronisation)
+  QHAP_CUDA_TRY(cudaMemsetAsync(flags, 0, sizeof(int32_t) * size_t(n_t) * n_t, stream));
+  QHAP_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(uint32_t) * 4, stream));
+  kb_flag_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, kBK, n_t, flags);
+  QHAP_LAUNCH_CHECK();
+  kb_list_kernel<<<n_t, 32, 0, stream>>>(n_t, flags, kb_cnt, kb_idx);
+  QHAP_LAUNCH_CHECK();
+  QHAP_TRY(exclusive_scan_i32(kb_cnt, blk_ptr, n_t, totals, reinterpret_cast<int32_t*>(totals + 1), stream));
+  if (g.nnz > 0) {
+    absmax_kernel<<<int(std::min<int64_t>(ceil_div(g.nnz, 256), int64_t(sm_count()) * 8)), 256, 0, stream>>>(g.nnz, jval, scal);
+    QHAP_LAUNCH_CHECK();
+  }
+  int64_t total_blocks = 0;
+  uint32_t amax_bits = 0;
+  QHAP_CUDA_TRY(cudaMemcpyAsync(&total_blocks, totals, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
+  QHAP_CUDA_TRY(cudaMemcpyAsync(&amax_bits, scal, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+  QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
+  if (total_blocks > cap_blocks) {
+    set_error("block path: %lld non-empty 64 x 64 tiles exceed the capacity %lld (16 x nnz / 4096 + n / 64): the graph is not "
+              "banded enough (long-range edges) -- use the CSR path (path = 2)", (long long)total_blocks, (long long)cap_blocks);
+    return QHAP_ERR_RANGE;
+  }
+  float amax;
+  memcpy(&amax, &amax_bits, sizeof(float));
+  if (!two_terms && amax > 2048.0f) {
+    set_error("block path: |J| = %g is not exactly representable in fp16 (> 2048)", double(amax));
+    return QHAP_ERR_RANGE;
+  }
+  float* scale = reinterpret_cast<float*>(scal + 1);
+  block_scale_kernel<<<int(ceil_div(std::max(n, 1), 256)), 256, 0, stream>>>(n, n_inst, inst_ptr_dev, c1_dev, scal, two_terms ? 0 : 1,
+                                                                            scale, c1row);
+  QHAP_LAUNCH_CHECK();
+  QHAP_CUDA_TRY(cudaMemsetAsync(jh, 0, sizeof(__half) * size_t(total_blocks) * kBK * kBK, stream));
+  if (two_terms) QHAP_CUDA_TRY(cudaMemsetAsync(jl, 0, sizeof(__half) * size_t(total_blocks) * kBK * kBK, stream));
+  block_fill_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, jval, n_t, kb_cnt, kb_idx, blk_ptr,
+                                                                            scale, jh, two_terms ? jl : nullptr);
+  QHAP_LAUNCH_CHECK();
+
+  DenseArgs a;
+  a.n = n; a.R = R; a.n_k = n_k; a.BN = kBK;
+  a.stage_out = 1;
+  a.j_terms = two_terms ? 2 : 1;
+  a.n_stages = std::min(kMaxStages, (kSmemBudget - 4 * kStageX) / (a.j_terms * kBK * kBK * 2 + 2 * kStageX));
+  a.n_tiles_m = int32_t(ceil_div(R, kBM));
+  a.n_tiles_n = n_t;
+  a.n_kblocks = n_t;
+  a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
+  a.c1 = c1row; a.c1_per_row = 1;
+  a.x = x; a.y = y;
+  QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
+
+  CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2];
+  const uint64_t brows = uint64_t(std::max<int64_t>(total_blocks, 1)) * kBK;
+  QHAP_TRY(make_map(&tm_jh, jh, kBK, brows, kBK, kBK));
+  QHAP_TRY(make_map(&tm_jl, two_terms ? jl : jh, kBK, brows, kBK, kBK));
+  for (int b = 0; b < 2; ++b) {
+    QHAP_TRY(make_map(&tm_h[b], xh[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
+    QHAP_TRY(make_map(&tm_l[b], xl[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
+  }
+  {
+    dim3 grid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
+    split_x_kernel<<<grid, 256, 0, stream>>>(n, R, n_k, x, xh[0], xl[0]);
+    QHAP_LAUNCH_CHECK();
+  }
+  const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
+  int cur = 0;
+  for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
+    const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
+    a.c2 = float(p.dt * (p.a0 - a_k));
+    a.c3 = float(p.dt * p.a0);
+    a.xh_out = xh[cur ^ 1];
+    a.xl_out = xl[cur ^ 1];
+    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a);
     QHAP_LAUNCH_CHECK();
     cur ^= 1;
   }

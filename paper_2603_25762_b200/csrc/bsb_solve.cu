@@ -22,19 +22,19 @@ struct SolveWs {
   size_t dense_bytes;
 };
 
-SolveWs carve(Workspace& ws, int32_t n, int64_t nnz, int32_t n_inst, int32_t R, bool dense, int32_t ld) {
+SolveWs carve(Workspace& ws, int32_t n, int64_t nnz, int32_t n_inst, int32_t R, bool dense, int32_t ld, bool block = false) {
   SolveWs s;
   s.inst_ptr = ws.take<int32_t>(size_t(n_inst) + 1);
   s.jval = ws.take<float>(size_t(nnz));
   s.sumsq = ws.take<double>(size_t(n_inst) + size_t(n));
   s.c1 = ws.take<float>(size_t(n_inst));
-  s.x_alt = dense ? nullptr : ws.take<float>(size_t(n) * R);
+  s.x_alt = (dense || block) ? nullptr : ws.take<float>(size_t(n) * R);
   s.cut = ws.take<int64_t>(size_t(n_inst) * R);
   s.wtot = ws.take<int64_t>(size_t(n_inst));
   s.best_cut = ws.take<int64_t>(size_t(n_inst));
   s.best_replica = ws.take<int32_t>(size_t(n_inst));
-  s.dense_bytes = dense ? dense_workspace_bytes(n, ld, R) : 0;
-  s.dense = dense ? static_cast<void*>(ws.take<char>(s.dense_bytes)) : nullptr;
+  s.dense_bytes = dense ? dense_workspace_bytes(n, ld, R) : (block ? block_workspace_bytes(n, nnz, R) : 0);
+  s.dense = (dense || block) ? static_cast<void*>(ws.take<char>(s.dense_bytes)) : nullptr;
   return s;
 }
 
@@ -54,7 +54,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   int path = p->path;
   const int32_t res_rc = (path == 0 || path == 3) ? resident_plan(graph->n, graph->nnz, p->replicas) : 0;
   if (path == 0) path = res_rc > 0 ? 3 : ((dense_J && n_inst == 1) ? 1 : 2);
-  QHAP_REQUIRE(path >= 1 && path <= 3, "path must be 0, 1, 2 or 3");
+  QHAP_REQUIRE(path >= 1 && path <= 4, "path must be 0, 1, 2, 3 or 4");
   QHAP_REQUIRE(path != 3 || res_rc > 0, "resident path: problem too large for shared memory (needs n R <= 65536)");
   if (path == 1) {
     QHAP_REQUIRE(dense_J && n_inst == 1, "dense path needs dense_J and a single instance");
@@ -63,7 +63,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   }
   const int32_t n = graph->n, R = p->replicas;
   Workspace ws(workspace);
-  SolveWs s = carve(ws, n, graph->nnz, n_inst, R, path == 1, dense_ld);
+  SolveWs s = carve(ws, n, graph->nnz, n_inst, R, path == 1, dense_ld, path == 4);
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
@@ -89,6 +89,8 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   if (p->steps_run > 0 && n > 0) {
     if (path == 1) {
       QHAP_TRY(dense_solve_steps(g, dense_J, dense_ld, dense_dtype, R, s.c1, *p, x, y, s.dense, s.dense_bytes, stream));
+    } else if (path == 4) {
+      QHAP_TRY(block_solve_steps(g, s.jval, p->weight_mode, R, n_inst, s.inst_ptr, s.c1, *p, x, y, s.dense, s.dense_bytes, stream));
     } else if (path == 3) {
       QHAP_TRY(resident_solve_steps(g, s.jval, R, res_rc, n_inst, s.inst_ptr, s.c1, *p, x, y, stream));
     } else {

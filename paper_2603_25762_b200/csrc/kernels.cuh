@@ -59,6 +59,12 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
                               const float* c1_dev, const qhap_bsb_params& p, float* x, float* y, void* ws, size_t ws_bytes,
                               cudaStream_t stream);
 
+// block-compressed J built from the CSR (64 x 64 fp16 tiles that hold a non-zero), same tcgen05 step; batches allowed
+size_t block_workspace_bytes(int32_t n, int64_t nnz, int32_t R);
+qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weight_mode, int32_t R, int32_t n_inst,
+                              const int32_t* inst_ptr_dev, const float* c1_dev, const qhap_bsb_params& p, float* x, float* y,
+                              void* ws, size_t ws_bytes, cudaStream_t stream);
+
 // ---- bsb_resident.cu: whole solve in shared memory for small problems (one CTA owns all spins of RC replicas)
 int32_t resident_plan(int32_t n, int64_t nnz, int32_t R);   // replicas per CTA, 0 = not applicable
 qhap_status resident_solve_steps(const CsrView& g, const float* jval, int32_t R, int32_t RC, int32_t n_inst,

@@ -221,6 +221,7 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
     xt = xo * (1.0 + 2.0 ** -23); yt = yo * (1.0 + 2.0 ** -23)        # the oracle's twin, one fp32 ulp away
     out = dict(free_dx=0.0, free_dy=0.0, resync_dx=0.0, resync_dy=0.0, horizon=steps, excluded=0, tail_dx=0.0)
     horizon_open = True
+    tainted = np.zeros(R, bool)
     for k in range(steps):
         # (a) resynchronised single step from the oracle's current state rounded to fp32
         xs32, ys32 = xo.astype(np.float32), yo.astype(np.float32)
@@ -237,13 +238,22 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         twin = max(np.abs(xt - xo).max(), np.abs(yt - yo).max())
         if horizon_open and twin > TWIN_TOL and not expect_full:
             out["horizon"], horizon_open = k, False
-        dx, dy, exc = diff(xh, yh, xo, yo, xpre)
+        # a replica whose GPU run took the OTHER wall decision at a marginal pre-clamp |x| (within WALL_BAND of 1) follows a
+        # legitimately different trajectory from then on (the wall is a discontinuity; replicas are independent): it leaves
+        # the free-running comparison, and the number of such replicas is bounded below
+        marginal = np.abs(np.abs(xpre) - 1.0) < WALL_BAND
+        flipped = marginal & ((yh == 0.0) != (yo == 0.0))
+        tainted |= flipped.any(axis=0)
+        keep = ~tainted
+        dx, dy, exc = diff(xh[:, keep], yh[:, keep], xo[:, keep], yo[:, keep], xpre[:, keep])
         if horizon_open:
             out["free_dx"], out["free_dy"] = max(out["free_dx"], dx), max(out["free_dy"], dy)
             out["excluded"] += exc
             assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, f"free-running step {k} (twin drift {twin:.1e}): max|dx| {dx:.3e}, max|dy| {dy:.3e}"
         else:
             out["tail_dx"] = max(out["tail_dx"], dx)
+    out["tainted"] = int(tainted.sum())
+    assert out["tainted"] <= max(2, 0.05 * R), out
     assert out["excluded"] <= 1e-3 * n * R * steps * 2
     assert out["horizon"] >= min(steps, MIN_HORIZON), out
     return out
@@ -252,7 +262,7 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
 def fmt_traj(o):
     return (f"free-running max|dx| {o['free_dx']:.2e} max|dy| {o['free_dy']:.2e} over {o['horizon']} steps "
             f"(after the horizon: {o['tail_dx']:.1e}); resync max|dx| {o['resync_dx']:.2e} max|dy| {o['resync_dy']:.2e}; "
-            f"excluded {o['excluded']}")
+            f"excluded {o['excluded']}, replicas dropped after a marginal wall flip {o.get('tainted', 0)}")
 
 
 def test_init_state_matches_generator(B, oracle, torch_mod):
@@ -407,6 +417,55 @@ def test_dense_solve_quality_cfg0(B, oracle, torch_mod):
         gse, _ = ser_reads(oracle, fr, res["best_spins"].cpu().numpy())
         ose, _ = ser_reads(oracle, fr, ores["best_spins"])
         assert gse <= ose + 0.001
+
+
+# ------------------------------------------------------- (3') tcgen05 step on a block-compressed J built from the CSR
+def test_block_path_read_graph_equals_dense_tile_skip(B, oracle, torch_mod):
+    """Integer read graph: path 4 stores only the non-empty 64 x 64 tiles of J; same MMAs in the same order as the
+    dense tile_skip step at BN = 64 -> bit-identical states."""
+    fr, p, g, w, J = dense_case(B, oracle, "cfg1-scaled")
+    dg = B.upload_csr(g)
+    outs = []
+    for path in (1, 4):
+        res = B.qhap_bsb_solve(dg, replicas=200, steps_total=p["T"], steps_run=25, seed=p["seed"], weight_mode=1, path=path,
+                               dense_J=J if path == 1 else None, finalize=False, tile_skip=1, dense_bn=64)
+        outs.append(res)
+    assert torch_mod.equal(outs[0]["x"], outs[1]["x"]) and torch_mod.equal(outs[0]["y"], outs[1]["y"])
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, 136, p["T"], p["seed"], steps=20, path=4)
+    print(f"block path cfg1-scaled: {fmt_traj(o)}")
+
+
+def test_block_path_snp_graph_batched(B, oracle, torch_mod):
+    """fp32 SNP weights (J = J_hi + J_lo, three MMAs per k-slice), block-diagonal batch with per-instance c0 whose
+    instances end inside tiles; against the oracle and against the CSR path; full solve quality."""
+    fr, p = synth.make_config(3, scale=0.01)
+    g = oracle.snp_graph(fr, 3, 0.1)
+    win = synth.block_windows(fr.n_snp, 500, 450)
+    bs = oracle.block_split(g, win)
+    o = compare_trajectory(B, oracle, torch_mod, bs, bs["w_fx"], 2, bs["n"], 256, p["T"], p["seed"], steps=30,
+                           inst_ptr=bs["inst_ptr"], path=4)
+    print(f"block path cfg3-scaled batched: {fmt_traj(o)}")
+    dg = B.upload_csr(bs)
+    R, T = 64, 400
+    rb = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, seed=p["seed"], weight_mode=2, path=4)
+    rs = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, seed=p["seed"], weight_mode=2, path=2)
+    cb, cs = rb["best_cut"].cpu().numpy(), rs["best_cut"].cpu().numpy()
+    assert np.all(cb >= cs - 0.005 * np.abs(cs)), (cb, cs)
+    spins = rb["best_spins"].cpu().numpy()
+    for b in range(len(win)):
+        lo, hi = int(bs["inst_ptr"][b]), int(bs["inst_ptr"][b + 1])
+        rp = (bs["row_ptr"][lo:hi + 1] - bs["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(bs["row_ptr"][lo]), int(bs["row_ptr"][hi]))
+        ccut, _ = oracle.cut_eval(rp, (bs["col"][sl] - lo).astype(np.int32), bs["w_fx"][sl], spins[lo:hi])
+        assert ccut[0] == cb[b]
+
+
+def test_block_path_refuses_long_range_graph(B, oracle, torch_mod):
+    """Pore-C long-range edges: the tiles would exceed the capacity -> QHAP_ERR_RANGE, no silent fallback."""
+    fr, p = synth.make_config(4, scale=0.02)
+    g = oracle.snp_graph(fr, 3, 0.1)
+    with pytest.raises(B.QhapError):
+        B.qhap_bsb_solve(B.upload_csr(g), replicas=128, steps_total=10, seed=1, weight_mode=2, path=4, finalize=False)
 
 
 # -------------------------------------------------------------------------------- full solve: quality and phasing

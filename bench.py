@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (1 = the config the metric is quoted on)")
-    ap.add_argument("--path", default="auto", choices=["auto", "dense", "dense-full", "sparse"],
+    ap.add_argument("--path", default="auto", choices=["auto", "dense", "dense-full", "sparse", "block"],
                     help="bSB step kernel: dense = tcgen05 tiles over the non-zero k-blocks of J (tile_skip, bit-identical to "
                          "dense-full = the whole N x N GEMM); sparse = CSR; auto = dense")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -206,10 +206,12 @@ def run_ours(args):
     n = fr.n_snp if snp else fr.n_frag
     seed = parallel.rank_seed(p["seed"], rank)
     if snp:
-        assert args.path in ("auto", "sparse"), "the SNP graphs (configs 3, 4) run on the sparse CSR path"
-        path, tile_skip = 2, 0
+        assert args.path in ("auto", "sparse", "block"), "the SNP graphs (configs 3, 4) have no dense J"
+        # auto: banded SNP graphs (config 3's blocks) -> tcgen05 step on the block-compressed J; long-range Pore-C graph -> CSR
+        path = {"auto": 4 if "porec_edges" not in p else 2, "sparse": 2, "block": 4}[args.path]
+        tile_skip = 0
     else:
-        path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1}[args.path]
+        path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1, "block": 4}[args.path]
         tile_skip = 0 if args.path == "dense-full" else 1
     dense_dtype = B.QHAP_DENSE_FP16 if path == 1 else B.QHAP_DENSE_NONE
     win = synth.block_windows(fr.n_snp, p["block"], p["stride"]) if "block" in p else None
@@ -226,7 +228,7 @@ def run_ours(args):
         if snp:
             g0 = B.qhap_build_snp_graph(frags, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
             g = B.qhap_block_split(g0, win_mine) if win is not None else g0
-            res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=2, cut_per_replica=False,
+            res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, cut_per_replica=False,
                                    workspace=state.get("ws"))
             state["ws"] = res["workspace"]
             cut, spins = res["best_cut"], res["best_spins"]
@@ -359,20 +361,22 @@ def run_ours(args):
         roofline = {"kernel": "sparse_step_kernel", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
                     "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms, "peak_source": peaks["which"]}
         roofline["frac"] = roofline["achieved"] / roofline["peak"]
-    elif tile_skip:
+    elif tile_skip or path == 4:
         # algorithmic bytes per launch: fp32 state 16 B + fp16 split copies written once (4 B) and read at
         # least once (4 B) per spin-update + the non-zero 64 x 64 fp16 blocks of J once
         hg = g.to_host()                              # bookkeeping for the byte count only
-        rows = np.repeat(np.arange(n, dtype=np.int64), np.diff(hg["row_ptr"]))
+        rows = np.repeat(np.arange(g.n, dtype=np.int64), np.diff(hg["row_ptr"]))
         nz_blocks = int(np.unique((rows // 64) * (1 << 32) + hg["col"].astype(np.int64) // 64).size)
-        alg_bytes = 24.0 * n * R + nz_blocks * 64 * 64 * 2.0
-        roofline = {"kernel": "dense_step_kernel (tile_skip)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9,
+        j_terms = 2 if (path == 4 and snp) else 1     # fp32 SNP weights are stored as J_hi + J_lo
+        alg_bytes = 24.0 * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms
+        roofline = {"kernel": "dense_step_kernel (tile_skip)" if path == 1 else "dense_step_kernel (block-compressed J)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9,
                     "peak": peaks["hbm"], "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms,
                     "peak_source": peaks["which"], "nonzero_64x64_blocks_of_J": nz_blocks}
         roofline["frac"] = roofline["achieved"] / roofline["peak"]
-        full_ms, _ = time_steps(1, 0, 200)            # the same kernel over ALL k-blocks (north_star's dense GEMM), 200 launches
-        extra["roofline_dense_full"] = tensor_roofline(full_ms)
-        extra["roofline_dense_full"]["spin_updates_per_s"] = n * R / (full_ms * 1e-3)
+        if path == 1:
+            full_ms, _ = time_steps(1, 0, 200)        # the same kernel over ALL k-blocks (north_star's dense GEMM), 200 launches
+            extra["roofline_dense_full"] = tensor_roofline(full_ms)
+            extra["roofline_dense_full"]["spin_updates_per_s"] = n * R / (full_ms * 1e-3)
     else:
         roofline = tensor_roofline(step_ms)
     prof = ROOT / "profiles" / "roofline_traffic.csv"              # dram bytes per launch from the committed ncu captures
@@ -389,7 +393,7 @@ def run_ours(args):
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if blocks else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": workload_name(args.config, fr, p),
                       "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM)" if tile_skip else " full GEMM"),
-                               2: "sparse-csr"}[path],
+                               2: "sparse-csr", 4: "tcgen05 step on the block-compressed J (64 x 64 tiles built from the CSR)"}[path],
                       "weight_mode": "fixed-point Eq. 14" if snp else "D-C", "replicas_per_gpu": R, "spins_solved": n_solved, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                       "parallelism": f"blocks x{world} (strong)" if blocks else f"replicas x{world} (weak)"},
            "region_ms": ms, "edges_replicas_per_s": edges * R * T * (1 if blocks else world) / (ms * 1e-3), "undirected_edges": edges,

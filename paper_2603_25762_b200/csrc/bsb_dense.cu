@@ -214,6 +214,12 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
+  // Programmatic dependent launch: the next step's CTAs may be scheduled as soon as SMs free up (their prologue above
+  // -- barrier init, TMEM allocation, descriptor prefetch -- overlaps this step's tail); everything below reads state
+  // written by the previous step, so it first waits for that grid to have completed and flushed.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
   const int n_tiles = a.n_tiles_m * a.n_tiles_n;
   const uint32_t stage_tx = kStageJ + 2u * kStageX;
 
@@ -476,6 +482,24 @@ __global__ void __launch_bounds__(256) block_fill_kernel(int32_t n, const int32_
 }
 
 // ------------------------------------------------------------------------------------------- host side
+// One step launch with the programmatic-stream-serialization attribute (see the kernel: griddepcontrol.wait).
+qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, const CUtensorMap& tjl, const CUtensorMap& th,
+                        const CUtensorMap& tl, const CUtensorMap& toh, const CUtensorMap& tol, const DenseArgs& a) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(unsigned(grid));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_step_kernel, tj, tjl, th, tl, toh, tol, a));
+  QHAP_LAUNCH_CHECK();
+  return QHAP_OK;
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -618,8 +642,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
     a.c3 = float(p.dt * p.a0);
     a.xh_out = xh[cur ^ 1];
     a.xl_out = xl[cur ^ 1];
-    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a);
-    QHAP_LAUNCH_CHECK();
+    QHAP_TRY(launch_step(grid, stream, tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a));
     cur ^= 1;
   }
   return QHAP_OK;
@@ -756,8 +779,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
     a.c3 = float(p.dt * p.a0);
     a.xh_out = xh[cur ^ 1];
     a.xl_out = xl[cur ^ 1];
-    dense_step_kernel<<<grid, kThreads, kSmemBytes, stream>>>(tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a);
-    QHAP_LAUNCH_CHECK();
+    QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a));
     cur ^= 1;
   }
   return QHAP_OK;

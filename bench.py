@@ -319,6 +319,44 @@ def run_ours(args):
     e2e_ms, _ = timed(e2e_pass, max(1, min(args.warmup, 2)), max(2, min(args.steps, 3)))
     e2e_value = work / (e2e_ms * 1e-3)
 
+    # ---- phases of one pass (CUDA events around each C-ABI call; one extra untimed-by-the-headline pass)
+    def phase_times():
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        flush.zero_()
+        torch.cuda.synchronize()
+        ev[0].record()
+        if snp:
+            g0 = B.qhap_build_snp_graph(dfr, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
+            gg = B.qhap_block_split(g0, win_mine) if win is not None else g0
+            JJ = None
+        else:
+            gg, JJ = B.qhap_build_read_graph(dfr, weight_mode=mode, dense_dtype=dense_dtype)
+            g0 = gg
+        ev[1].record()
+        res = B.qhap_bsb_solve(gg, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=JJ, tile_skip=tile_skip,
+                               cut_per_replica=False, workspace=state.get("ws"))
+        ev[2].record()
+        sp = res["best_spins"]
+        if snp:
+            if win is not None and world == 1:
+                sp = B.qhap_block_stitch(fr.n_snp, win_mine, sp)
+            B.qhap_phase_readout_snps(dfr.h1, sp[:fr.n_snp] if sp.numel() >= fr.n_snp else sp)
+        else:
+            B.qhap_phase_readout_reads(dfr, sp)
+        ev[3].record()
+        torch.cuda.synchronize()
+        t = [ev[i].elapsed_time(ev[i + 1]) for i in range(3)]
+        # algorithmic bytes of the build (DESIGN.md 4.1 / 4.2): fragment entries in, directed edges out (+ dense J)
+        if snp:
+            b_bytes = 6.0 * fr.nnz + 20.0 * g0.nnz
+        else:
+            b_bytes = 5.0 * fr.nnz + 16.0 * g0.nnz + (2.0 * JJ.numel() if JJ is not None else 0.0)
+        return {"graph_build_ms": t[0], "bsb_solve_ms": t[1], "readout_ms": t[2], "graph_build_algorithmic_bytes": b_bytes,
+                "graph_build_GBps": b_bytes / (t[0] * 1e-3) / 1e9, "graph_build_frac_of_hbm_peak": b_bytes / (t[0] * 1e-3) / 1e9 / measured_peaks()["hbm"],
+                "directed_edges": int(g0.nnz)}
+
+    phases = phase_times()
+
     # ---- roofline of the dominant kernel (the bSB step): launches timed with CUDA events on the launching stream
     J = None
     if path == 1:
@@ -355,9 +393,13 @@ def run_ours(args):
     if path == 2:
         # algorithmic bytes per launch: 16 B of fp32 state per spin-update (read x, read y, write y, write x')
         # + the CSR once per launch (int32 col + fp32 val per directed entry, int32 row_ptr per row)
-        # (+ SURVEY 8(d): 4 B per replica for every non-zero whose column lies outside the L2-resident band: config 4's
-        # long-range Pore-C entries -- not counted here, so the figure is a lower bound of the traffic the method needs)
-        alg_bytes = 16.0 * g.n * R + 8.0 * g.nnz + 4.0 * (g.n + 1)
+        # + SURVEY 8(d): 4 B per replica for every non-zero whose column lies far outside the swept band (|col - row| > 4096:
+        # config 4's long-range Pore-C entries), whose x rows cannot come from the cached neighbourhood
+        hg = g.to_host()                              # bookkeeping for the byte count only
+        rows = np.repeat(np.arange(g.n, dtype=np.int64), np.diff(hg["row_ptr"]))
+        long_range = int((np.abs(hg["col"].astype(np.int64) - rows) > 4096).sum())   # x rows far outside the swept band
+        alg_bytes = 16.0 * g.n * R + 8.0 * g.nnz + 4.0 * (g.n + 1) + 4.0 * R * long_range
+        extra["long_range_nnz"] = long_range
         roofline = {"kernel": "sparse_step_kernel", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
                     "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms, "peak_source": peaks["which"]}
         roofline["frac"] = roofline["achieved"] / roofline["peak"]
@@ -379,15 +421,14 @@ def run_ours(args):
             extra["roofline_dense_full"]["spin_updates_per_s"] = n * R / (full_ms * 1e-3)
     else:
         roofline = tensor_roofline(step_ms)
-    prof = ROOT / "profiles" / "roofline_traffic.csv"              # dram bytes per launch from the committed ncu captures
+    prof = ROOT / "profiles" / "roofline_traffic.csv"      # dram bytes per launch from the committed ncu captures (kernel, config)
     if prof.exists():
-        try:
-            for line in prof.read_text().splitlines()[1:]:
-                k, v = line.split(",")[:2]
-                if roofline["kernel"].startswith(k) and ((" (tile_skip)" in roofline["kernel"]) == ("tile_skip" in line)):
-                    roofline["traffic"] = float(v)
-        except Exception:
-            pass
+        for line in prof.read_text().splitlines()[1:]:
+            f = line.split(",")
+            if len(f) >= 3 and f[1] == str(args.config):
+                for rl in [roofline] + [v for k, v in extra.items() if k.startswith("roofline")]:
+                    if rl["kernel"] == f[0]:
+                        rl["traffic"] = float(f[2])
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if blocks else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -399,7 +440,7 @@ def run_ours(args):
            "region_ms": ms, "edges_replicas_per_s": edges * R * T * (1 if blocks else world) / (ms * 1e-3), "undirected_edges": edges,
            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
            "gpu_launches": int(launches), "bsb_step_launches_per_solve": int(step_launches),
-           "clocks": clocks, "roofline": roofline, "library": B.qhap_version()}
+           "clocks": clocks, "roofline": roofline, "phases": phases, "library": B.qhap_version()}
     out.update(extra)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O

@@ -207,8 +207,8 @@ def run_ours(args):
     seed = parallel.rank_seed(p["seed"], rank)
     if snp:
         assert args.path in ("auto", "sparse", "block"), "the SNP graphs (configs 3, 4) have no dense J"
-        # auto: banded SNP graphs (config 3's blocks) -> tcgen05 step on the block-compressed J; long-range Pore-C graph -> CSR
-        path = {"auto": 4 if "porec_edges" not in p else 2, "sparse": 2, "block": 4}[args.path]
+        # auto: tcgen05 step on the block-compressed J (config 4: tiles for the banded part + remainder CSR for the long-range edges)
+        path = {"auto": 4, "sparse": 2, "block": 4}[args.path]
         tile_skip = 0
     else:
         path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1, "block": 4}[args.path]
@@ -408,9 +408,22 @@ def run_ours(args):
         # least once (4 B) per spin-update + the non-zero 64 x 64 fp16 blocks of J once
         hg = g.to_host()                              # bookkeeping for the byte count only
         rows = np.repeat(np.arange(g.n, dtype=np.int64), np.diff(hg["row_ptr"]))
-        nz_blocks = int(np.unique((rows // 64) * (1 << 32) + hg["col"].astype(np.int64) // 64).size)
+        tile_id = (rows // 64) * (1 << 32) + hg["col"].astype(np.int64) // 64
+        tiles, inv, cnt = np.unique(tile_id, return_inverse=True, return_counts=True)
         j_terms = 2 if (path == 4 and snp) else 1     # fp32 SNP weights are stored as J_hi + J_lo
-        alg_bytes = 24.0 * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms
+        thr = 1
+        if path == 4:                                 # the library's rule: keep all tiles if they fit the
+            cap = 16 * g.nnz // 4096 + (g.n + 63) // 64 + 1      # capacity, else only tiles with >= 16, 64, ... entries
+            while int((cnt >= thr).sum()) > cap:
+                thr = 16 if thr == 1 else thr * 4
+        nz_blocks = int((cnt >= thr).sum())
+        rem = cnt[inv] < thr                          # entries that go through the remainder CSR gather
+        rem_rows = int(np.unique(rows[rem]).size)
+        # 16 B fp32 state + 4 B fp16 copies written + 4 B read at least once per spin-update, the kept tiles once, and for
+        # the remainder: (col, val) once, one x row gathered per entry, y read-modify-written for the rows that have one
+        alg_bytes = 24.0 * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms + int(rem.sum()) * (8.0 + 4.0 * R) + rem_rows * 8.0 * R
+        extra["remainder_nnz"] = int(rem.sum())
+        extra["tile_threshold"] = thr
         roofline = {"kernel": "dense_step_kernel (tile_skip)" if path == 1 else "dense_step_kernel (block-compressed J)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9,
                     "peak": peaks["hbm"], "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms,
                     "peak_source": peaks["which"], "nonzero_64x64_blocks_of_J": nz_blocks}

@@ -111,8 +111,9 @@ typedef struct {
   int32_t weight_mode;  /* QHAP_WEIGHT_*: which CSR arrays define w (J = -w)                              */
   int32_t path;         /* 0 auto, 1 dense tcgen05 GEMM (needs dense_J), 2 sparse CSR, 3 shared-memory resident */
                         /* (small problems, n R <= 65536: all steps in one launch; same bits as path 2),    */
-                        /* 4 tcgen05 step on a block-compressed J built from the CSR (banded graphs, batches */
-                        /* allowed; synchronises the stream once; QHAP_ERR_RANGE if the graph is not banded) */
+                        /* 4 tcgen05 step on a block-compressed J built from the CSR (64 x 64 tiles; entries  */
+                        /* of sparsely filled tiles -- long-range edges -- go through a remainder CSR gather; */
+                        /* batches allowed; the plan synchronises the stream once or a few times)            */
   int32_t tile_skip;    /* dense path: 1 = skip all-zero 64-column blocks of J (bit-identical result)     */
   int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
   int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */

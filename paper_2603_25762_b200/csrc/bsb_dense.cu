@@ -434,7 +434,8 @@ __global__ void __launch_bounds__(256) absmax_kernel(int64_t nnz, const float* _
 // they are); c1row[i] = c1[instance of i] 2^-15 / scale[0]  (exact power-of-two factors)
 __global__ void __launch_bounds__(256) block_scale_kernel(int32_t n, int32_t n_inst, const int32_t* __restrict__ inst_ptr,
                                                           const float* __restrict__ c1, const uint32_t* __restrict__ amax,
-                                                          int32_t unit, float* __restrict__ scale, float* __restrict__ c1row) {
+                                                          int32_t unit, float* __restrict__ scale, float* __restrict__ c1row,
+                                                          float* __restrict__ c1plain) {
   const float mx = __uint_as_float(*amax);
   const float sc = (unit || !(mx > 0.f)) ? 1.0f : ldexpf(1.0f, 13 - ilogbf(mx));
   const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -450,6 +451,127 @@ __global__ void __launch_bounds__(256) block_scale_kernel(int32_t n, int32_t n_i
     inst = lo;
   }
   c1row[i] = c1[inst] * (1.0f / kXScale) * (1.0f / sc);
+  c1plain[i] = c1[inst];
+}
+
+// Tile occupancy: cnt[tn][kb] = number of entries of tile (tn, kb)  (one warp per row; integer atomics).
+__global__ void __launch_bounds__(256) tile_count_kernel(int32_t n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
+                                                         int32_t n_kblocks, int32_t* __restrict__ cnt) {
+  const int32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n) return;
+  const int lane = threadIdx.x & 31;
+  int32_t* f = cnt + size_t(a / kBK) * n_kblocks;
+  for (int32_t e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) atomicAdd(f + col[e] / kBK, 1);
+}
+
+// One CTA per tile row: ascending list of the k-blocks with at least `thr` entries (at least one list entry per tile row).
+__global__ void __launch_bounds__(32) tile_list_kernel(int32_t n_kblocks, const int32_t* __restrict__ cnt, int32_t thr,
+                                                       int32_t* __restrict__ kb_cnt, int32_t* __restrict__ kb_idx) {
+  const int tn = blockIdx.x, lane = threadIdx.x;
+  const int32_t* f = cnt + size_t(tn) * n_kblocks;
+  int32_t* out = kb_idx + size_t(tn) * n_kblocks;
+  int32_t c = 0;
+  for (int32_t base = 0; base < n_kblocks; base += 32) {
+    const int32_t kb = base + lane;
+    const bool on = kb < n_kblocks && f[kb] >= thr;
+    const uint32_t m = __ballot_sync(0xffffffffu, on);
+    if (on) out[c + __popc(m & ((1u << lane) - 1u))] = kb;
+    c += __popc(m);
+  }
+  if (lane == 0) {
+    if (c == 0) { out[0] = tn < n_kblocks ? tn : 0; c = 1; }   // the diagonal tile (possibly empty) keeps the pipeline uniform
+    kb_cnt[tn] = c;
+  }
+}
+
+__device__ __forceinline__ bool tile_listed(const int32_t* list, int32_t cnt, int32_t kb, int& pos) {
+  int lo = 0, hi = cnt;                                    // list[lo] <= kb < list[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (list[mid] <= kb) lo = mid; else hi = mid;
+  }
+  pos = lo;
+  return list[lo] == kb;
+}
+
+// Remainder = entries whose tile is not listed (sparse long-range edges).  Pass 0 counts them per row, pass 1 writes
+// them (ascending column order is kept: ballot compaction over 32 entries at a time).
+template <int FILL>
+__global__ void __launch_bounds__(256) remainder_kernel(int32_t n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
+                                                        const float* __restrict__ jval, int32_t n_kblocks,
+                                                        const int32_t* __restrict__ kb_cnt, const int32_t* __restrict__ kb_idx,
+                                                        int32_t* __restrict__ rem_ptr, int32_t* __restrict__ rem_col,
+                                                        float* __restrict__ rem_val) {
+  const int32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n) return;
+  const int lane = threadIdx.x & 31;
+  const int32_t tn = a / kBK;
+  const int32_t* list = kb_idx + size_t(tn) * n_kblocks;
+  const int32_t cnt = kb_cnt[tn];
+  int32_t outp = FILL ? rem_ptr[a] : 0;
+  for (int32_t e0 = row_ptr[a]; e0 < row_ptr[a + 1]; e0 += 32) {
+    const int32_t e = e0 + lane;
+    bool rem = false;
+    int pos;
+    if (e < row_ptr[a + 1]) rem = !tile_listed(list, cnt, col[e] / kBK, pos);
+    const uint32_t m = __ballot_sync(0xffffffffu, rem);
+    if (FILL && rem) {
+      const int32_t o = outp + __popc(m & ((1u << lane) - 1u));
+      rem_col[o] = col[e];
+      rem_val[o] = jval[e];
+    }
+    outp += __popc(m);
+  }
+  if (!FILL && lane == 0) rem_ptr[a] = outp;
+}
+
+// y += c1[instance] * sum over the row's remainder entries of J x_old  -- one warp per row, lanes across replicas
+// (float4), rows without remainder entries cost one row_ptr read.  Runs BEFORE the tile step of the same bSB step, on the
+// fp32 x that step will then update in place; the tile step's fma(c1, F_tiles, fma(-c2, x, y)) completes the sum.
+__global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t R, const int32_t* __restrict__ rem_ptr,
+                                                             const int32_t* __restrict__ rem_col, const float* __restrict__ rem_val,
+                                                             const float* __restrict__ c1row_plain, const float* __restrict__ x,
+                                                             float* __restrict__ y) {
+  const int32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n) return;
+  const int32_t e0 = rem_ptr[a], e1 = rem_ptr[a + 1];
+  if (e0 == e1) return;
+  const int lane = threadIdx.x & 31;
+  const float c1 = c1row_plain[a];
+  for (int32_t r = lane * 4; r < R; r += 128) {
+    if (r + 4 <= R && (R & 3) == 0) {
+      float4 F = make_float4(0.f, 0.f, 0.f, 0.f);
+      int32_t e = e0;
+      for (; e + 4 <= e1; e += 4) {                      // four independent gathers in flight, summed in ascending order
+        float v[4];
+        float4 xv[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          v[q] = __ldg(rem_val + e + q);
+          xv[q] = *reinterpret_cast<const float4*>(x + size_t(__ldg(rem_col + e + q)) * R + r);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          F.x = fmaf(v[q], xv[q].x, F.x); F.y = fmaf(v[q], xv[q].y, F.y); F.z = fmaf(v[q], xv[q].z, F.z); F.w = fmaf(v[q], xv[q].w, F.w);
+        }
+      }
+      for (; e < e1; ++e) {
+        const float v = __ldg(rem_val + e);
+        const float4 xv = *reinterpret_cast<const float4*>(x + size_t(__ldg(rem_col + e)) * R + r);
+        F.x = fmaf(v, xv.x, F.x); F.y = fmaf(v, xv.y, F.y); F.z = fmaf(v, xv.z, F.z); F.w = fmaf(v, xv.w, F.w);
+      }
+      float4* py = reinterpret_cast<float4*>(y + size_t(a) * R + r);
+      float4 yv = *py;
+      yv.x = fmaf(c1, F.x, yv.x); yv.y = fmaf(c1, F.y, yv.y); yv.z = fmaf(c1, F.z, yv.z); yv.w = fmaf(c1, F.w, yv.w);
+      *py = yv;
+    } else {
+      for (int32_t rr = r; rr < min(r + 4, R); ++rr) {
+        float F = 0.f;
+        for (int32_t e = e0; e < e1; ++e) F = fmaf(__ldg(rem_val + e), x[size_t(__ldg(rem_col + e)) * R + rr], F);
+        y[size_t(a) * R + rr] = fmaf(c1, F, y[size_t(a) * R + rr]);
+      }
+    }
+  }
 }
 
 // One warp per row: scatter the row's entries into their tiles.  Tile (tn, kb) is block blk_ptr[tn] + (rank of kb in the
@@ -468,11 +590,8 @@ __global__ void __launch_bounds__(256) block_fill_kernel(int32_t n, const int32_
   const float sc = scale[0];
   for (int32_t e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
     const int32_t c = col[e], kb = c / kBK;
-    int lo = 0, hi = cnt;                                  // list[lo] <= kb < list[hi]
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (list[mid] <= kb) lo = mid; else hi = mid;
-    }
+    int lo;
+    if (!tile_listed(list, cnt, kb, lo)) continue;         // remainder entry (handled by remainder_step_kernel)
     const size_t idx = (size_t(base + lo) * kBK + size_t(a % kBK)) * kBK + size_t(c % kBK);
     const float vs = jval[e] * sc;
     const __half h = __float2half_rn(vs);
@@ -673,6 +792,10 @@ size_t block_workspace_bytes(int32_t n, int64_t nnz, int32_t R) {
   ws.take<int32_t>(n_t * n_t);            // kb_idx
   ws.take<int32_t>(n_t * n_t);            // flags
   ws.take<float>(size_t(n));              // c1row
+  ws.take<float>(size_t(n));              // c1plain
+  ws.take<int32_t>(size_t(n) + 1);        // rem_ptr
+  ws.take<int32_t>(size_t(nnz));          // rem_col
+  ws.take<float>(size_t(nnz));            // rem_val
   ws.take<uint32_t>(4);                   // absmax, scale
   ws.take<int64_t>(2);                    // total blocks, overflow
   const size_t cap = size_t(block_capacity(n, nnz)) * kBK * kBK;
@@ -699,6 +822,10 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   int32_t* kb_idx = ws.take<int32_t>(size_t(n_t) * n_t);
   int32_t* flags = ws.take<int32_t>(size_t(n_t) * n_t);
   float* c1row = ws.take<float>(size_t(n));
+  float* c1plain = ws.take<float>(size_t(n));
+  int32_t* rem_ptr = ws.take<int32_t>(size_t(n) + 1);
+  int32_t* rem_col = ws.take<int32_t>(size_t(g.nnz));
+  float* rem_val = ws.take<float>(size_t(g.nnz));
   uint32_t* scal = ws.take<uint32_t>(4);
   int64_t* totals = ws.take<int64_t>(2);
   const int64_t cap_blocks = block_capacity(n, g.nnz);
@@ -707,27 +834,41 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   __half* jl = ws.take<__half>(cap);
   const bool two_terms = weight_mode == QHAP_WEIGHT_FX;      // integer counts are exact in fp16 (|J| <= 2048 checked below)
 
-  // tile lists (the same kernels as tile_skip at BN = 64), block offsets, capacity check (one host synchronisation)
+  // tile occupancy -> tile lists -> block offsets.  All tiles are kept if they fit the capacity (banded graphs); otherwise
+  // only tiles with at least thr = 16, 64, ... entries are kept and the rest of the entries (long-range edges) become a
+  // remainder CSR that a small gather kernel adds into y before each tile step.  One host synchronisation per attempt.
   QHAP_CUDA_TRY(cudaMemsetAsync(flags, 0, sizeof(int32_t) * size_t(n_t) * n_t, stream));
   QHAP_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(uint32_t) * 4, stream));
-  kb_flag_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, kBK, n_t, flags);
+  tile_count_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, n_t, flags);
   QHAP_LAUNCH_CHECK();
-  kb_list_kernel<<<n_t, 32, 0, stream>>>(n_t, flags, kb_cnt, kb_idx);
-  QHAP_LAUNCH_CHECK();
-  QHAP_TRY(exclusive_scan_i32(kb_cnt, blk_ptr, n_t, totals, reinterpret_cast<int32_t*>(totals + 1), stream));
   if (g.nnz > 0) {
     absmax_kernel<<<int(std::min<int64_t>(ceil_div(g.nnz, 256), int64_t(sm_count()) * 8)), 256, 0, stream>>>(g.nnz, jval, scal);
     QHAP_LAUNCH_CHECK();
   }
   int64_t total_blocks = 0;
   uint32_t amax_bits = 0;
-  QHAP_CUDA_TRY(cudaMemcpyAsync(&total_blocks, totals, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
-  QHAP_CUDA_TRY(cudaMemcpyAsync(&amax_bits, scal, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
-  QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
-  if (total_blocks > cap_blocks) {
-    set_error("block path: %lld non-empty 64 x 64 tiles exceed the capacity %lld (16 x nnz / 4096 + n / 64): the graph is not "
-              "banded enough (long-range edges) -- use the CSR path (path = 2)", (long long)total_blocks, (long long)cap_blocks);
-    return QHAP_ERR_RANGE;
+  int32_t thr = 1;
+  for (;; thr = (thr == 1 ? 16 : thr * 4)) {
+    tile_list_kernel<<<n_t, 32, 0, stream>>>(n_t, flags, thr, kb_cnt, kb_idx);
+    QHAP_LAUNCH_CHECK();
+    QHAP_TRY(exclusive_scan_i32(kb_cnt, blk_ptr, n_t, totals, reinterpret_cast<int32_t*>(totals + 1), stream));
+    QHAP_CUDA_TRY(cudaMemcpyAsync(&total_blocks, totals, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
+    QHAP_CUDA_TRY(cudaMemcpyAsync(&amax_bits, scal, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+    QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
+    if (total_blocks <= cap_blocks) break;
+    if (thr > kBK * kBK) {
+      set_error("block path: %lld tiles exceed the capacity %lld", (long long)total_blocks, (long long)cap_blocks);
+      return QHAP_ERR_RANGE;
+    }
+  }
+  const bool has_rem = thr > 1;
+  if (has_rem) {
+    const int rb = int(ceil_div(int64_t(n) * 32, 256));
+    remainder_kernel<0><<<rb, 256, 0, stream>>>(n, g.row_ptr, g.col, jval, n_t, kb_cnt, kb_idx, rem_ptr, rem_col, rem_val);
+    QHAP_LAUNCH_CHECK();
+    QHAP_TRY(exclusive_scan_i32(rem_ptr, rem_ptr, n, totals, reinterpret_cast<int32_t*>(totals + 1), stream));
+    remainder_kernel<1><<<rb, 256, 0, stream>>>(n, g.row_ptr, g.col, jval, n_t, kb_cnt, kb_idx, rem_ptr, rem_col, rem_val);
+    QHAP_LAUNCH_CHECK();
   }
   float amax;
   memcpy(&amax, &amax_bits, sizeof(float));
@@ -737,7 +878,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   }
   float* scale = reinterpret_cast<float*>(scal + 1);
   block_scale_kernel<<<int(ceil_div(std::max(n, 1), 256)), 256, 0, stream>>>(n, n_inst, inst_ptr_dev, c1_dev, scal, two_terms ? 0 : 1,
-                                                                            scale, c1row);
+                                                                            scale, c1row, c1plain);
   QHAP_LAUNCH_CHECK();
   QHAP_CUDA_TRY(cudaMemsetAsync(jh, 0, sizeof(__half) * size_t(total_blocks) * kBK * kBK, stream));
   if (two_terms) QHAP_CUDA_TRY(cudaMemsetAsync(jl, 0, sizeof(__half) * size_t(total_blocks) * kBK * kBK, stream));
@@ -779,6 +920,10 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
     a.c3 = float(p.dt * p.a0);
     a.xh_out = xh[cur ^ 1];
     a.xl_out = xl[cur ^ 1];
+    if (has_rem) {
+      remainder_step_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, R, rem_ptr, rem_col, rem_val, c1plain, x, y);
+      QHAP_LAUNCH_CHECK();
+    }
     QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a));
     cur ^= 1;
   }

@@ -424,6 +424,10 @@ def run_ours(args):
         alg_bytes = 24.0 * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms + int(rem.sum()) * (8.0 + 4.0 * R) + rem_rows * 8.0 * R
         extra["remainder_nnz"] = int(rem.sum())
         extra["tile_threshold"] = thr
+        if int(rem.sum()) > 0:
+            extra["roofline_note"] = ("the remainder gathers (4 B x R per far non-zero, SURVEY 8(d)) are counted as algorithmic HBM bytes, but "
+                                      "x (%.0f MB) largely stays in the 126 MB L2, so most of them are L2 hits: frac can exceed 1; "
+                                      "state + tiles alone = %.0f MB per launch" % (4e-6 * g.n * R, (24.0 * g.n * R + nz_blocks * 8192.0 * j_terms) / 1e6))
         roofline = {"kernel": "dense_step_kernel (tile_skip)" if path == 1 else "dense_step_kernel (block-compressed J)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9,
                     "peak": peaks["hbm"], "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms,
                     "peak_source": peaks["which"], "nonzero_64x64_blocks_of_J": nz_blocks}

@@ -220,3 +220,50 @@ def solve(row_ptr, col, w_int, jval, x0, y0, *, steps_total, dt=1.25, a0=1.0, c0
     r = best_replica(cut)
     return dict(x=x, y=y, c0=c0, spins=s, cut=cut, energy=en, best_replica=r, best_cut=int(cut[r]),
                 best_spins=s[:, r].copy())
+
+
+# ---------------------------------------------------------------------------------------------- O6
+# SNP-based iterative refinement, PAPER.md:L325-L338 [Eq. 15-17].  Plain numpy, in the paper's
+# order.  Readings (R16): the termination test (cut <= 0, or one side empty) is made right after the solve and
+# BEFORE the counter / weight update of that iteration; the smaller subset on a tie is the -1 side; every iteration
+# starts bSB from a fresh seeded state handed in by the caller (the oracle draws no numbers).
+def gauge_transform(row_ptr, col, w_fx, w, spins):
+    """Eq. 15: w'_uv = -w_uv if s_u != s_v else w_uv, on the fixed-point and the fp32 weights alike (exact sign flips)."""
+    rp, cl = _c(row_ptr, np.int32), _c(col, np.int32)
+    s = _c(spins, np.int8).astype(np.int64)
+    rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
+    sg = s[rows] * s[cl]
+    return (np.asarray(w_fx, np.int64) * sg).astype(np.int64), (np.asarray(w, np.float32) * sg.astype(np.float32)).astype(np.float32)
+
+
+def smaller_subset(spins) -> np.ndarray:
+    """Boolean mask of S_min (Eq. 16): the side with fewer vertices; the -1 side on a tie."""
+    s = _c(spins, np.int8)
+    n_pos, n_neg = int((s > 0).sum()), int((s < 0).sum())
+    return (s > 0) if n_pos < n_neg else (s < 0)
+
+
+def refine_snp(row_ptr, col, w_fx, w, init_states, *, steps_total, max_iter, dt=1.25, a0=1.0, n_threads=1):
+    """Iterative refinement.  init_states(t) -> (x0, y0) fp32 [n][R] for iteration t = 0, 1, ...
+    Returns dict(flip_count [n] int32, iterations (solves run), cuts (best cut of every solve), w_fx, w (final weights))."""
+    rp, cl = _c(row_ptr, np.int32), _c(col, np.int32)
+    wfx, wf = np.asarray(w_fx, np.int64).copy(), np.asarray(w, np.float32).copy()
+    n = len(rp) - 1
+    count = np.zeros(n, np.int32)
+    cuts = []
+    for t in range(max_iter):
+        x0, y0 = init_states(t)
+        res = solve(rp, cl, wfx, (-wf).astype(np.float32), x0, y0, steps_total=steps_total, dt=dt, a0=a0, n_threads=n_threads)
+        s = res["best_spins"]
+        cuts.append(int(res["best_cut"]))
+        if res["best_cut"] <= 0 or abs(int(s.astype(np.int64).sum())) == n:      # L333: non-positive cut or a single subset
+            break
+        count[smaller_subset(s)] += 1                                          # Eq. 16
+        wfx, wf = gauge_transform(rp, cl, wfx, wf, s)                          # Eq. 15
+    return dict(flip_count=count, iterations=len(cuts), cuts=cuts, w_fx=wfx, w=wf)
+
+
+def refine_readout(h1, flip_count) -> np.ndarray:
+    """Eq. 17: H1'[u] = H1[u] if C(p_u) is even else H2[u] = 1 - H1[u]."""
+    h = np.zeros(len(flip_count), np.uint8) if h1 is None else _c(h1, np.uint8)
+    return np.where(np.asarray(flip_count) % 2 == 0, h, 1 - h).astype(np.int8)

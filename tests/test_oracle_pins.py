@@ -453,3 +453,36 @@ def test_init_state_is_uniform_and_fp32(oracle):
     assert not np.array_equal(x, y) and not np.array_equal(x[:, 0], x[:, 1])
     x2, _ = synth.bsb_init_state(124, 500, 64)
     assert not np.array_equal(x, x2)
+
+
+# ------------------------------------------------------------------------------------ O6 iterative refinement (f1)
+def test_refine_gauge_identity_and_planted_recovery(oracle):
+    """Eq. 15 is a gauge transform: E_{w'}(t) = E_w(s o t) for every t (exact, int64), so E_{w'}(all +1) = E_w(s).
+    Error-free reads: the first solve is optimal, the transformed graph's best cut is <= 0 -> the loop stops after two
+    solves with C = indicator of the smaller side, and Eq. 17 returns the planted haplotype (SE = HE = 0)."""
+    fr = synth.make_fragments(seed=11, L=60_000, n_snp=80, n_reads=60, len_law=("uniform", 6_000, 15_000), flip=0.0,
+                              missing=0.0, qual=("const", 30))
+    g = oracle.snp_graph(fr, 10, 0.1)
+    rng = np.random.default_rng(0)
+    s = rng.choice(np.array([-1, 1], np.int8), size=g["n"])
+    wfx2, w2 = oracle.gauge_transform(g["row_ptr"], g["col"], g["w_fx"], g["w"], s)
+    assert np.array_equal(np.abs(wfx2), np.abs(g["w_fx"])) and np.array_equal(np.abs(w2), np.abs(g["w"]))
+    for _ in range(5):
+        t = rng.choice(np.array([-1, 1], np.int8), size=g["n"])
+        _, e2 = oracle.cut_eval(g["row_ptr"], g["col"], wfx2, t)
+        _, e1 = oracle.cut_eval(g["row_ptr"], g["col"], g["w_fx"], (s * t).astype(np.int8))
+        assert e1[0] == e2[0]
+    ones = np.ones(g["n"], np.int8)
+    assert np.array_equal(oracle.gauge_transform(g["row_ptr"], g["col"], g["w_fx"], g["w"], ones)[0], g["w_fx"])
+    m = oracle.smaller_subset(np.array([1, -1, -1, 1, 1], np.int8))
+    assert m.tolist() == [False, True, True, False, False]
+    assert oracle.smaller_subset(np.array([1, -1], np.int8)).tolist() == [False, True]          # tie -> the -1 side
+    R, T = 16, 300
+    res = oracle.refine_snp(g["row_ptr"], g["col"], g["w_fx"], g["w"], lambda t: synth.bsb_init_state(100 + t, g["n"], R),
+                            steps_total=T, max_iter=6, n_threads=4)
+    assert res["iterations"] == 2 and res["cuts"][0] > 0 and res["cuts"][1] <= 0, res["cuts"]
+    hap = oracle.refine_readout(fr.h1, res["flip_count"])
+    covered = np.bincount(fr.snp_idx[fr.allele <= 1], minlength=fr.n_snp) > 0
+    mm = oracle.switch_hamming(hap[covered], fr.hap_a[covered])
+    assert mm["se"] == 0.0 and mm["he"] == 0.0
+    assert set(np.unique(res["flip_count"])) <= {0, 1}

@@ -156,6 +156,23 @@ QHAP_API qhap_status qhap_block_split(const qhap_csr *graph, int32_t n_blocks, c
 QHAP_API qhap_status qhap_block_stitch(int32_t n, int32_t n_blocks, const int64_t *win /*HOST*/, const int8_t *block_spins,
                               int8_t *out, void *workspace, size_t *ws_bytes, void *stream);
 
+/* (f1) SNP-based iterative refinement, PAPER.md:L325-L338 [Eq. 15-17]; readings in DESIGN.md R16.
+ * qhap_gauge_transform: Eq. 15, w'_uv = -w_uv where spins[u] != spins[v] (w_fx and/or w, in place; exact sign flips).
+ * qhap_flip_count_update: Eq. 16, flip_count[u] += 1 for u in the smaller subset of `spins` (the -1 side on a tie).
+ * qhap_refine_readout: Eq. 17, hap1[u] = h1[u] if flip_count[u] is even else 1 - h1[u].
+ * qhap_snp_refine: the loop -- solve (seed + t, seeded start state, path/replicas/steps from `params`), stop if the best
+ *   cut is <= 0 or one side is empty, else Eq. 16 and Eq. 15 -- at most max_iter solves on ONE instance; the graph's
+ *   weights are updated in place; flip_count [n] is zeroed first; `iterations` and `cuts` [max_iter] are HOST outputs
+ *   (the call synchronises the stream once per iteration). */
+QHAP_API qhap_status qhap_gauge_transform(const qhap_csr *graph, const int8_t *spins /*[n]*/, void *stream);
+QHAP_API qhap_status qhap_flip_count_update(int32_t n, const int8_t *spins, int32_t *flip_count, void *workspace, size_t *ws_bytes,
+                                   void *stream);
+QHAP_API qhap_status qhap_refine_readout(int32_t n, const uint8_t *h1 /*may be NULL*/, const int32_t *flip_count, int8_t *hap1,
+                                void *stream);
+QHAP_API qhap_status qhap_snp_refine(qhap_csr *graph, const qhap_bsb_params *params, int32_t max_iter, float *x, float *y,
+                            int32_t *flip_count, int32_t *iterations /*HOST*/, int64_t *cuts /*HOST [max_iter]*/, void *workspace,
+                            size_t *ws_bytes, void *stream);
+
 QHAP_API const char *qhap_last_error(void);
 /* Number of CUDA kernels this library has launched in this process so far (monotonic; bench.py reports the difference
  * over its timed region as "gpu_launches"). */

@@ -25,6 +25,7 @@ QHAP_DENSE_NONE, QHAP_DENSE_FP16, QHAP_DENSE_BF16 = 0, 1, 2
 
 EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_bsb_solve", "qhap_cut_eval",
            "qhap_phase_readout_reads", "qhap_phase_readout_snps", "qhap_block_split", "qhap_block_stitch",
+           "qhap_gauge_transform", "qhap_flip_count_update", "qhap_refine_readout", "qhap_snp_refine",
            "qhap_last_error", "qhap_launch_count", "qhap_version"]
 
 
@@ -46,7 +47,7 @@ class _BsbParams(C.Structure):
                 ("finalize", C.c_int32), ("dense_bn", C.c_int32)]
 
 
-for _name in EXPORTS[:8]:
+for _name in EXPORTS[:12]:
     getattr(_lib, _name).restype = C.c_int
 _lib.qhap_last_error.restype = C.c_char_p
 _lib.qhap_version.restype = C.c_char_p
@@ -372,3 +373,56 @@ def qhap_block_stitch(n: int, windows: np.ndarray, block_spins: torch.Tensor) ->
     ws_bytes = C.c_size_t(ws.numel())
     _check(call(_ptr(ws), C.byref(ws_bytes)), "qhap_block_stitch")
     return out[:n]
+
+
+# ------------------------------------------------------------------ (f1) SNP-based iterative refinement, Eq. 15-17
+def qhap_gauge_transform(graph: Csr, spins: torch.Tensor) -> None:
+    """Eq. 15 in place on graph.w_fx / graph.w."""
+    gs = graph.c_struct()
+    _check(_lib.qhap_gauge_transform(C.byref(gs), _ptr(spins), _stream()), "qhap_gauge_transform")
+
+
+def qhap_flip_count_update(spins: torch.Tensor, flip_count: torch.Tensor) -> None:
+    """Eq. 16: flip_count += 1 on the smaller subset of spins."""
+    n = spins.numel()
+
+    def call(ws, ws_bytes):
+        return _lib.qhap_flip_count_update(C.c_int32(n), _ptr(spins), _ptr(flip_count), ws, ws_bytes, _stream())
+    ws_bytes = C.c_size_t(0)
+    _check(call(None, C.byref(ws_bytes)), "qhap_flip_count_update (size query)")
+    ws = _workspace(ws_bytes.value)
+    ws_bytes = C.c_size_t(ws.numel())
+    _check(call(_ptr(ws), C.byref(ws_bytes)), "qhap_flip_count_update")
+
+
+def qhap_refine_readout(h1: Optional[torch.Tensor], flip_count: torch.Tensor) -> torch.Tensor:
+    """Eq. 17 -> hap1 [n] int8."""
+    n = flip_count.numel()
+    hap = torch.empty(max(n, 1), dtype=torch.int8, device=_dev())
+    _check(_lib.qhap_refine_readout(C.c_int32(n), _ptr(h1), _ptr(flip_count), _ptr(hap), _stream()), "qhap_refine_readout")
+    return hap[:n]
+
+
+def qhap_snp_refine(graph: Csr, *, replicas: int, steps_total: int, max_iter: int, dt: float = 1.25, a0: float = 1.0,
+                    c0: float = 0.0, seed: int = 0, path: int = 0, workspace: Optional[torch.Tensor] = None) -> dict:
+    """The refinement loop on one instance; graph.w_fx / graph.w are updated in place."""
+    dev = _dev()
+    n, R = graph.n, int(replicas)
+    x = torch.empty((n, R), dtype=torch.float32, device=dev)
+    y = torch.empty((n, R), dtype=torch.float32, device=dev)
+    flip = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    p = _BsbParams(R, steps_total, 0, steps_total, dt, a0, c0, seed, QHAP_WEIGHT_FX, path, 0, 1, 1, 0)
+    gs = graph.c_struct()
+    iters = C.c_int32(0)
+    cuts = (C.c_int64 * max_iter)()
+
+    def call(ws, ws_bytes):
+        return _lib.qhap_snp_refine(C.byref(gs), C.byref(p), C.c_int32(max_iter), _ptr(x), _ptr(y), _ptr(flip), C.byref(iters), cuts,
+                                    ws, ws_bytes, _stream())
+    ws_bytes = C.c_size_t(0)
+    _check(call(None, C.byref(ws_bytes)), "qhap_snp_refine (size query)")
+    if workspace is None or workspace.numel() < ws_bytes.value:
+        workspace = _workspace(ws_bytes.value)
+    ws_bytes = C.c_size_t(workspace.numel())
+    _check(call(_ptr(workspace), C.byref(ws_bytes)), "qhap_snp_refine")
+    return dict(flip_count=flip[:n], iterations=int(iters.value), cuts=[int(c) for c in cuts[:iters.value]], workspace=workspace)

@@ -602,3 +602,62 @@ def test_cfg1_full_size_sampled(B, oracle, torch_mod):
     ose, ohe = ser_reads(oracle, fr, ores["best_spins"])
     print(f"cfg1 full size: gpu best cut {gcut} (replica {r}), oracle(64 replicas) {ores['best_cut']}; SE gpu {gse:.5f} oracle {ose:.5f}")
     assert gse <= ose + 0.001
+
+
+# ------------------------------------------------------------------- (f1) SNP-based iterative refinement, Eq. 15-17
+def test_refine_pieces_bit_exact(B, oracle, torch_mod):
+    """Eq. 15 (gauge transform of w_fx and w), Eq. 16 (flip counter on the smaller subset, ties included) and Eq. 17
+    (readout by parity) against the oracle on the same spins: integer work and exact sign flips -> bit-exact."""
+    fr, p = synth.make_config(3, scale=0.005)
+    g = oracle.snp_graph(fr, 3, 0.1)
+    rng = np.random.default_rng(5)
+    flip_o = np.zeros(g["n"], np.int32)
+    flip_g = torch_mod.zeros(g["n"], dtype=torch_mod.int32, device="cuda")
+    dg = B.upload_csr(g)
+    wfx, wf = g["w_fx"].copy(), g["w"].copy()
+    for it in range(4):
+        s = rng.choice(np.array([-1, 1], np.int8), size=g["n"], p=[0.5, 0.5] if it != 2 else [0.3, 0.7])
+        if it == 3:                                   # an exact tie: the -1 side is the smaller subset
+            s = np.where(np.arange(g["n"]) % 2 == 0, 1, -1).astype(np.int8)[: g["n"]]
+            if g["n"] % 2:
+                s[-1] = -1 if (s > 0).sum() > (s < 0).sum() else 1
+        sg = torch_mod.from_numpy(s).cuda()
+        wfx, wf = oracle.gauge_transform(g["row_ptr"], g["col"], wfx, wf, s)
+        flip_o[oracle.smaller_subset(s)] += 1
+        B.qhap_gauge_transform(dg, sg)
+        B.qhap_flip_count_update(sg, flip_g)
+        assert np.array_equal(dg.w_fx.cpu().numpy(), wfx) and np.array_equal(dg.w.cpu().numpy(), wf)
+        assert np.array_equal(flip_g.cpu().numpy(), flip_o)
+    h1 = rng.integers(0, 2, size=g["n"]).astype(np.uint8)
+    hap = B.qhap_refine_readout(torch_mod.from_numpy(h1).cuda(), flip_g).cpu().numpy()
+    assert np.array_equal(hap, oracle.refine_readout(h1, flip_o))
+    assert np.array_equal(B.qhap_refine_readout(None, flip_g).cpu().numpy(), oracle.refine_readout(None, flip_o))
+
+
+def test_refine_loop_against_oracle(B, oracle, torch_mod):
+    """The whole loop (seed + t start states on both sides).  bSB is chaotic, so the iterates may differ; what is compared:
+    on error-free reads both stop after the same two or three solves with the planted haplotype; on noisy reads the GPU's final switch
+    error is <= the oracle's + 0.1 pp, the first cut is within 0.5 %, and the invariants of the loop hold on the GPU
+    (weights keep their magnitudes; the last cut is <= 0 or max_iter was reached)."""
+    for flip_rate, name in ((0.0, "error-free"), (0.05, "noisy")):
+        fr = synth.make_fragments(seed=21, L=400_000, n_snp=500, n_reads=400, len_law=("uniform", 8_000, 25_000), flip=flip_rate,
+                                  missing=0.0, qual=("normal", 18, 5, 3, 40))
+        g = oracle.snp_graph(fr, 10, 0.1)
+        R, T, K = 64, 400, 6
+        ores = oracle.refine_snp(g["row_ptr"], g["col"], g["w_fx"], g["w"], lambda t: synth.bsb_init_state(77 + t, g["n"], R),
+                                 steps_total=T, max_iter=K, n_threads=8)
+        for path in (2, 4):
+            dg = B.upload_csr(g)
+            gres = B.qhap_snp_refine(dg, replicas=R, steps_total=T, max_iter=K, seed=77, path=path)
+            assert np.array_equal(np.abs(dg.w_fx.cpu().numpy()), np.abs(g["w_fx"]))
+            assert gres["iterations"] == K or gres["cuts"][-1] <= 0
+            assert gres["cuts"][0] >= ores["cuts"][0] - 0.005 * abs(ores["cuts"][0])
+            covered = np.bincount(fr.snp_idx[fr.allele <= 1], minlength=fr.n_snp) > 0
+            ghap = B.qhap_refine_readout(None, gres["flip_count"]).cpu().numpy()
+            gm = oracle.switch_hamming(ghap[covered], fr.hap_a[covered])
+            om = oracle.switch_hamming(oracle.refine_readout(None, ores["flip_count"])[covered], fr.hap_a[covered])
+            print(f"refine {name} path {path}: gpu iterations {gres['iterations']} cuts {gres['cuts']} SE {gm['se']:.4f} | "
+                  f"oracle iterations {ores['iterations']} cuts {ores['cuts']} SE {om['se']:.4f}")
+            assert gm["se"] <= om["se"] + 0.001
+            if flip_rate == 0.0:
+                assert gres["iterations"] == ores["iterations"] <= 3 and gm["se"] == 0.0 and gm["he"] == 0.0

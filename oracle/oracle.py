@@ -267,3 +267,45 @@ def refine_readout(h1, flip_count) -> np.ndarray:
     """Eq. 17: H1'[u] = H1[u] if C(p_u) is even else H2[u] = 1 - H1[u]."""
     h = np.zeros(len(flip_count), np.uint8) if h1 is None else _c(h1, np.uint8)
     return np.where(np.asarray(flip_count) % 2 == 0, h, 1 - h).astype(np.int8)
+
+
+# ---------------------------------------------------------------------------------------------- O7
+# Connected components and per-component batching, PAPER.md:L248 ("each connected component ... independently"), L319
+# (SURVEY.md 8(f) f2).  Canonical form (DESIGN.md R14): components are numbered by their smallest vertex, vertices keep
+# their ascending order inside a component, components with fewer than `min_size` vertices are dropped (singletons carry
+# no phase information).  The library step is scipy's connected_components; the rest is index arithmetic.
+def component_split(g: dict, min_size: int = 2) -> dict:
+    """Block-diagonal CSR of the kept components + perm (new index -> old vertex) + inst_ptr."""
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    n = int(g["n"])
+    rp, cl = _c(g["row_ptr"], np.int32), _c(g["col"], np.int32)
+    A = csr_matrix((np.ones(len(cl), np.int8), cl, rp), shape=(n, n))
+    _, lab = connected_components(A, directed=False)
+    first = np.full(lab.max() + 1 if n else 0, n, np.int64)
+    np.minimum.at(first, lab, np.arange(n))
+    root = first[lab]                                   # canonical label = smallest vertex of the component
+    size = np.bincount(root, minlength=n)[root] if n else np.zeros(0, np.int64)
+    keep = size >= min_size
+    order = np.lexsort((np.arange(n), root))            # by component (smallest vertex), then by vertex
+    perm = order[keep[order]].astype(np.int32)
+    inv = np.full(n, -1, np.int64)
+    inv[perm] = np.arange(len(perm))
+    roots_kept = root[perm]
+    starts = np.flatnonzero(np.r_[True, roots_kept[1:] != roots_kept[:-1]]) if len(perm) else np.zeros(0, np.int64)
+    inst_ptr = np.r_[starts, len(perm)].astype(np.int32)
+    deg = (rp[1:] - rp[:-1])[perm]
+    new_rp = np.r_[0, np.cumsum(deg)].astype(np.int32)
+    idx = np.concatenate([np.arange(rp[v], rp[v + 1]) for v in perm]) if len(perm) else np.zeros(0, np.int64)
+    out = dict(n=len(perm), nnz=int(new_rp[-1]), row_ptr=new_rp, col=inv[cl[idx]].astype(np.int32), perm=perm, inst_ptr=inst_ptr)
+    for k in ("d", "c", "w_fx", "w"):
+        if g.get(k) is not None:
+            out[k] = np.asarray(g[k])[idx]
+    return out
+
+
+def component_merge(n: int, perm, comp_spins) -> np.ndarray:
+    """Spins of the kept components back to the original vertices; dropped vertices get 0 (unphased)."""
+    s = np.zeros(n, np.int8)
+    s[np.asarray(perm)] = np.asarray(comp_spins, np.int8)
+    return s

@@ -486,3 +486,49 @@ def test_refine_gauge_identity_and_planted_recovery(oracle):
     mm = oracle.switch_hamming(hap[covered], fr.hap_a[covered])
     assert mm["se"] == 0.0 and mm["he"] == 0.0
     assert set(np.unique(res["flip_count"])) <= {0, 1}
+
+
+# ------------------------------------------------------------------------------- O7 connected components (f2)
+def test_component_split_known_graph_and_bfs(oracle):
+    """A hand-made graph with known components, and random graphs against a plain BFS."""
+    # components: {0, 3, 4}, {1}, {2, 5}, {6, 7, 8} (path), 9 isolated
+    edges = [(0, 3), (3, 4), (2, 5), (6, 7), (7, 8)]
+    n = 10
+    rows = [[] for _ in range(n)]
+    for a, b in edges:
+        rows[a].append(b); rows[b].append(a)
+    rp = np.r_[0, np.cumsum([len(r) for r in rows])].astype(np.int32)
+    cl = np.array([c for r in rows for c in sorted(r)], np.int32)
+    g = dict(n=n, nnz=len(cl), row_ptr=rp, col=cl, w_fx=np.arange(1, len(cl) + 1, dtype=np.int64))
+    cs = oracle.component_split(g, 2)
+    assert cs["perm"].tolist() == [0, 3, 4, 2, 5, 6, 7, 8] and cs["inst_ptr"].tolist() == [0, 3, 5, 8]
+    assert cs["row_ptr"].tolist() == [0, 1, 3, 4, 5, 6, 7, 9, 10]
+    assert cs["col"].tolist() == [1, 0, 2, 1, 4, 3, 6, 5, 7, 6]
+    # weights travel with their entries: entry (0,3) had w 1; (3,0) 4; (3,4) 5 ...
+    assert cs["w_fx"][0] == 1 and cs["w_fx"][1] == g["w_fx"][rp[3]]
+    assert oracle.component_split(g, 1)["inst_ptr"].tolist() == [0, 3, 4, 6, 9, 10]
+    assert oracle.component_merge(n, cs["perm"], np.ones(8, np.int8)).tolist() == [1, 0, 1, 1, 1, 1, 1, 1, 1, 0]
+    rng = np.random.default_rng(3)
+    for _ in range(5):
+        n = 60
+        m = rng.random((n, n)) < 0.02
+        m = np.triu(m, 1); m = m | m.T
+        rp = np.r_[0, np.cumsum(m.sum(1))].astype(np.int32)
+        cl = np.concatenate([np.flatnonzero(m[i]) for i in range(n)]).astype(np.int32)
+        cs = oracle.component_split(dict(n=n, nnz=len(cl), row_ptr=rp, col=cl), 2)
+        seen, comps = np.zeros(n, bool), []
+        for v in range(n):                                # plain BFS in vertex order
+            if seen[v]:
+                continue
+            comp, todo = [], [v]
+            seen[v] = True
+            while todo:
+                u = todo.pop()
+                comp.append(u)
+                for wv in np.flatnonzero(m[u]):
+                    if not seen[wv]:
+                        seen[wv] = True; todo.append(int(wv))
+            if len(comp) >= 2:
+                comps.append(sorted(comp))
+        assert cs["perm"].tolist() == [v for c in comps for v in c]
+        assert np.diff(cs["inst_ptr"]).tolist() == [len(c) for c in comps]

@@ -173,6 +173,17 @@ QHAP_API qhap_status qhap_snp_refine(qhap_csr *graph, const qhap_bsb_params *par
                             int32_t *flip_count, int32_t *iterations /*HOST*/, int64_t *cuts /*HOST [max_iter]*/, void *workspace,
                             size_t *ws_bytes, void *stream);
 
+/* (f2) Connected components: the kept components (>= min_size vertices; numbered by their smallest
+ * vertex; vertices ascending inside a component) as ONE block-diagonal CSR for qhap_bsb_solve's batch mode (per-component
+ * c0 and best replica).  `out` arrays need the INPUT's sizes as capacity (row_ptr [n+1], col and the value arrays
+ * [graph->nnz]; a NULL value array is skipped); out->n and out->nnz are written.  perm: device [n] (new index -> old
+ * vertex); inst_ptr: HOST [n+1]; n_comp: HOST.  Synchronises the stream.
+ * qhap_component_merge: out[perm[i]] = comp_spins[i]; vertices of dropped components get 0 (unphased). */
+QHAP_API qhap_status qhap_component_split(const qhap_csr *graph, int32_t min_size, qhap_csr *out, int32_t *perm, int32_t *inst_ptr,
+                                 int32_t *n_comp, void *workspace, size_t *ws_bytes, void *stream);
+QHAP_API qhap_status qhap_component_merge(int32_t n, int32_t n_kept, const int32_t *perm, const int8_t *comp_spins, int8_t *out,
+                                 void *stream);
+
 QHAP_API const char *qhap_last_error(void);
 /* Number of CUDA kernels this library has launched in this process so far (monotonic; bench.py reports the difference
  * over its timed region as "gpu_launches"). */

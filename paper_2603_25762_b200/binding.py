@@ -26,6 +26,7 @@ QHAP_DENSE_NONE, QHAP_DENSE_FP16, QHAP_DENSE_BF16 = 0, 1, 2
 EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_bsb_solve", "qhap_cut_eval",
            "qhap_phase_readout_reads", "qhap_phase_readout_snps", "qhap_block_split", "qhap_block_stitch",
            "qhap_gauge_transform", "qhap_flip_count_update", "qhap_refine_readout", "qhap_snp_refine",
+           "qhap_component_split", "qhap_component_merge",
            "qhap_last_error", "qhap_launch_count", "qhap_version"]
 
 
@@ -47,7 +48,7 @@ class _BsbParams(C.Structure):
                 ("finalize", C.c_int32), ("dense_bn", C.c_int32)]
 
 
-for _name in EXPORTS[:12]:
+for _name in EXPORTS[:14]:
     getattr(_lib, _name).restype = C.c_int
 _lib.qhap_last_error.restype = C.c_char_p
 _lib.qhap_version.restype = C.c_char_p
@@ -426,3 +427,39 @@ def qhap_snp_refine(graph: Csr, *, replicas: int, steps_total: int, max_iter: in
     ws_bytes = C.c_size_t(workspace.numel())
     _check(call(_ptr(workspace), C.byref(ws_bytes)), "qhap_snp_refine")
     return dict(flip_count=flip[:n], iterations=int(iters.value), cuts=[int(c) for c in cuts[:iters.value]], workspace=workspace)
+
+
+# ------------------------------------------------------------------ (f2) connected components, per-component batching
+def qhap_component_split(graph: Csr, min_size: int = 2):
+    """-> (block-diagonal Csr of the kept components with inst_ptr set, perm tensor [n_kept] int32)."""
+    dev = _dev()
+    n, nnz = graph.n, graph.nnz
+
+    def like(t, dt):
+        return torch.empty(max(nnz, 1), dtype=dt, device=dev) if t is not None else None
+    out = Csr(0, 0, torch.empty(n + 1, dtype=torch.int32, device=dev), torch.empty(max(nnz, 1), dtype=torch.int32, device=dev),
+              like(graph.d, torch.int32), like(graph.c, torch.int32), like(graph.w_fx, torch.int64), like(graph.w, torch.float32))
+    perm = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    inst_ptr = np.zeros(n + 1, np.int32)
+    n_comp = C.c_int32(0)
+    gs, os_ = graph.c_struct(), out.c_struct()
+
+    def call(ws, ws_bytes):
+        return _lib.qhap_component_split(C.byref(gs), C.c_int32(min_size), C.byref(os_), _ptr(perm), inst_ptr.ctypes.data_as(C.c_void_p),
+                                         C.byref(n_comp), ws, ws_bytes, _stream())
+    ws_bytes = C.c_size_t(0)
+    _check(call(None, C.byref(ws_bytes)), "qhap_component_split (size query)")
+    ws = _workspace(ws_bytes.value)
+    ws_bytes = C.c_size_t(ws.numel())
+    _check(call(_ptr(ws), C.byref(ws_bytes)), "qhap_component_split")
+    m, mnnz = int(os_.n), int(os_.nnz)
+    res = Csr(m, mnnz, out.row_ptr[:m + 1], out.col[:mnnz], *(t[:mnnz] if t is not None else None for t in (out.d, out.c, out.w_fx, out.w)),
+              inst_ptr=inst_ptr[:n_comp.value + 1].copy())
+    return res, perm[:m]
+
+
+def qhap_component_merge(n: int, perm: torch.Tensor, comp_spins: torch.Tensor) -> torch.Tensor:
+    out = torch.empty(max(n, 1), dtype=torch.int8, device=_dev())
+    _check(_lib.qhap_component_merge(C.c_int32(n), C.c_int32(perm.numel()), _ptr(perm), _ptr(comp_spins), _ptr(out), _stream()),
+           "qhap_component_merge")
+    return out[:n]

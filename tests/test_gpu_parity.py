@@ -661,3 +661,69 @@ def test_refine_loop_against_oracle(B, oracle, torch_mod):
             assert gm["se"] <= om["se"] + 0.001
             if flip_rate == 0.0:
                 assert gres["iterations"] == ores["iterations"] <= 3 and gm["se"] == 0.0 and gm["he"] == 0.0
+
+
+# ------------------------------------------------------------------ (f2) connected components, per-component batching
+def gapped_fragments(seed):
+    """Three stretches of reads separated by coverage gaps -> several components plus uncovered / singleton SNPs."""
+    parts = [synth.make_fragments(seed=seed + k, L=120_000, n_snp=150, n_reads=90, len_law=("uniform", 6_000, 20_000), flip=0.03,
+                                  missing=0.02, qual=("normal", 18, 5, 3, 40)) for k in range(3)]
+    n_snp = 3 * 150 + 20
+    fp, si, al, qu, ha = [0], [], [], [], np.zeros(n_snp, np.uint8)
+    for k, f in enumerate(parts):
+        off = k * 160                                     # 10 uncovered SNPs between the stretches
+        for i in range(f.n_frag):
+            sl = slice(int(f.frag_ptr[i]), int(f.frag_ptr[i + 1]))
+            si.append(f.snp_idx[sl] + off); al.append(f.allele[sl]); qu.append(f.qual[sl]); fp.append(fp[-1] + (sl.stop - sl.start))
+        ha[off:off + 150] = f.hap_a
+    return synth.Fragments(n_frag=len(fp) - 1, n_snp=n_snp, frag_ptr=np.array(fp, np.int64), snp_idx=np.concatenate(si).astype(np.int32),
+                           allele=np.concatenate(al).astype(np.uint8), qual=np.concatenate(qu).astype(np.uint8),
+                           frag_flags=np.zeros(len(fp) - 1, np.uint8), h1=np.zeros(n_snp, np.uint8), hap_a=ha,
+                           frag_hap=np.zeros(len(fp) - 1, np.uint8), snp_pos=np.arange(n_snp, dtype=np.int64))
+
+
+@pytest.mark.parametrize("min_size", [2, 1])
+def test_component_split_bit_exact_and_batched_solve(B, oracle, torch_mod, min_size):
+    fr = gapped_fragments(31)
+    g = oracle.snp_graph(fr, 10, 0.1)
+    ocs = oracle.component_split(g, min_size)
+    dcs, perm = B.qhap_component_split(B.upload_csr(g), min_size)
+    h = dcs.to_host()
+    assert h["n"] == ocs["n"] and h["nnz"] == ocs["nnz"] and len(ocs["inst_ptr"]) >= 4
+    for k in ("row_ptr", "col", "w_fx", "w"):
+        assert np.array_equal(h[k], ocs[k]), k
+    assert np.array_equal(perm.cpu().numpy(), ocs["perm"]) and np.array_equal(dcs.inst_ptr, ocs["inst_ptr"])
+    if min_size != 2:
+        return
+    # per-component solve (per-instance c0, best replica per component) and merge back; against the oracle per component
+    R, T = 32, 300
+    res = B.qhap_bsb_solve(dcs, replicas=R, steps_total=T, seed=9, weight_mode=2, path=2)
+    x0, y0 = synth.bsb_init_state(9, ocs["n"], R)
+    spins = res["best_spins"].cpu().numpy()
+    for b in range(len(ocs["inst_ptr"]) - 1):
+        lo, hi = int(ocs["inst_ptr"][b]), int(ocs["inst_ptr"][b + 1])
+        rp = (ocs["row_ptr"][lo:hi + 1] - ocs["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(ocs["row_ptr"][lo]), int(ocs["row_ptr"][hi]))
+        cl = (ocs["col"][sl] - lo).astype(np.int32)
+        o = oracle.solve(rp, cl, ocs["w_fx"][sl], (-ocs["w"][sl]).astype(np.float32), x0[lo:hi], y0[lo:hi], steps_total=T, n_threads=4)
+        gcut = int(res["best_cut"].cpu()[b])
+        assert gcut >= o["best_cut"] - 0.005 * abs(o["best_cut"]), (b, gcut, o["best_cut"])
+        ccut, _ = oracle.cut_eval(rp, cl, ocs["w_fx"][sl], spins[lo:hi])
+        assert ccut[0] == gcut
+    merged = B.qhap_component_merge(g["n"], perm, res["best_spins"]).cpu().numpy()
+    assert np.array_equal(merged, oracle.component_merge(g["n"], ocs["perm"], spins))
+    assert (merged == 0).sum() == g["n"] - ocs["n"] >= 20
+
+
+def test_component_split_read_graph_and_empty(B, oracle, torch_mod):
+    fr = gapped_fragments(41)
+    g = oracle.read_graph(fr)
+    ocs = oracle.component_split(g, 2)
+    dcs, perm = B.qhap_component_split(B.upload_csr(g), 2)
+    h = dcs.to_host()
+    for k in ("row_ptr", "col", "d", "c"):
+        assert np.array_equal(h[k], ocs[k]), k
+    assert np.array_equal(perm.cpu().numpy(), ocs["perm"]) and np.array_equal(dcs.inst_ptr, ocs["inst_ptr"])
+    empty = dict(n=5, nnz=0, row_ptr=np.zeros(6, np.int32), col=np.zeros(0, np.int32), w_fx=np.zeros(0, np.int64), w=np.zeros(0, np.float32))
+    dcs, perm = B.qhap_component_split(B.upload_csr(empty), 2)
+    assert dcs.n == 0 and dcs.nnz == 0 and perm.numel() == 0 and dcs.inst_ptr.tolist() == [0]

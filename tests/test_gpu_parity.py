@@ -172,7 +172,7 @@ def test_cut_eval_empty_graph(B, torch_mod):
 
 # ------------------------------------------------------------------------------------------ (3)(4) bSB steps
 def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, steps=50, path=2, dense_J=None, inst_ptr=None,
-                       c0=None, tile_skip=0, expect_full=False):
+                       c0=None, tile_skip=0, expect_full=False, min_horizon=MIN_HORIZON):
     """Trajectory parity over the first `steps` steps from identical fp32 initial states (R18).
 
     (a) RESYNCHRONISED: at every step k the GPU starts from fp32(oracle state after k steps) and takes ONE step; the oracle
@@ -256,7 +256,7 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
     out["tainted"] = int(tainted.sum())
     assert out["tainted"] <= max(2, 0.5 * R), out     # the free-running check must not become vacuous
     assert out["excluded"] <= 1e-3 * n * R * steps * 2
-    assert out["horizon"] >= min(steps, MIN_HORIZON), out
+    assert out["horizon"] >= min(steps, min_horizon), out
     return out
 
 
@@ -727,3 +727,34 @@ def test_component_split_read_graph_and_empty(B, oracle, torch_mod):
     empty = dict(n=5, nnz=0, row_ptr=np.zeros(6, np.int32), col=np.zeros(0, np.int32), w_fx=np.zeros(0, np.int64), w=np.zeros(0, np.float32))
     dcs, perm = B.qhap_component_split(B.upload_csr(empty), 2)
     assert dcs.n == 0 and dcs.nnz == 0 and perm.numel() == 0 and dcs.inst_ptr.tolist() == [0]
+
+
+# ------------------------------------------- (f3) read graph with Pore-C fragments: band structure lost
+def test_read_graph_with_porec_fragments_on_tile_paths(B, oracle, torch_mod):
+    """Pore-C fragments enter the read graph unweighted (L348) and connect reads far apart in start order, so J is not
+    banded: the dense tile_skip lists and the block path's tiles / remainder come from the actual occupancy.
+    Graph build bit-exact; dense tile_skip == full GEMM bit for bit; block path against the oracle and the CSR path."""
+    fr = porec_like(seed=23, n_snp=900, n_reads=700)
+    g = oracle.read_graph(fr)
+    rows = np.repeat(np.arange(g["n"]), np.diff(g["row_ptr"]))
+    assert (np.abs(g["col"] - rows) > 128).sum() > 50, "the case must contain long-range read-read edges"
+    dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=0, dense_dtype=B.QHAP_DENSE_FP16)
+    assert_csr_equal(dg.to_host(), g, ("d", "c"))
+    w = oracle.read_weights(g, 0)
+    outs = []
+    for path, skip in ((1, 0), (1, 1), (4, 0), (2, 0)):
+        res = B.qhap_bsb_solve(dg, replicas=96, steps_total=500, steps_run=6, seed=3, weight_mode=0, path=path,   # 6 steps: before
+                               dense_J=J if path == 1 else None, tile_skip=skip, dense_bn=64, finalize=False)          # walls amplify
+        outs.append((res["x"].cpu().numpy(), res["y"].cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    for k in (2,):
+        assert np.abs(outs[k][0] - outs[3][0]).max() <= TRAJ_TOL and np.abs(outs[k][1] - outs[3][1]).max() <= TRAJ_TOL
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 0, g["n"], 96, 500, 3, steps=20, path=4, min_horizon=3)   # stiff: w = D
+    print(f"read graph with Pore-C fragments, block path: {fmt_traj(o)}")
+    res = B.qhap_bsb_solve(dg, replicas=64, steps_total=500, seed=3, weight_mode=0, path=4)
+    x0, y0 = synth.bsb_init_state(3, g["n"], 64)
+    ores = oracle.solve(g["row_ptr"], g["col"], w, (-w).astype(np.float32), x0, y0, steps_total=500, n_threads=8)
+    gcut = int(res["best_cut"].cpu()[0])
+    assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
+    ccut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, res["best_spins"].cpu().numpy())
+    assert ccut[0] == gcut

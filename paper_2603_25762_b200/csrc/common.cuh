@@ -96,8 +96,9 @@ inline bool workspace_protocol(const Workspace& need, void* workspace, size_t* w
 // Exclusive scan of `n` int32 counts into out[0..n] (out[n] = total), in place allowed (out == in is fine when
 // in has n+1 slots).  Single launch; total returned through *total_dev (int64, device) when not NULL.
 // Sets *overflow_dev (int32, device) to 1 if the total does not fit int32.
+// `scratch` (optional, device, ceil(n / 4096) + 1 int64): enables the multi-CTA scan for long arrays.
 qhap_status exclusive_scan_i32(const int32_t* in, int32_t* out, int64_t n, int64_t* total_dev, int32_t* overflow_dev,
-                               cudaStream_t stream);
+                               cudaStream_t stream, int64_t* scratch = nullptr);
 
 static inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 

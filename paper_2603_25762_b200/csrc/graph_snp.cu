@@ -305,6 +305,7 @@ extern "C" qhap_status qhap_build_snp_graph(const qhap_frags* fr, int32_t linkag
   c.flags = ws.take<int32_t>(4);
   c.total = ws.take<int64_t>(2);
   c.table = ws.take<double>(94 * 94);
+  int64_t* scan_scratch = ws.take<int64_t>(size_t(std::max(nf, ns)) / 4096 + 2);
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
@@ -326,13 +327,13 @@ extern "C" qhap_status qhap_build_snp_graph(const qhap_frags* fr, int32_t linkag
     count_nonmissing_kernel<<<int(ceil_div(int64_t(nf) * 32, 256)), 256, 0, stream>>>(nf, fr->frag_ptr, fr->allele, c.k);
     QHAP_LAUNCH_CHECK();
   }
-  QHAP_TRY(exclusive_scan_i32(c.k, c.k, nf, c.total, c.flags, stream));
+  QHAP_TRY(exclusive_scan_i32(c.k, c.k, nf, c.total, c.flags, stream, scan_scratch));
   if (nf > 0) {
     compact_kernel<<<int(ceil_div(int64_t(nf) * 32, 256)), 256, 0, stream>>>(nf, fr->frag_ptr, fr->snp_idx, fr->allele, fr->qual,
                                                                          fr->h1, c);
     QHAP_LAUNCH_CHECK();
   }
-  QHAP_TRY(exclusive_scan_i32(c.colptr, c.colptr, ns, nullptr, nullptr, stream));
+  QHAP_TRY(exclusive_scan_i32(c.colptr, c.colptr, ns, nullptr, nullptr, stream, scan_scratch));
   int64_t cnnz = 0;
   QHAP_CUDA_TRY(cudaMemcpyAsync(&cnnz, c.total, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
   QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
@@ -346,7 +347,7 @@ extern "C" qhap_status qhap_build_snp_graph(const qhap_frags* fr, int32_t linkag
     QHAP_CUDA_TRY(cudaMemsetAsync(out->row_ptr, 0, sizeof(int32_t) * (size_t(ns) + 1), stream));
     QHAP_TRY(launch_rows<false>(ns, fr->frag_flags, linkage_tenths, alpha, c, out->row_ptr, nullptr, nullptr, nullptr, stream));
   }
-  QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, ns, c.total + 1, c.flags + 1, stream));
+  QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, ns, c.total + 1, c.flags + 1, stream, scan_scratch));
   int64_t total = 0;
   int32_t flags[4] = {0, 0, 0, 0};
   QHAP_CUDA_TRY(cudaMemcpyAsync(&total, c.total + 1, sizeof(total), cudaMemcpyDeviceToHost, stream));

@@ -69,7 +69,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
-  QHAP_REQUIRE(x && y, "x and y must not be NULL");
+  QHAP_REQUIRE((x && y) || graph->n == 0, "x and y must not be NULL");
   QHAP_REQUIRE(n == 0 || (graph->row_ptr && (graph->nnz == 0 || graph->col)), "graph arrays must not be NULL");
   if (p->weight_mode == QHAP_WEIGHT_FX) QHAP_REQUIRE(graph->nnz == 0 || graph->w_fx, "w_fx required for weight_mode 2");
   else QHAP_REQUIRE(graph->nnz == 0 || (graph->d && (p->weight_mode == 0 || graph->c)), "d (and c) required for weight_mode 0/1");

@@ -758,3 +758,39 @@ def test_read_graph_with_porec_fragments_on_tile_paths(B, oracle, torch_mod):
     assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
     ccut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, res["best_spins"].cpu().numpy())
     assert ccut[0] == gcut
+
+
+# ------------------------------------------------------------------------------------- degenerate inputs, every path
+def test_bsb_solve_degenerate_inputs(B, oracle, torch_mod):
+    """No edges (F = 0: each spin follows the scalar recurrence), a single replica, an empty graph, zero steps."""
+    n, R, T = 70, 3, 40
+    g = dict(n=n, nnz=0, row_ptr=np.zeros(n + 1, np.int32), col=np.zeros(0, np.int32), d=np.zeros(0, np.int32), c=np.zeros(0, np.int32))
+    x0, y0 = synth.bsb_init_state(5, n, R)
+    xo, yo, _ = oracle.bsb_run(g["row_ptr"], g["col"], np.zeros(0, np.float32), x0.astype(np.float64), y0.astype(np.float64),
+                               steps_total=T, n_threads=1)
+    dg = B.upload_csr(g)
+    J = torch_mod.zeros((72, 72), dtype=torch_mod.float16, device="cuda")
+    for path in (2, 3, 4, 1):
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, seed=5, weight_mode=1, path=path, dense_J=J if path == 1 else None)
+        assert np.abs(res["x"].cpu().numpy() - xo).max() <= 1e-5 and np.abs(res["y"].cpu().numpy() - yo).max() <= 1e-5, path
+        assert int(res["best_cut"].cpu()[0]) == 0 and int(res["best_replica"].cpu()[0]) == 0
+    # single replica on a real graph, all paths agree with the oracle over the first steps
+    fr, p = synth.make_config(0)
+    og = oracle.read_graph(fr)
+    w = oracle.read_weights(og, 1)
+    dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, 1)
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], (-w).astype(np.float32), x0.astype(np.float64), y0.astype(np.float64),
+                               steps_total=p["T"], steps_run=8, n_threads=1)
+    for path in (2, 3, 4, 1):
+        res = B.qhap_bsb_solve(dg, replicas=1, steps_total=p["T"], steps_run=8, seed=p["seed"], weight_mode=1, path=path,
+                               dense_J=J if path == 1 else None, finalize=False)
+        assert np.abs(res["x"].cpu().numpy() - xo).max() <= TRAJ_TOL, path
+        # zero steps: the seeded state comes back untouched
+        res0 = B.qhap_bsb_solve(dg, replicas=1, steps_total=p["T"], steps_run=0, seed=p["seed"], weight_mode=1, path=path,
+                                dense_J=J if path == 1 else None, finalize=False)
+        assert np.array_equal(res0["x"].cpu().numpy(), x0) and np.array_equal(res0["y"].cpu().numpy(), y0)
+    # empty graph
+    e = dict(n=0, nnz=0, row_ptr=np.zeros(1, np.int32), col=np.zeros(0, np.int32), d=np.zeros(0, np.int32), c=np.zeros(0, np.int32))
+    res = B.qhap_bsb_solve(B.upload_csr(e), replicas=4, steps_total=10, seed=1, weight_mode=1, path=2)
+    assert res["x"].numel() == 0 and int(res["best_cut"].cpu()[0]) == 0

@@ -443,7 +443,7 @@ def run_ours(args):
         for line in prof.read_text().splitlines()[1:]:
             f = line.split(",")
             if len(f) >= 3 and f[1] == str(args.config):
-                for rl in [roofline] + [v for k, v in extra.items() if k.startswith("roofline")]:
+                for rl in [roofline] + [v for k, v in extra.items() if k.startswith("roofline") and isinstance(v, dict)]:
                     if rl["kernel"] == f[0]:
                         rl["traffic"] = float(f[2])
 

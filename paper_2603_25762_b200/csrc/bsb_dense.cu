@@ -34,17 +34,20 @@ constexpr int kBK = 64;                  // spins per k-block: 64 fp16 = one 128
 constexpr int kMaxBN = 256;              // output spins per tile (UMMA N), runtime 32..256 in steps of 32
 constexpr int kMaxStages = 8;             // shared-memory pipeline depth: as many stages as fit (3 at BN = 256, 5 at BN = 64)
 constexpr int kStageX = kBM * kBK * 2;               // 16 KB each for x_hi, x_lo
-constexpr int kSmemBudget = 216 * 1024;              // operand stages; + 1 KB alignment slack + barriers <= 227 KB
+constexpr int kSmemBudget = 224 * 1024;              // operand stages (+ fp16 staging + state ring); + 1 KB slack + 1 KB barriers <= 227 KB
 constexpr int kEpiWarps = 16;
 constexpr int kChunk = 8;                // accumulator columns (spins) per tcgen05.ld in the epilogue
 constexpr int kThreads = 64 + 32 * kEpiWarps;
+constexpr int kRingSlot = kChunk * 32 * 4;           // one work item of x (or y): 8 spins x 32 replicas fp32 = 1 KB
+constexpr int kRingBytes = kEpiWarps * 2 * 2 * kRingSlot;   // per warp: 2 slots x (x, y)
 constexpr int kTmemCols = 512;                       // 2 accumulator stages x 256 columns
-constexpr size_t kSmemBytes = size_t(kSmemBudget) + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr size_t kSmemBytes = size_t(kSmemBudget) + 1024 /*alignment slack*/ + 1024 /*barriers*/;
 
 struct DenseArgs {
   int32_t n, R, n_k;          // spins, replicas, row pitch (elements) of the fp16 copies
   int32_t BN;                 // tile width in output spins
   int32_t n_stages;           // shared-memory stages of (BN x 64 J tile, 128 x 64 x_hi, 128 x 64 x_lo)
+  int32_t ring;               // 1: the fp32 state of the work items arrives through per-warp TMA boxes (BN == 64, R % 4 == 0)
   int32_t stage_out;          // 1: the fp16 copies leave through swizzled shared-memory tiles and TMA stores (BN == 64)
   int32_t n_tiles_m, n_tiles_n, n_kblocks;
   const int32_t* kb_cnt;      // [n_tiles_n] number of listed k-blocks per N tile, or nullptr = all k-blocks
@@ -179,7 +182,8 @@ __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
                   const __grid_constant__ CUtensorMap tm_xh,
                   const __grid_constant__ CUtensorMap tm_xl, const __grid_constant__ CUtensorMap tm_oh,
-                  const __grid_constant__ CUtensorMap tm_ol, const DenseArgs a) {
+                  const __grid_constant__ CUtensorMap tm_ol, const __grid_constant__ CUtensorMap tm_sx,
+                  const __grid_constant__ CUtensorMap tm_sy, const DenseArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;       // 128B swizzle needs 1024-byte alignment
   const int kStages = a.n_stages;
@@ -191,6 +195,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + s); };
   auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 2 + s); };
   const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStages + 4);
+  auto ring_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 6 + s); };
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && ptx::elect_one()) {
@@ -205,6 +210,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       ptx::mbar_init(tfull_bar(s), 1);
       ptx::mbar_init(tempty_bar(s), kEpiWarps);
     }
+    for (int s = 0; s < 2 * kEpiWarps; ++s) ptx::mbar_init(ring_bar(s), 1);
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc(tmem_slot, kTmemCols);
@@ -308,6 +314,28 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       ch += P;
       if (ch * kChunk >= a.BN || (tile / a.n_tiles_m) * a.BN + ch * kChunk >= a.n) { tile += gridDim.x; ch = par; }
     };
+    // last chunk of this warp in a tile: hand the accumulator stage back; with fp16 staging, all epilogue warps have then
+    // written their pieces of the tile -> one thread hands the two staging tiles to TMA.  The elected thread first waits
+    // until the previous tile's stores have finished reading their buffer, so that after the barrier every warp may
+    // overwrite that buffer (it is the next tile's).
+    auto tile_done = [&](int tile, uint32_t stg) {
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      if (a.stage_out) {
+        ptx::fence_proxy_async();
+        if (ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
+        ptx::named_barrier_sync(1, kEpiWarps * 32);
+        if (ew == 0 && lane == 0) {
+          const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+          ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
+          ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+          ptx::tma_store_commit();
+        }
+        ++tcount;
+      }
+    };
     auto step = [&](int& tile, int& ch, const float (&xc)[kChunk], const float (&yc)[kChunk], float (&xn)[kChunk],
                     float (&yn)[kChunk]) -> bool {
       if (ch == par) {                         // first chunk of a tile: the accumulator must be complete
@@ -323,30 +351,61 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       ptx::tmem_ld_wait();
       const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
       epi_update_store(a, ec, tile, ch, v, xc, yc, stg);
-      if (ntile != tile) {                     // last chunk of this warp in the tile: hand the accumulator stage back
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
-        if (a.stage_out) {
-          // all epilogue warps have written their pieces of this tile -> one thread hands the two tiles to TMA.
-          // The elected thread first waits until the previous tile's stores have finished reading their buffer, so
-          // that after the barrier every warp may overwrite that buffer (it is the next tile's).
-          ptx::fence_proxy_async();
-          if (ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
-          ptx::named_barrier_sync(1, kEpiWarps * 32);
-          if (ew == 0 && lane == 0) {
-            const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
-            ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
-            ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
-            ptx::tma_store_commit();
-          }
-          ++tcount;
-        }
-      }
+      if (ntile != tile) tile_done(tile, stg);
       tile = ntile; ch = nch;
       return nhave;
     };
+    if (a.ring) {
+      // State through TMA: every warp owns two 2 KB slots (x and y of one work item: a box of 8 spins x 32 replicas
+      // each).  The item two ahead is requested as soon as the current item's values are in registers, so the loads
+      // need no registers, no address arithmetic and no LSU slots; out-of-range rows / replicas arrive as zeros.
+      const uint32_t ring_w = stg_base + 4u * kStageX + uint32_t(ew) * (4u * kRingSlot);
+      const uint32_t rbar0 = ring_bar(2 * ew);
+      auto issue = [&](int tile, int ch, int slot) {
+        if (ptx::elect_one()) {
+          const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+          const uint32_t dst = ring_w + uint32_t(slot) * (2u * kRingSlot);
+          ptx::mbar_arrive_expect_tx(rbar0 + 8u * slot, 2u * kRingSlot);
+          ptx::tma_load_2d(dst, &tm_sx, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
+          ptx::tma_load_2d(dst + kRingSlot, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
+        }
+        __syncwarp();
+      };
+      int t0 = blockIdx.x, c0 = par, t1 = t0, c1i = c0, t2, c2i;
+      if (t0 < n_tiles) {
+        issue(t0, c0, 0);
+        advance(t1, c1i);
+        if (t1 < n_tiles) issue(t1, c1i, 1);
+        t2 = t1; c2i = c1i;
+        if (t1 < n_tiles) advance(t2, c2i);
+      }
+      for (uint32_t k = 0; t0 < n_tiles; ++k) {
+        const int slot = int(k & 1u);
+        if (c0 == par) {                         // first chunk of a tile: the accumulator must be complete
+          ptx::mbar_wait(tfull_bar(acc), acc_phase);
+          ptx::tc_fence_after();
+        }
+        uint32_t v[kChunk];
+        ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + c0 * kChunk), v);
+        ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
+        float xv[kChunk], yv[kChunk];
+        const uint32_t src = ring_w + uint32_t(slot) * (2u * kRingSlot) + uint32_t(lane) * 4u;
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(xv[j]) : "r"(src + uint32_t(j) * 128u));
+          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
+        }
+        __syncwarp();                            // every lane has its values: the slot may be refilled
+        if (t1 < n_tiles && t2 < n_tiles) issue(t2, c2i, slot);
+        ptx::tmem_ld_wait();
+        const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
+        epi_update_store(a, ec, t0, c0, v, xv, yv, stg);
+        if (t1 != t0) tile_done(t0, stg);
+        t0 = t1; c0 = c1i; t1 = t2; c1i = c2i;
+        if (t2 < n_tiles) advance(t2, c2i);
+      }
+      if (a.stage_out && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
+    } else {
     int tile = blockIdx.x, ch = par;
     if (tile < n_tiles) {
       float xa[kChunk], ya[kChunk], xb[kChunk], yb[kChunk];
@@ -356,6 +415,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if (!step(tile, ch, xb, yb, xa, ya)) break;
       }
       if (a.stage_out && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();   // smem must outlive the bulk reads
+    }
     }
   }
 
@@ -603,7 +663,8 @@ __global__ void __launch_bounds__(256) block_fill_kernel(int32_t n, const int32_
 // ------------------------------------------------------------------------------------------- host side
 // One step launch with the programmatic-stream-serialization attribute (see the kernel: griddepcontrol.wait).
 qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, const CUtensorMap& tjl, const CUtensorMap& th,
-                        const CUtensorMap& tl, const CUtensorMap& toh, const CUtensorMap& tol, const DenseArgs& a) {
+                        const CUtensorMap& tl, const CUtensorMap& toh, const CUtensorMap& tol, const CUtensorMap& tsx,
+                        const CUtensorMap& tsy, const DenseArgs& a) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(unsigned(grid));
   cfg.blockDim = dim3(kThreads);
@@ -614,7 +675,7 @@ qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, co
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_step_kernel, tj, tjl, th, tl, toh, tol, a));
+  QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_step_kernel, tj, tjl, th, tl, toh, tol, tsx, tsy, a));
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;
 }
@@ -655,6 +716,32 @@ qhap_status make_map(CUtensorMap* m, const void* base, uint64_t inner, uint64_t 
     return QHAP_ERR_CUDA;
   }
   return QHAP_OK;
+}
+
+// fp32 state [n][R] (replica index contiguous): box = one work item of a warp, 32 replicas x kChunk spins, no swizzle, OOB -> 0.
+qhap_status make_state_map(CUtensorMap* m, const float* base, int32_t n, int32_t R) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) {
+    set_error("cuTensorMapEncodeTiled not available from the driver");
+    return QHAP_ERR_CUDA;
+  }
+  const cuuint64_t dims[2] = {cuuint64_t(R), cuuint64_t(n)};
+  const cuuint64_t strides[1] = {cuuint64_t(R) * 4};
+  const cuuint32_t box[2] = {32, uint32_t(kChunk)};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    set_error("cuTensorMapEncodeTiled (state) failed with CUresult %d", int(r));
+    return QHAP_ERR_CUDA;
+  }
+  return QHAP_OK;
+}
+
+// state ring usable: tile one box wide, row pitch a multiple of 16 bytes, 16-byte aligned bases
+bool ring_ok(int32_t BN, int32_t R, const float* x, const float* y) {
+  return BN == kBK && R % 4 == 0 && ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(y)) & 15) == 0;
 }
 
 int32_t pitch_of(int32_t n) { return int32_t(ceil_div(n, 64) * 64); }
@@ -718,7 +805,8 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   // fp16 copies through TMA stores: the tile must be exactly one 64-column box wide (tile_skip's width); the two
   // staging buffers (2 x 32 KB) come out of the operand-stage budget
   a.stage_out = (BN == kBK) ? 1 : 0;
-  a.n_stages = std::min(kMaxStages, (kSmemBudget - (a.stage_out ? 4 * kStageX : 0)) / (BN * kBK * 2 + 2 * kStageX));
+  a.ring = ring_ok(BN, R, x, y) ? 1 : 0;
+  a.n_stages = std::min(kMaxStages, (kSmemBudget - (a.stage_out ? 4 * kStageX : 0) - (a.ring ? kRingBytes : 0)) / (BN * kBK * 2 + 2 * kStageX));
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = int32_t(ceil_div(n, BN));
   a.n_kblocks = n_kb;
@@ -733,7 +821,9 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
     attr_set = true;
   }
 
-  CUtensorMap tm_j, tm_h[2], tm_l[2];
+  CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
+  QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));
+  QHAP_TRY(make_state_map(&tm_sy, y, n, a.ring ? R : 4));
   QHAP_TRY(make_map(&tm_j, dense_J, uint64_t(ld), uint64_t(ld), uint64_t(ld), uint32_t(BN)));
   for (int b = 0; b < 2; ++b) {
     QHAP_TRY(make_map(&tm_h[b], xh[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
@@ -761,7 +851,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
     a.c3 = float(p.dt * p.a0);
     a.xh_out = xh[cur ^ 1];
     a.xl_out = xl[cur ^ 1];
-    QHAP_TRY(launch_step(grid, stream, tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a));
+    QHAP_TRY(launch_step(grid, stream, tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));
     cur ^= 1;
   }
   return QHAP_OK;
@@ -889,8 +979,9 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   DenseArgs a;
   a.n = n; a.R = R; a.n_k = n_k; a.BN = kBK;
   a.stage_out = 1;
+  a.ring = ring_ok(kBK, R, x, y) ? 1 : 0;
   a.j_terms = two_terms ? 2 : 1;
-  a.n_stages = std::min(kMaxStages, (kSmemBudget - 4 * kStageX) / (a.j_terms * kBK * kBK * 2 + 2 * kStageX));
+  a.n_stages = std::min(kMaxStages, (kSmemBudget - 4 * kStageX - (a.ring ? kRingBytes : 0)) / (a.j_terms * kBK * kBK * 2 + 2 * kStageX));
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = n_t;
   a.n_kblocks = n_t;
@@ -899,7 +990,9 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.x = x; a.y = y;
   QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
 
-  CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2];
+  CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2], tm_sx, tm_sy;
+  QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));
+  QHAP_TRY(make_state_map(&tm_sy, y, n, a.ring ? R : 4));
   const uint64_t brows = uint64_t(std::max<int64_t>(total_blocks, 1)) * kBK;
   QHAP_TRY(make_map(&tm_jh, jh, kBK, brows, kBK, kBK));
   QHAP_TRY(make_map(&tm_jl, two_terms ? jl : jh, kBK, brows, kBK, kBK));
@@ -924,7 +1017,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
       remainder_step_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, R, rem_ptr, rem_col, rem_val, c1plain, x, y);
       QHAP_LAUNCH_CHECK();
     }
-    QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], a));
+    QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));
     cur ^= 1;
   }
   return QHAP_OK;

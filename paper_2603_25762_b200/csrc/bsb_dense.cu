@@ -277,11 +277,21 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           const uint64_t djl = ptx::umma_desc_k_sw128(sj + kTileJ);
           const uint64_t dh = ptx::umma_desc_k_sw128(sj + kStageJ);
           const uint64_t dl = ptx::umma_desc_k_sw128(sj + kStageJ + kStageX);
+          // UMMA_K = 16 for 16-bit inputs: +32 B per step.  Two straight-line variants: a test of j_terms inside the
+          // unrolled issue sequence costs the full GEMM 12 % (measured: 165 -> 186 us per step at cfg1).
+          if (a.j_terms == 2) {
 #pragma unroll
-          for (int kk = 0; kk < kBK / 16; ++kk) {                         // UMMA_K = 16 for 16-bit inputs: +32 B per step
-            ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
-            ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
-            if (a.j_terms == 2) ptx::umma_f16(d_tmem, dh + 2u * kk, djl + 2u * kk, idesc, 1u);   // x_lo J_lo ~ 2^-22: dropped
+            for (int kk = 0; kk < kBK / 16; ++kk) {
+              ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+              ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
+              ptx::umma_f16(d_tmem, dh + 2u * kk, djl + 2u * kk, idesc, 1u);   // x_lo J_lo ~ 2^-22: dropped
+            }
+          } else {
+#pragma unroll
+            for (int kk = 0; kk < kBK / 16; ++kk) {
+              ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+              ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
+            }
           }
           ptx::umma_commit(empty_bar(stage));                            // frees the smem stage when these MMAs are done
           if (j == nkb - 1) ptx::umma_commit(tfull_bar(acc));            // accumulator complete -> epilogue

@@ -109,7 +109,7 @@ typedef struct {
   double c0;            /* <= 0: automatic 0.5 sqrt(N-1) / ||J||_F per instance                           */
   uint64_t seed;        /* used when init_state != 0                                                      */
   int32_t weight_mode;  /* QHAP_WEIGHT_*: which CSR arrays define w (J = -w)                              */
-  int32_t path;         /* 0 auto (3 if small, 1 if dense_J is given, else 4; 2 below 1024 vertices), 1 dense tcgen05 GEMM (needs dense_J), 2 sparse CSR, 3 shared-memory resident */
+  int32_t path;         /* 0 auto (3 if small, 1 if dense_J is given, else 4; 2 below 1024 or above 2^20 vertices), 1 dense tcgen05 GEMM (needs dense_J), 2 sparse CSR, 3 shared-memory resident */
                         /* (small problems, n R <= 65536: all steps in one launch; same bits as path 2),    */
                         /* 4 tcgen05 step on a block-compressed J built from the CSR (64 x 64 tiles; entries  */
                         /* of sparsely filled tiles -- long-range edges -- go through a remainder CSR gather; */

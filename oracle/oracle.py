@@ -1,8 +1,10 @@
 """ctypes front end of the QHap CPU oracle (oracle/qhap_oracle.cpp) -- TEST INFRASTRUCTURE ONLY.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / ``--impl reference`` legs may import
-this module.  It imports nothing from the CUDA package.  All arithmetic lives in the C++ file; this
-module compiles it with g++ (once, into oracle/_build/) and marshals numpy arrays.
+this module.  It imports nothing from the CUDA package.  The arithmetic of O1-O5 lives in the C++ file, which this
+module compiles with g++ (once, into oracle/_build/) and calls with numpy arrays; O6 (iterative refinement, Eq. 15-17)
+and O7 (connected components; scipy's connected_components is the library step) are plain numpy below.
+Pins: tests/test_oracle_pins.py (O6: gauge identity + planted recovery; O7: hand-made graph + plain BFS).
 """
 from __future__ import annotations
 

@@ -31,7 +31,7 @@ namespace {
 
 constexpr int kBM = 128;                 // replicas per tile (UMMA M)
 constexpr int kBK = 64;                  // spins per k-block: 64 fp16 = one 128-byte swizzle row
-constexpr int kMaxBN = 256;              // output spins per tile (UMMA N), runtime 32..256 in steps of 32
+constexpr int kMaxBN = 256;              // output spins per tile (UMMA N), runtime 32..256 in steps of 16
 constexpr int kMaxStages = 8;             // shared-memory pipeline depth: as many stages as fit (3 at BN = 256, 5 at BN = 64)
 constexpr int kStageX = kBM * kBK * 2;               // 16 KB each for x_hi, x_lo
 constexpr int kSmemBudget = 224 * 1024;              // operand stages (+ fp16 staging + state ring); + 1 KB slack + 1 KB barriers <= 227 KB
@@ -98,7 +98,7 @@ __device__ __forceinline__ void epi_pack(int j, float xn, uint32_t (&hp)[kChunk 
   else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
 }
 
-// fp32 state of one work item (16 spins x this thread's replica) -> registers; masked entries read as 0.
+// fp32 state of one work item (kChunk spins x this thread's replica) -> registers; masked entries read as 0.
 // Element offsets are 32-bit (the host checks n R < 2^32): one integer add and one wide multiply-add per address.
 __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, float (&xv)[kChunk],
                                          float (&yv)[kChunk]) {
@@ -123,7 +123,7 @@ __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec
 }
 
 // Fused update of one work item: y' = y + dt(-(a0 - a_k) x + c0 F), x' = x + dt a0 y', inelastic wall; stores x', y'
-// (fp32, coalesced across the warp's 32 replicas) and the fp16 split of x' (32 contiguous bytes per thread).
+// (fp32, coalesced across the warp's 32 replicas) and the fp16 split of x' (16 contiguous bytes per thread and array: into the staging tiles, or directly).
 __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tile, int ch,
                                                  const uint32_t (&v)[kChunk], const float (&xv)[kChunk],
                                                  const float (&yv)[kChunk], uint32_t stg) {
@@ -167,7 +167,7 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
       ptx::st_shared_v4(base + piece * 16u, hp[4 * q], hp[4 * q + 1], hp[4 * q + 2], hp[4 * q + 3]);
       ptx::st_shared_v4(base + kStageX + piece * 16u, lp[4 * q], lp[4 * q + 1], lp[4 * q + 2], lp[4 * q + 3]);
     }
-  } else if (r_ok && i0 < a.n) {               // n_k >= round_up(n, 64) keeps the 16-spin run in bounds
+  } else if (r_ok && i0 < a.n) {               // n_k >= round_up(n, 64) keeps the kChunk-spin run in bounds
     uint4* ph = reinterpret_cast<uint4*>(a.xh_out + size_t(r) * a.n_k + i0);
     uint4* pl = reinterpret_cast<uint4*>(a.xl_out + size_t(r) * a.n_k + i0);
 #pragma unroll

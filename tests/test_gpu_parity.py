@@ -794,3 +794,52 @@ def test_bsb_solve_degenerate_inputs(B, oracle, torch_mod):
     e = dict(n=0, nnz=0, row_ptr=np.zeros(1, np.int32), col=np.zeros(0, np.int32), d=np.zeros(0, np.int32), c=np.zeros(0, np.int32))
     res = B.qhap_bsb_solve(B.upload_csr(e), replicas=4, steps_total=10, seed=1, weight_mode=1, path=2)
     assert res["x"].numel() == 0 and int(res["best_cut"].cpu()[0]) == 0
+
+
+# ----------------------------------------------------------- BASELINE.json configs[3] at FULL size (block path, 47 blocks)
+def test_cfg3_full_size_sampled(B, oracle, torch_mod):
+    """cfg3 as `bench.py --config 3` runs it: 250k reads x 210k SNPs, SNP graph (depth 3/10) bit-exact, 47 blocks of 5,000
+    SNPs bit-exact, tcgen05 step on the block-compressed J with R = 256 and the device-side seeded start state: the first
+    10 steps of sampled replicas of the first and the last block against the oracle; after the full solve the cuts of
+    those blocks bit-exact and the stitched haplotype close to the planted one."""
+    fr, p = synth.make_config(3)
+    dfr = B.upload_frags(fr)
+    og = oracle.snp_graph(fr, p["linkage_tenths"], 0.1)
+    g = B.qhap_build_snp_graph(dfr, p["linkage_tenths"], 0.1)
+    assert_csr_equal(g.to_host(), og, ("w_fx", "w"))
+    win = synth.block_windows(fr.n_snp, p["block"], p["stride"])
+    obs = oracle.block_split(og, win)
+    bs = B.qhap_block_split(g, win)
+    assert_csr_equal(bs.to_host(), obs, ("w_fx", "w"))
+    n, R, T = obs["n"], p["R"], p["T"]
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    sample = np.array([0, 31, 128, R - 1])
+    res = B.qhap_bsb_solve(bs, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=2, path=4, finalize=False)
+    xg = res["x"].cpu().numpy()
+    blocks = (0, len(win) - 1)
+    sub = {}
+    for b in blocks:
+        lo, hi = int(obs["inst_ptr"][b]), int(obs["inst_ptr"][b + 1])
+        rp = (obs["row_ptr"][lo:hi + 1] - obs["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(obs["row_ptr"][lo]), int(obs["row_ptr"][hi]))
+        cl = (obs["col"][sl] - lo).astype(np.int32)
+        sub[b] = (lo, hi, rp, cl, sl)
+        xo, yo, _ = oracle.bsb_run(rp, cl, (-obs["w"][sl]).astype(np.float32), x0[lo:hi][:, sample].astype(np.float64),
+                                   y0[lo:hi][:, sample].astype(np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+        dx = np.abs(xg[lo:hi][:, sample] - xo).max()
+        print(f"cfg3 full size, block {b}: 10 steps, 4 sampled replicas: max|dx| {dx:.2e}")
+        assert dx <= TRAJ_TOL
+    res = B.qhap_bsb_solve(bs, replicas=R, steps_total=T, seed=p["seed"], weight_mode=2, path=4)
+    spins = res["best_spins"].cpu().numpy()
+    for b in blocks:
+        lo, hi, rp, cl, sl = sub[b]
+        ccut, _ = oracle.cut_eval(rp, cl, obs["w_fx"][sl], spins[lo:hi])
+        assert ccut[0] == int(res["best_cut"].cpu()[b]) > 0
+    st = B.qhap_block_stitch(fr.n_snp, win, res["best_spins"]).cpu().numpy()
+    assert np.array_equal(st, oracle.block_stitch(fr.n_snp, win, [spins[int(obs["inst_ptr"][b]):int(obs["inst_ptr"][b + 1])]
+                                                                  for b in range(len(win))]))
+    hap = B.qhap_phase_readout_snps(dfr.h1, torch_mod.from_numpy(st).cuda()).cpu().numpy()
+    covered = np.bincount(fr.snp_idx[fr.allele <= 1], minlength=fr.n_snp) > 0
+    m = oracle.switch_hamming(hap[covered], fr.hap_a[covered])
+    print(f"cfg3 full size: stitched SE {m['se']:.5f} HE {m['he']:.5f} over {int(covered.sum())} covered SNPs")
+    assert m["se"] <= 0.02

@@ -843,3 +843,26 @@ def test_cfg3_full_size_sampled(B, oracle, torch_mod):
     m = oracle.switch_hamming(hap[covered], fr.hap_a[covered])
     print(f"cfg3 full size: stitched SE {m['se']:.5f} HE {m['he']:.5f} over {int(covered.sum())} covered SNPs")
     assert m["se"] <= 0.02
+
+
+# ------------------------------------------------- BASELINE.json configs[4] at FULL size (hybrid block path, one instance)
+def test_cfg4_full_size_sampled(B, oracle, torch_mod):
+    """cfg4 as `bench.py --config 4` runs it: cfg3's reads + Pore-C fragments (about 500k long-range edges), one instance
+    of 210,000 SNPs, R = 128: SNP graph bit-exact; the first 10 steps of sampled replicas on the hybrid block path (tiles +
+    remainder CSR) and on the CSR path against the oracle run on exactly those replicas."""
+    fr, p = synth.make_config(4)
+    og = oracle.snp_graph(fr, p["linkage_tenths"], p["alpha"])
+    g = B.qhap_build_snp_graph(B.upload_frags(fr), p["linkage_tenths"], p["alpha"])
+    assert_csr_equal(g.to_host(), og, ("w_fx", "w"))
+    rows = np.repeat(np.arange(og["n"]), np.diff(og["row_ptr"]))
+    assert (np.abs(og["col"] - rows) > 4096).sum() > 500_000
+    n, R, T = og["n"], p["R"], p["T"]
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    sample = np.array([0, 63, R - 1])
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], (-og["w"]).astype(np.float32), x0[:, sample].astype(np.float64),
+                               y0[:, sample].astype(np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+    for path in (4, 2):
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=2, path=path, finalize=False)
+        dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
+        print(f"cfg4 full size, path {path}: 10 steps, 3 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL

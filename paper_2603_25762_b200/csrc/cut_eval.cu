@@ -10,7 +10,7 @@ namespace qhap {
 
 namespace {
 
-constexpr int kRowsPerWarp = 32;
+constexpr int kRowsPerWarp = 8;   // a CTA of 8 warps owns 64 consecutive rows and one chunk of replicas
 
 template <class SpinT, int VEC>
 struct SpinLoad;
@@ -49,26 +49,38 @@ __global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const in
                                                              const int32_t* __restrict__ inst_ptr,
                                                              unsigned long long* __restrict__ cut,
                                                              unsigned long long* __restrict__ wtot) {
-  const int lane = threadIdx.x & 31;
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  // Work item of a CTA = (tile of 8 x kRowsPerWarp consecutive rows, chunk of 32 x VEC replicas); its 8 warps split the
+  // rows.  The partial cuts of the 8 warps are summed in shared memory and leave with ONE atomicAdd per replica and CTA
+  // (integer adds: any order gives the same bits); a tile that straddles an instance boundary flushes per warp instead.
+  __shared__ long long s_acc[8][32 * VEC];
+  const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
   const int chunks = (R + 32 * VEC - 1) / (32 * VEC);
-  const int64_t n_tiles = (int64_t(n) + kRowsPerWarp - 1) / kRowsPerWarp;
-  const int64_t n_warps = (int64_t(gridDim.x) * blockDim.x) >> 5;
-  for (int64_t work = warp; work < n_tiles * chunks; work += n_warps) {
+  constexpr int kTileRows = 8 * kRowsPerWarp;
+  const int64_t n_tiles = (int64_t(n) + kTileRows - 1) / kTileRows;
+  for (int64_t work = blockIdx.x; work < n_tiles * chunks; work += gridDim.x) {
     const int chunk = int(work % chunks);
-    const int32_t a0 = int32_t(work / chunks) * kRowsPerWarp;
+    const int32_t t0 = int32_t(work / chunks) * kTileRows;
+    const int32_t a0 = min(n, t0 + wic * kRowsPerWarp);
     const int32_t a1 = min(n, a0 + kRowsPerWarp);
     const int r = chunk * 32 * VEC + lane * VEC;
     const bool active = r < R;  // R % VEC == 0 is guaranteed by the dispatcher
     // instance of the first row (binary search; inst_ptr is tiny)
     int inst = 0;
+    bool one_inst = true;         // the whole CTA tile lies in one instance (block-uniform)
     if (n_inst > 1) {
       int lo = 0, hi = n_inst;
+      const int32_t key = min(a0, n - 1);
       while (hi - lo > 1) {
         int mid = (lo + hi) >> 1;
-        if (inst_ptr[mid] <= a0) lo = mid; else hi = mid;
+        if (inst_ptr[mid] <= key) lo = mid; else hi = mid;
       }
       inst = lo;
+      lo = 0; hi = n_inst;
+      while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (inst_ptr[mid] <= t0) lo = mid; else hi = mid;
+      }
+      one_inst = min(n, t0 + kTileRows) <= inst_ptr[lo + 1];
     }
     int64_t acc[VEC];
 #pragma unroll
@@ -116,7 +128,27 @@ __global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const in
         }
       }
     }
-    flush(inst);
+    if (!one_inst) {
+      flush(inst);
+    } else {
+#pragma unroll
+      for (int k = 0; k < VEC; ++k) s_acc[wic][lane * VEC + k] = acc[k];
+      if (chunk == 0) {
+        int64_t t = warp_sum(wsum);
+        if (lane == 0 && t != 0) atomicAdd(&wtot[inst], (unsigned long long)t);
+      }
+      __syncthreads();
+      if (wic == 0 && active) {
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+          long long t = 0;
+#pragma unroll
+          for (int w8 = 0; w8 < 8; ++w8) t += s_acc[w8][lane * VEC + k];
+          if (t != 0) atomicAdd(&cut[size_t(inst) * R + r + k], (unsigned long long)t);
+        }
+      }
+    }
+    __syncthreads();
   }
 }
 
@@ -183,8 +215,8 @@ qhap_status launch_cut(const CsrView& g, int mode, const SpinT* spins, int32_t R
   if (g.n == 0 || R == 0) return QHAP_OK;
   const bool vec4 = (R % 4 == 0) && ((reinterpret_cast<uintptr_t>(spins) & (4 * sizeof(SpinT) - 1)) == 0);
   const int chunks = vec4 ? (R + 127) / 128 : (R + 31) / 32;
-  const int64_t work = ceil_div(g.n, kRowsPerWarp) * chunks;
-  const int blocks = int(std::min<int64_t>(ceil_div(work, 8), int64_t(sm_count()) * 8));
+  const int64_t work = ceil_div(g.n, 8 * kRowsPerWarp) * chunks;
+  const int blocks = int(std::max<int64_t>(1, std::min<int64_t>(work, int64_t(sm_count()) * 8)));
   auto* cu = reinterpret_cast<unsigned long long*>(cut);
   auto* wt = reinterpret_cast<unsigned long long*>(wtot);
   if (vec4)

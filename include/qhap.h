@@ -109,15 +109,20 @@ typedef struct {
   double c0;            /* <= 0: automatic 0.5 sqrt(N-1) / ||J||_F per instance                           */
   uint64_t seed;        /* used when init_state != 0                                                      */
   int32_t weight_mode;  /* QHAP_WEIGHT_*: which CSR arrays define w (J = -w)                              */
-  int32_t path;         /* 0 auto (3 if small, 1 if dense_J is given, else 4; 2 below 1024 or above 2^20 vertices), 1 dense tcgen05 GEMM (needs dense_J), 2 sparse CSR, 3 shared-memory resident */
-                        /* (small problems, n R <= 65536: all steps in one launch; same bits as path 2),    */
-                        /* 4 tcgen05 step on a block-compressed J built from the CSR (64 x 64 tiles; entries  */
-                        /* of sparsely filled tiles -- long-range edges -- go through a remainder CSR gather; */
-                        /* batches allowed; the plan synchronises the stream once or a few times)            */
-  int32_t tile_skip;    /* dense path: 1 = skip all-zero 64-column blocks of J (bit-identical result)     */
+  int32_t path;         /* which bSB step kernel:                                                           */
+                        /*  1 tcgen05 GEMM over the dense J (needs dense_J, fp16, one instance);              */
+                        /*  2 sparse CSR step;                                                                */
+                        /*  3 shared-memory resident (small problems, n R <= 65536: all steps in one launch;  */
+                        /*    same bits as path 2);                                                           */
+                        /*  4 tcgen05 step on a block-compressed J built from the CSR (64 x 64 tiles; entries */
+                        /*    of sparsely filled tiles -- long-range edges -- go through a remainder CSR      */
+                        /*    gather; batches allowed; the plan synchronises the stream once or a few times); */
+                        /*  0 auto: 3 if it fits, else 1 if dense_J is given, else 4 (2 below 1024 or above   */
+                        /*    2^20 vertices)                                                                  */
+  int32_t tile_skip;    /* path 1: 1 = visit only the 64-column blocks of J that hold a non-zero (bit-identical) */
   int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
   int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */
-  int32_t dense_bn;     /* dense path: tile width in output spins (multiple of 16 in 16..256); 0 = automatic          */
+  int32_t dense_bn;     /* path 1: tile width in output spins (multiple of 16 in 32..256); 0 = automatic      */
 } qhap_bsb_params;
 
 /* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`

@@ -212,6 +212,8 @@ def run_ours(args):
         tile_skip = 0
     else:
         path = {"auto": 1, "sparse": 2, "dense": 1, "dense-full": 1, "block": 4}[args.path]
+        if args.path == "auto" and n * R <= 65536:
+            path = 3                                  # config 0: the whole solve in one shared-memory-resident launch
         tile_skip = 0 if args.path == "dense-full" else 1
     dense_dtype = B.QHAP_DENSE_FP16 if path == 1 else B.QHAP_DENSE_NONE
     win = synth.block_windows(fr.n_snp, p["block"], p["stride"]) if "block" in p else None
@@ -390,7 +392,7 @@ def run_ours(args):
                 "peak_source": peaks["which"] + ": sustained bf16 (fp16 inputs run at the same kind::f16 rate)"}
 
     extra = {}
-    if path == 2:
+    if path in (2, 3):
         # algorithmic bytes per launch: 16 B of fp32 state per spin-update (read x, read y, write y, write x')
         # + the CSR once per launch (int32 col + fp32 val per directed entry, int32 row_ptr per row)
         # + SURVEY 8(d): 4 B per replica for every non-zero whose column lies far outside the swept band (|col - row| > 4096:
@@ -400,7 +402,7 @@ def run_ours(args):
         long_range = int((np.abs(hg["col"].astype(np.int64) - rows) > 4096).sum())   # x rows far outside the swept band
         alg_bytes = 16.0 * g.n * R + 8.0 * g.nnz + 4.0 * (g.n + 1) + 4.0 * R * long_range
         extra["long_range_nnz"] = long_range
-        roofline = {"kernel": "sparse_step_kernel", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
+        roofline = {"kernel": "sparse_step_kernel" if path == 2 else "bsb_resident_kernel (latency-bound: one launch runs all T steps; per-step figures)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9, "peak": peaks["hbm"],
                     "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms, "peak_source": peaks["which"]}
         roofline["frac"] = roofline["achieved"] / roofline["peak"]
     elif tile_skip or path == 4:
@@ -451,7 +453,7 @@ def run_ours(args):
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if blocks else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": workload_name(args.config, fr, p),
                       "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM)" if tile_skip else " full GEMM"),
-                               2: "sparse-csr", 4: "tcgen05 step on the block-compressed J (64 x 64 tiles built from the CSR)"}[path],
+                               2: "sparse-csr", 3: "shared-memory resident (one launch for all steps)", 4: "tcgen05 step on the block-compressed J (64 x 64 tiles built from the CSR)"}[path],
                       "weight_mode": "fixed-point Eq. 14" if snp else "D-C", "replicas_per_gpu": R, "spins_solved": n_solved, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                       "parallelism": f"blocks x{world} (strong)" if blocks else f"replicas x{world} (weak)"},
            "region_ms": ms, "edges_replicas_per_s": edges * R * T * (1 if blocks else world) / (ms * 1e-3), "undirected_edges": edges,

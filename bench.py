@@ -50,6 +50,8 @@ def parse_args():
                          "dense-full = the whole N x N GEMM); sparse = CSR; auto = dense")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU seconds of the oracle sample")
+    ap.add_argument("--refine-iters", type=int, default=0,
+                    help="SNP configs with one instance (config 4): also time qhap_snp_refine (Eq. 15-17) with at most this many solves")
     return ap.parse_args()
 
 
@@ -358,6 +360,26 @@ def run_ours(args):
                 "directed_edges": int(g0.nnz)}
 
     phases = phase_times()
+
+    # ---- the widened rows of SURVEY 8(f), timed once each (not part of the headline pass)
+    def timed_once(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        r = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return r, e0.elapsed_time(e1)
+
+    g_full = B.qhap_build_snp_graph(dfr, p.get("linkage_tenths", 10), p.get("alpha", 0.1)) if snp else \
+        B.qhap_build_read_graph(dfr, weight_mode=mode)[0]
+    B.qhap_component_split(g_full, 2)                                      # warm-up
+    (cs, _perm), cs_ms = timed_once(lambda: B.qhap_component_split(g_full, 2))
+    phases["component_split_ms"] = cs_ms
+    phases["components_kept"] = int(len(cs.inst_ptr) - 1)
+    if snp and win is None and args.refine_iters > 0:
+        rr, rf_ms = timed_once(lambda: B.qhap_snp_refine(g_full, replicas=R, steps_total=T, max_iter=args.refine_iters, seed=seed, path=path))
+        phases["refine"] = {"ms": rf_ms, "iterations": rr["iterations"], "cuts": rr["cuts"], "max_iter": args.refine_iters}
 
     # ---- roofline of the dominant kernel (the bSB step): launches timed with CUDA events on the launching stream
     J = None

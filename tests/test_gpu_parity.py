@@ -866,3 +866,25 @@ def test_cfg4_full_size_sampled(B, oracle, torch_mod):
         dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
         print(f"cfg4 full size, path {path}: 10 steps, 3 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
         assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
+
+
+# ------------------------------------------------------------------- non-default bSB constants on every step path
+@pytest.mark.parametrize("dt,a0,c0,begin", [(0.7, 1.5, 0.02, 0), (1.25, 1.0, 0.0, 900), (0.4, 0.6, 0.05, 37)])
+def test_bsb_constants_every_path(B, oracle, torch_mod, dt, a0, c0, begin):
+    """dt, a0, an explicit c0 and a resume point in the middle of the ramp reach every kernel the same way (R10b, R10c):
+    8 steps from the same state on the CSR, resident, dense and block paths against the oracle."""
+    fr, p = synth.make_config(0)
+    og = oracle.read_graph(fr)
+    w = oracle.read_weights(og, 1)
+    dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    R, T = 48, 1000
+    x0, y0 = synth.bsb_init_state(3, fr.n_frag, R)
+    x0 = (x0 * 6).clip(-1, 1).astype(np.float32)          # spread the state so that walls are active from the first step
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], (-w).astype(np.float32), x0.astype(np.float64), y0.astype(np.float64),
+                               steps_total=T, step_begin=begin, steps_run=8, dt=dt, a0=a0, c0=c0 if c0 > 0 else None, n_threads=2)
+    for path in (2, 3, 1, 4):
+        xg, yg = torch_mod.from_numpy(x0.copy()).cuda(), torch_mod.from_numpy(y0.copy()).cuda()
+        B.qhap_bsb_solve(dg, replicas=R, steps_total=T, step_begin=begin, steps_run=8, dt=dt, a0=a0, c0=c0, weight_mode=1, path=path,
+                         x=xg, y=yg, dense_J=J if path == 1 else None, tile_skip=1, finalize=False)
+        dx = np.abs(xg.cpu().numpy() - xo).max(); dy = np.abs(yg.cpu().numpy() - yo).max()
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (path, dx, dy)

@@ -827,11 +827,8 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
 
-  static bool attr_set = false;
-  if (!attr_set) {
-    QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
-    attr_set = true;
-  }
+  // per device and cheap: set on every call (a process may drive several devices)
+  QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
   QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));

@@ -120,11 +120,7 @@ qhap_status resident_solve_steps(const CsrView& g, const float* jval, int32_t R,
   QHAP_REQUIRE(RC >= 1 && kResThreads % RC == 0, "resident path: bad replica group");
   const size_t smem = resident_smem_bytes(g.n, g.nnz, RC);
   QHAP_REQUIRE(smem <= 200 * 1024, "resident path: problem does not fit in shared memory");
-  static size_t attr = 0;
-  if (smem > attr) {
-    QHAP_CUDA_TRY(cudaFuncSetAttribute(bsb_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    attr = 200 * 1024;
-  }
+  QHAP_CUDA_TRY(cudaFuncSetAttribute(bsb_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));   // per device
   ResidentArgs a;
   a.n = g.n; a.R = R; a.RC = RC; a.n_inst = n_inst; a.nnz = g.nnz;
   a.row_ptr = g.row_ptr; a.col = g.col; a.jval = jval; a.inst_ptr = inst_ptr_dev; a.c1 = c1;

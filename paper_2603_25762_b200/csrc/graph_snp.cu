@@ -263,11 +263,7 @@ void host_llr_table(double* T) {
 template <bool FILL>
 qhap_status launch_rows(int32_t n_snp, const uint8_t* flags, int32_t tenths, double alpha, const Compact& c, int32_t* row_ptr,
                         int32_t* col, int64_t* w_fx, float* w, cudaStream_t stream) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    QHAP_CUDA_TRY(cudaFuncSetAttribute(snp_rows_kernel<8192, 512, FILL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 12));
-    attr_set = true;
-  }
+  QHAP_CUDA_TRY(cudaFuncSetAttribute(snp_rows_kernel<8192, 512, FILL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 12));   // per device
   snp_rows_kernel<128, 64, FILL><<<n_snp, 64, 128 * 12, stream>>>(n_snp, 1, flags, tenths, alpha, c, row_ptr, col, w_fx, w);
   QHAP_LAUNCH_CHECK();
   snp_rows_kernel<1024, 256, FILL><<<n_snp, 256, 1024 * 12, stream>>>(n_snp, 2, flags, tenths, alpha, c, row_ptr, col, w_fx, w);

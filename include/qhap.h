@@ -97,6 +97,16 @@ QHAP_API qhap_status qhap_build_snp_graph(const qhap_frags *frags, int32_t linka
                                  const double *llr_table, qhap_csr *out, void *workspace, size_t *ws_bytes,
                                  void *stream);
 
+/* Second half of the capacity protocol without repeating the first: fills out->col / w_fx / w (capacity out->nnz)
+ * from what the preceding qhap_build_snp_graph call (count pass, out->col == NULL or capacity too small) left in
+ * `workspace` and in out->row_ptr.  The caller passes the SAME frags, linkage_tenths, alpha, workspace and
+ * out->row_ptr and must not have written to the workspace or to row_ptr in between; the fragment arrays are not read
+ * again.  Sizes, parameters and the row_ptr address are checked against a tag the count pass stored in the workspace
+ * (mismatch: QHAP_ERR_INVALID_ARG); capacity too small: QHAP_ERR_WORKSPACE.  The result is bit-identical to the one
+ * qhap_build_snp_graph itself writes when called with col != NULL. */
+QHAP_API qhap_status qhap_build_snp_graph_fill(const qhap_frags *frags, int32_t linkage_tenths, double alpha, qhap_csr *out,
+                                      void *workspace, size_t *ws_bytes, void *stream);
+
 /* bSB parameters (PAPER.md:L265 gives the outline; constants from BASELINE.json; readings R10a-f):
  *   a_k = a0 k / (steps_total - 1), k = step_begin .. step_begin + steps_run - 1
  *   F = J x (x of the previous step);  y += dt (-(a0 - a_k) x + c0 F);  x += dt a0 y;  |x| > 1: x = sign(x), y = 0. */

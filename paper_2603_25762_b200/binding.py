@@ -23,7 +23,7 @@ QHAP_OK, QHAP_ERR_INVALID_ARG, QHAP_ERR_RANGE, QHAP_ERR_WORKSPACE, QHAP_ERR_CUDA
 QHAP_WEIGHT_D, QHAP_WEIGHT_D_MINUS_C, QHAP_WEIGHT_FX = 0, 1, 2
 QHAP_DENSE_NONE, QHAP_DENSE_FP16, QHAP_DENSE_BF16 = 0, 1, 2
 
-EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_bsb_solve", "qhap_cut_eval",
+EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_build_snp_graph_fill", "qhap_bsb_solve", "qhap_cut_eval",
            "qhap_phase_readout_reads", "qhap_phase_readout_snps", "qhap_block_split", "qhap_block_stitch",
            "qhap_gauge_transform", "qhap_flip_count_update", "qhap_refine_readout", "qhap_snp_refine",
            "qhap_component_split", "qhap_component_merge",
@@ -48,7 +48,7 @@ class _BsbParams(C.Structure):
                 ("finalize", C.c_int32), ("dense_bn", C.c_int32)]
 
 
-for _name in EXPORTS[:14]:
+for _name in EXPORTS[:15]:
     getattr(_lib, _name).restype = C.c_int
 _lib.qhap_last_error.restype = C.c_char_p
 _lib.qhap_version.restype = C.c_char_p
@@ -212,32 +212,37 @@ def qhap_build_read_graph(frags: Frags, weight_mode: int = QHAP_WEIGHT_D, dense_
 
 
 def qhap_build_snp_graph(frags: Frags, linkage_tenths: int = 10, alpha: float = 0.1,
-                         llr_table: Optional[np.ndarray] = None) -> Csr:
-    """(2) SNP-graph build -> Csr with w_fx (int64, 2^-32) and w (fp32).  PAPER.md:L287-L319, L85, L350."""
+                         llr_table: Optional[np.ndarray] = None, resume: bool = True) -> Csr:
+    """(2) SNP-graph build -> Csr with w_fx (int64, 2^-32) and w (fp32).  PAPER.md:L287-L319, L85, L350.
+    Count call, allocation, then qhap_build_snp_graph_fill on the same workspace (`resume=False`: the fill call is
+    qhap_build_snp_graph again, which repeats the count pass)."""
     dev = _dev()
     g = Csr(frags.n_snp, 0, torch.empty(frags.n_snp + 1, dtype=torch.int32, device=dev))
     fs = frags.c_struct()
-    state = {"cs": g.c_struct()}
     tab = None
     if llr_table is not None:
         tab = np.ascontiguousarray(llr_table, dtype=np.float64)
         assert tab.size == 94 * 94
     tab_p = tab.ctypes.data_as(C.c_void_p) if tab is not None else None
+    args = (C.byref(fs), C.c_int32(linkage_tenths), C.c_double(alpha))
 
-    def call(ws, ws_bytes, cs):
-        cs = cs if cs is not None else state["cs"]
-        state["cs"] = cs
-        return _lib.qhap_build_snp_graph(C.byref(fs), C.c_int32(linkage_tenths), C.c_double(alpha), tab_p, C.byref(cs), ws,
-                                         ws_bytes, _stream())
-
-    def alloc():
-        nnz = state["cs"].nnz
-        g.col = torch.empty(max(nnz, 1), dtype=torch.int32, device=dev)
-        g.w_fx = torch.empty(max(nnz, 1), dtype=torch.int64, device=dev)
-        g.w = torch.empty(max(nnz, 1), dtype=torch.float32, device=dev)
-        return g.c_struct(capacity=max(nnz, 1))
-    _two_phase("qhap_build_snp_graph", call, alloc)
-    g.nnz = int(state["cs"].nnz)
+    ws_bytes = C.c_size_t(0)
+    cs = g.c_struct()
+    _check(_lib.qhap_build_snp_graph(*args, tab_p, C.byref(cs), None, C.byref(ws_bytes), _stream()), "qhap_build_snp_graph (size query)")
+    ws = _workspace(ws_bytes.value)
+    ws_bytes = C.c_size_t(ws.numel())
+    _check(_lib.qhap_build_snp_graph(*args, tab_p, C.byref(cs), _ptr(ws), C.byref(ws_bytes), _stream()), "qhap_build_snp_graph (count)")
+    nnz = int(cs.nnz)
+    g.col = torch.empty(max(nnz, 1), dtype=torch.int32, device=dev)
+    g.w_fx = torch.empty(max(nnz, 1), dtype=torch.int64, device=dev)
+    g.w = torch.empty(max(nnz, 1), dtype=torch.float32, device=dev)
+    cs = g.c_struct(capacity=max(nnz, 1))
+    ws_bytes = C.c_size_t(ws.numel())
+    if resume:
+        _check(_lib.qhap_build_snp_graph_fill(*args, C.byref(cs), _ptr(ws), C.byref(ws_bytes), _stream()), "qhap_build_snp_graph_fill")
+    else:
+        _check(_lib.qhap_build_snp_graph(*args, tab_p, C.byref(cs), _ptr(ws), C.byref(ws_bytes), _stream()), "qhap_build_snp_graph (fill)")
+    g.nnz = int(cs.nnz)
     g.col, g.w_fx, g.w = g.col[:g.nnz], g.w_fx[:g.nnz], g.w[:g.nnz]
     return g
 

@@ -129,6 +129,79 @@ def test_snp_graph_bit_exact(B, oracle, case, tenths):
     # the library's own table (C library pow/log10 on this box) gives the same bits
     g2 = B.qhap_build_snp_graph(B.upload_frags(fr), tenths, 0.1)
     assert_csr_equal(g2.to_host(), exp, ("w_fx", "w"))
+    # the fill call that repeats the count pass (no resume from the workspace) writes the same graph
+    g3 = B.qhap_build_snp_graph(B.upload_frags(fr), tenths, 0.1, llr_table=oracle.llr_table(), resume=False)
+    assert_csr_equal(g3.to_host(), exp, ("w_fx", "w"))
+
+
+def test_snp_graph_fill_rejects_foreign_workspace(B, torch_mod):
+    """qhap_build_snp_graph_fill checks the tag the count pass left in the workspace: a workspace that was not written by
+    the count pass for these arguments (zeroed here; other linkage depth) is refused, never read as row data."""
+    import ctypes as C
+    fr, _ = synth.make_config(3, scale=0.01)
+    d = B.upload_frags(fr)
+    fs = d.c_struct()
+    lib = B._lib
+    row_ptr = torch_mod.empty(fr.n_snp + 1, dtype=torch_mod.int32, device="cuda")
+    g = B.Csr(fr.n_snp, 0, row_ptr)
+    cs = g.c_struct()
+    nb = C.c_size_t(0)
+    assert lib.qhap_build_snp_graph(C.byref(fs), C.c_int32(3), C.c_double(0.1), None, C.byref(cs), None, C.byref(nb), None) == 0
+    ws = torch_mod.zeros(nb.value, dtype=torch_mod.uint8, device="cuda")
+    p = C.c_void_p(ws.data_ptr())
+    assert lib.qhap_build_snp_graph(C.byref(fs), C.c_int32(3), C.c_double(0.1), None, C.byref(cs), p, C.byref(nb), None) == 0
+    nnz = int(cs.nnz)
+    assert nnz > 0
+    g.col = torch_mod.empty(nnz, dtype=torch_mod.int32, device="cuda")
+    g.w_fx = torch_mod.empty(nnz, dtype=torch_mod.int64, device="cuda")
+    g.w = torch_mod.empty(nnz, dtype=torch_mod.float32, device="cuda")
+    cs = g.c_struct(capacity=nnz)
+    # other linkage depth than the count pass
+    assert lib.qhap_build_snp_graph_fill(C.byref(fs), C.c_int32(5), C.c_double(0.1), C.byref(cs), p, C.byref(nb), None) == B.QHAP_ERR_INVALID_ARG
+    # capacity one short
+    cs_small = g.c_struct(capacity=nnz - 1)
+    assert lib.qhap_build_snp_graph_fill(C.byref(fs), C.c_int32(3), C.c_double(0.1), C.byref(cs_small), p, C.byref(nb), None) == B.QHAP_ERR_WORKSPACE
+    # the matching call works, and a wiped workspace is refused afterwards
+    assert lib.qhap_build_snp_graph_fill(C.byref(fs), C.c_int32(3), C.c_double(0.1), C.byref(cs), p, C.byref(nb), None) == 0
+    ws.zero_()
+    assert lib.qhap_build_snp_graph_fill(C.byref(fs), C.c_int32(3), C.c_double(0.1), C.byref(cs), p, C.byref(nb), None) == B.QHAP_ERR_INVALID_ARG
+
+
+def fragments_from_lists(n_snp, lists, porec, seed):
+    """Fragments with the given (strictly ascending) SNP index lists; random alleles and qualities, 5 % missing."""
+    rng = np.random.default_rng(seed)
+    ptr = np.concatenate([[0], np.cumsum([len(l) for l in lists])]).astype(np.int64)
+    idx = np.concatenate(lists).astype(np.int32)
+    al = rng.integers(0, 2, len(idx)).astype(np.uint8)
+    al[rng.random(len(idx)) < 0.05] = 2
+    q = rng.integers(3, 41, len(idx)).astype(np.uint8)
+    nf = len(lists)
+    return synth.Fragments(nf, n_snp, ptr, idx, al, q, np.asarray(porec, np.uint8), rng.integers(0, 2, n_snp).astype(np.uint8),
+                           np.zeros(n_snp, np.uint8), np.zeros(nf, np.uint8), np.arange(n_snp, dtype=np.int64))
+
+
+def test_snp_graph_every_row_class(B, oracle):
+    """Rows of all six table classes of the row-gather build (direct / hash x 128 / 1024 / 8192 slots) in one graph:
+    short reads (direct 128), a 400-SNP and a 2,500-SNP read (direct 1024 / 8192), and SNPs shared by few, ~20 and ~60
+    scattered multi-contact fragments (hash 128 / 1024 / 8192).  Bit-exact against the oracle."""
+    n_snp = 60_000
+    rng = np.random.default_rng(9)
+    lists, porec = [], []
+    for s in range(0, 3_000, 7):                                  # short reads, windows <= 128
+        lists.append(np.arange(s, s + 20)); porec.append(0)
+    lists.append(np.arange(4_000, 4_400)); porec.append(0)        # window 400
+    lists.append(np.arange(5_000, 7_500)); porec.append(0)        # window 2,500
+    hubs = [(10_000, 3), (20_000, 20), (30_000, 60)]              # (hub SNP, number of scattered fragments through it)
+    for hub, m in hubs:
+        for _ in range(m):
+            others = rng.choice(np.arange(8_000, n_snp), size=30, replace=False)
+            lists.append(np.unique(np.concatenate([[hub], others]))); porec.append(1)
+    fr = fragments_from_lists(n_snp, lists, porec, seed=3)
+    exp = oracle.snp_graph(fr, 10, 0.1)
+    deg = np.diff(exp["row_ptr"])
+    assert deg[4_200] > 85 and deg[6_000] > 680 and 85 < deg[20_000] <= 680 and deg[30_000] > 680   # the classes are hit
+    g = B.qhap_build_snp_graph(B.upload_frags(fr), 10, 0.1, llr_table=oracle.llr_table())
+    assert_csr_equal(g.to_host(), exp, ("w_fx", "w"))
 
 
 def test_block_split_and_stitch_bit_exact(B, oracle, torch_mod):

@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--path", default="auto", choices=["auto", "dense", "dense-full", "sparse", "block"],
                     help="bSB step kernel: dense = tcgen05 tiles over the non-zero k-blocks of J (tile_skip, bit-identical to "
                          "dense-full = the whole N x N GEMM); sparse = CSR; auto = dense")
+    ap.add_argument("--step-launch", type=int, default=0, choices=[0, 1],
+                    help="tcgen05 paths: 0 = one launch runs all T steps where the tiles allow (tile-level dependencies between "
+                         "steps), 1 = one launch per step; same bits")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU seconds of the oracle sample")
     ap.add_argument("--refine-iters", type=int, default=0,
@@ -233,7 +236,7 @@ def run_ours(args):
             g0 = B.qhap_build_snp_graph(frags, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
             g = B.qhap_block_split(g0, win_mine) if win is not None else g0
             res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, cut_per_replica=False,
-                                   workspace=state.get("ws"))
+                                   step_launch=args.step_launch, workspace=state.get("ws"))
             state["ws"] = res["workspace"]
             cut, spins = res["best_cut"], res["best_spins"]
             if win is not None:
@@ -244,7 +247,7 @@ def run_ours(args):
             state["g"] = g
             return cut, hap
         g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype)
-        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip,
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip, step_launch=args.step_launch,
                                cut_per_replica=False, workspace=state.get("ws"))
         state["ws"] = res["workspace"]
         cut, spins = res["best_cut"], res["best_spins"]
@@ -337,7 +340,7 @@ def run_ours(args):
             gg, JJ = B.qhap_build_read_graph(dfr, weight_mode=mode, dense_dtype=dense_dtype)
             g0 = gg
         ev[1].record()
-        res = B.qhap_bsb_solve(gg, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=JJ, tile_skip=tile_skip,
+        res = B.qhap_bsb_solve(gg, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=JJ, tile_skip=tile_skip, step_launch=args.step_launch,
                                cut_per_replica=False, workspace=state.get("ws"))
         ev[2].record()
         sp = res["best_spins"]
@@ -391,7 +394,7 @@ def run_ours(args):
         res0 = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=0, seed=seed, weight_mode=mode, path=2, finalize=False)
         x, y = res0["x"], res0["y"]
         kw = dict(replicas=R, steps_total=T, weight_mode=mode, path=path_, x=x, y=y, dense_J=J if path_ == 1 else None, finalize=False,
-                  tile_skip=skip_)
+                  tile_skip=skip_, step_launch=args.step_launch)
         r = B.qhap_bsb_solve(g, step_begin=0, steps_run=min(20, steps_), **kw)          # warm-up (also sizes the workspace)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
@@ -462,6 +465,16 @@ def run_ours(args):
             extra["roofline_dense_full"]["spin_updates_per_s"] = n * R / (full_ms * 1e-3)
     else:
         roofline = tensor_roofline(step_ms)
+    # fused launch: one launch ran all T steps; the per-launch figures are T x the per-step ones
+    spl = T if (path in (1, 4) and step_launches < T) else 1
+    roofline["steps_per_launch"] = spl
+    roofline["step_ms"] = step_ms
+    if spl > 1:
+        for kb_ in ("bytes_per_launch", "flops_per_launch"):
+            if kb_ in roofline:
+                roofline[kb_.replace("launch", "step")] = roofline[kb_]
+                roofline[kb_] = roofline[kb_] * spl
+        roofline["launch_ms"] = step_ms * spl
     prof = ROOT / "profiles" / "roofline_traffic.csv"      # dram bytes per launch from the committed ncu captures (kernel, config)
     if prof.exists():
         for line in prof.read_text().splitlines()[1:]:
@@ -469,7 +482,7 @@ def run_ours(args):
             if len(f) >= 3 and f[1] == str(args.config):
                 for rl in [roofline] + [v for k, v in extra.items() if k.startswith("roofline") and isinstance(v, dict)]:
                     if rl["kernel"] == f[0]:
-                        rl["traffic"] = float(f[2])
+                        rl["traffic"] = float(f[2]) * rl.get("steps_per_launch", 1)      # the CSV holds bytes per bSB step
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if blocks else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",

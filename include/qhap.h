@@ -133,6 +133,9 @@ typedef struct {
   int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
   int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */
   int32_t dense_bn;     /* path 1: tile width in output spins (multiple of 16 in 32..256); 0 = automatic      */
+  int32_t step_launch;  /* paths 1, 4: 0 = automatic (ONE launch runs all steps_run steps when the tiles allow:    */
+                        /*    tiles of step k+1 start as soon as the tiles they read have finished step k);       */
+                        /*    1 = one launch per step.  Same bits either way                                      */
 } qhap_bsb_params;
 
 /* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`

@@ -12,8 +12,8 @@
 // Jacobi update across CTAs: the fp16 copies are double-buffered (read buffer b, write buffer 1-b); fp32 x, y are
 // private to the tile that owns them and are updated in place.  One launch per step (grid-wide step boundary).
 //
-// Warp roles (576 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one elected lane),
-// warps 2..17 = epilogue (TMEM lane quarter = warp % 4, four warps per quarter interleave 8-column chunks; the state of
+// Warp roles (608 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one elected lane), warp 18 =
+// TMA stores of the fp16 copies, warps 2..17 = epilogue (TMEM lane quarter = warp % 4, four warps per quarter interleave 8-column chunks; the state of
 // the next chunk is prefetched into registers; at BN = 64 the fp16 copies leave through shared memory and TMA stores).
 // Pipelines: n_stages shared-memory stages (full/empty mbarriers) and 2 TMEM accumulator stages (tmem_full/tmem_empty).
 #include <cuda.h>
@@ -37,7 +37,8 @@ constexpr int kStageX = kBM * kBK * 2;               // 16 KB each for x_hi, x_l
 constexpr int kSmemBudget = 224 * 1024;              // operand stages (+ fp16 staging + state ring); + 1 KB slack + 1 KB barriers <= 227 KB
 constexpr int kEpiWarps = 16;
 constexpr int kChunk = 8;                // accumulator columns (spins) per tcgen05.ld in the epilogue
-constexpr int kThreads = 64 + 32 * kEpiWarps;
+constexpr int kStoreWarp = 2 + kEpiWarps;  // one lane: TMA stores of the fp16 copies (+ the fused steps' progress signal)
+constexpr int kThreads = 32 * (kStoreWarp + 1);
 constexpr int kRingSlot = kChunk * 32 * 4;           // one work item of x (or y): 8 spins x 32 replicas fp32 = 1 KB
 constexpr int kRingBytes = kEpiWarps * 2 * 2 * kRingSlot;   // per warp: 2 slots x (x, y)
 constexpr int kTmemCols = 512;                       // 2 accumulator stages x 256 columns
@@ -62,7 +63,24 @@ struct DenseArgs {
   float* y;
   __half* xh_out;             // [R][n_k] next step's split copies
   __half* xl_out;
+  // Fused steps: one launch runs n_steps bSB steps.  Virtual tile vt = s tile_stride + tile (step s of this launch); the
+  // operand loads of tile (tn, tm) at step s wait until every tile (kb, tm), kb in tn's k-block list, has finished step
+  // s - 1 (`done` counts the steps each tile has completed in this launch).  Needs BN == kBK (k-block == tile row),
+  // k-block lists, TMA-stored copies and at least two tiles per CTA and step (state prefetch distance).
+  int32_t n_steps;            // steps run by this launch (1 unless fused)
+  int32_t fused;
+  int32_t tile_stride;        // n_tiles rounded up to a multiple of the grid
+  int32_t k0, steps_total;    // ramp (R10b): step index of s = 0, T
+  double dt, a0;
+  uint32_t* done;             // [n_tiles_n * n_tiles_m], zero at launch
+  uint32_t fence_every;       // state ring: generic -> async proxy fence after every fence_every-th tile of a CTA
 };
+
+// c2 = fp32(dt (a0 - a_k)), a_k = a0 k / (T - 1): the same individually rounded fp64 operations as the host loop
+__device__ __forceinline__ float ramp_c2(const DenseArgs& a, int s) {
+  const double a_k = a.steps_total > 1 ? __ddiv_rn(__dmul_rn(a.a0, double(a.k0 + s)), double(a.steps_total - 1)) : 0.0;
+  return __double2float_rn(__dmul_rn(a.dt, __dsub_rn(a.a0, a_k)));
+}
 
 // fp32 -> two fp16 terms of xs = 2^15 x (|x| <= 1 -> |xs| <= 32768, inside fp16's range): hi = rn(xs), lo = rn(xs - hi)
 // (the difference is exact in fp32).  The scale keeps lo a NORMAL fp16 number for every |x| >= 2^-17, so that
@@ -196,12 +214,16 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 2 + s); };
   const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStages + 4);
   auto ring_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 6 + s); };
+  auto stg_full = [&](uint32_t b) { return bar_base + 8u * (2 * kMaxStages + 6 + 2 * kEpiWarps + b); };       // staging tile b written
+  auto stg_empty = [&](uint32_t b) { return bar_base + 8u * (2 * kMaxStages + 8 + 2 * kEpiWarps + b); };      // ... read by its TMA store
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && ptx::elect_one()) {
     ptx::prefetch_tensormap(&tm_j);
     ptx::prefetch_tensormap(&tm_xh);
     ptx::prefetch_tensormap(&tm_xl);
+    ptx::prefetch_tensormap(&tm_oh);
+    ptx::prefetch_tensormap(&tm_ol);
     for (int s = 0; s < kStages; ++s) {
       ptx::mbar_init(full_bar(s), 1);
       ptx::mbar_init(empty_bar(s), 1);
@@ -211,6 +233,10 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       ptx::mbar_init(tempty_bar(s), kEpiWarps);
     }
     for (int s = 0; s < 2 * kEpiWarps; ++s) ptx::mbar_init(ring_bar(s), 1);
+    for (uint32_t b = 0; b < 2; ++b) {
+      ptx::mbar_init(stg_full(b), kEpiWarps);
+      ptx::mbar_init(stg_empty(b), 1);
+    }
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc(tmem_slot, kTmemCols);
@@ -227,16 +253,30 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   const int n_tiles = a.n_tiles_m * a.n_tiles_n;
+  const int stride = a.tile_stride, vt_end = a.n_steps * a.tile_stride;   // virtual tiles: step-major, holes in [n_tiles, stride)
   const uint32_t stage_tx = kStageJ + 2u * kStageX;
 
   if (warp == 0) {
     // ===================================================================================== TMA producer
-    if (ptx::elect_one()) {
+    // Lane 0 issues the loads.  Fused steps: before a tile of step s > 0 the WHOLE warp polls the progress counters of
+    // the tiles it reads (one k-block per lane, so the L2 round trips overlap), then lane 0 crosses to the async proxy.
+    if (lane == 0 || a.fused) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
+        const int s = vt / stride, tile = vt - s * stride;
+        if (tile >= n_tiles) continue;
         const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;      // M fastest: neighbouring CTAs share the J tile in L2
         const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
+        if (s > 0) {
+          for (int j = lane; j < nkb; j += 32)                           // tile (kb, tm) has finished step s - 1
+            ptx::wait_at_least_acquire(a.done + a.kb_idx[size_t(tn) * a.n_kblocks + j] * a.n_tiles_m + tm, uint32_t(s));
+          __syncwarp();
+          ptx::fence_proxy_async_global();
+        }
+        if (lane != 0) continue;
+        const CUtensorMap* mh = (s & 1) ? &tm_oh : &tm_xh;               // odd steps of a fused launch read what even steps wrote
+        const CUtensorMap* ml = (s & 1) ? &tm_ol : &tm_xl;
         for (int j = 0; j < nkb; ++j) {
           const int kb = a.kb_cnt ? a.kb_idx[size_t(tn) * a.n_kblocks + j] : j;
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
@@ -249,8 +289,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           } else {
             ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
           }
-          ptx::tma_load_2d(sj + kStageJ, &tm_xh, full_bar(stage), kb * kBK, tm * kBM);
-          ptx::tma_load_2d(sj + kStageJ + kStageX, &tm_xl, full_bar(stage), kb * kBK, tm * kBM);
+          ptx::tma_load_2d(sj + kStageJ, mh, full_bar(stage), kb * kBK, tm * kBM);
+          ptx::tma_load_2d(sj + kStageJ + kStageX, ml, full_bar(stage), kb * kBK, tm * kBM);
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
@@ -262,7 +302,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     uint32_t phase = 0;
     int acc = 0;
     uint32_t acc_phase = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
+      const int tile = vt % stride;
+      if (tile >= n_tiles) continue;
       const int tn = tile / a.n_tiles_m;
       const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
       ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);                    // epilogue has drained this accumulator stage
@@ -301,6 +343,32 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       }
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
+  } else if (warp == kStoreWarp) {
+    // ==================================================================================== fp16 copy stores
+    // One thread hands each finished pair of staging tiles to TMA, returns the buffer once the bulk reads are done and --
+    // fused steps -- signals the tile's completion (done[tile] += 1) once the writes have COMPLETED.  Off the epilogue's
+    // critical path: the epilogue warps only arrive on / wait for the two staging barriers.
+    if (a.stage_out && lane == 0) {
+      const uint32_t stg_base = smem_base + uint32_t(kStages) * kStageBytes;
+      uint32_t tc = 0;
+      for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
+        const int s = vt / stride, tile = vt - s * stride;
+        if (tile >= n_tiles) continue;
+        const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+        const uint32_t b = tc & 1u, stg = stg_base + b * (2u * kStageX);
+        ptx::mbar_wait(stg_full(b), (tc >> 1) & 1u);
+        ptx::tma_store_2d((s & 1) ? &tm_xh : &tm_oh, stg, tn * a.BN, tm * kBM);
+        ptx::tma_store_2d((s & 1) ? &tm_xl : &tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+        ptx::tma_store_commit();
+        ptx::tma_store_wait_read_all();
+        ptx::mbar_arrive(stg_empty(b));
+        if (a.fused) {
+          ptx::tma_store_wait_all();
+          ptx::signal_add_release(a.done + tile, 1u);
+        }
+        ++tc;
+      }
+    }
   } else {
     // ========================================================================================= epilogue
     // Work item = (tile, 16-column chunk).  The fp32 state of item k+1 is loaded into registers before item k is
@@ -319,49 +387,63 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     // fp16 output staging: two buffers of (x_hi tile, x_lo tile) behind the operand stages, alternated per tile
     const uint32_t stg_base = smem_base + uint32_t(kStages) * kStageBytes;
     uint32_t tcount = 0;
-    // every warp owns chunk `par` of every tile (possibly fully masked), so that it arrives on tmem_empty once per tile
-    auto advance = [&](int& tile, int& ch) {
+    int cur_s = 0;                             // step (of this launch) whose ramp constant ec.c2 holds
+    if (a.fused) ec.c2 = ramp_c2(a, 0);
+    // every warp owns chunk `par` of every tile (possibly fully masked), so that it arrives on tmem_empty once per tile.
+    // Items are addressed by the VIRTUAL tile (step-major); the last wave of a step may have a hole for this CTA.
+    auto advance = [&](int& vt, int& ch) {
       ch += P;
-      if (ch * kChunk >= a.BN || (tile / a.n_tiles_m) * a.BN + ch * kChunk >= a.n) { tile += gridDim.x; ch = par; }
+      if (ch * kChunk >= a.BN || ((vt % stride) / a.n_tiles_m) * a.BN + ch * kChunk >= a.n) {
+        vt += gridDim.x;
+        if (vt % stride >= n_tiles) vt += gridDim.x;      // hole -> first wave of the next step (stride % grid == 0)
+        ch = par;
+      }
     };
-    // last chunk of this warp in a tile: hand the accumulator stage back; with fp16 staging, all epilogue warps have then
-    // written their pieces of the tile -> one thread hands the two staging tiles to TMA.  The elected thread first waits
-    // until the previous tile's stores have finished reading their buffer, so that after the barrier every warp may
-    // overwrite that buffer (it is the next tile's).
-    auto tile_done = [&](int tile, uint32_t stg) {
+    auto set_step = [&](int vt) {
+      if (a.fused) {
+        const int s = vt / stride;
+        if (s != cur_s) { cur_s = s; ec.c2 = ramp_c2(a, s); }
+      }
+    };
+    // last chunk of this warp in a tile: hand the accumulator stage back and arrive on the staging tile's barrier (the
+    // store warp takes it from there).  Fused steps: the fp32 state was written with generic stores and is re-read
+    // through TMA one step later by the same warp (requested while the warp works on the tile BEFORE it in the CTA's
+    // order), so every lane crosses to the async proxy in between: after every fence_every-th tile, with
+    // fence_every <= (fewest tiles a CTA has per step) - 1, the fence that follows a tile's stores comes at most
+    // fence_every - 1 tiles later, the request at least (tiles per step) - 1 tiles later.
+    auto tile_done = [&]() {
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
       if (a.stage_out) {
         ptx::fence_proxy_async();
-        if (ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
-        ptx::named_barrier_sync(1, kEpiWarps * 32);
-        if (ew == 0 && lane == 0) {
-          const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
-          ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
-          ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
-          ptx::tma_store_commit();
-        }
+        if (a.fused && a.ring && (tcount + 1u) % a.fence_every == 0u) ptx::fence_proxy_async_global();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(stg_full(tcount & 1u));
         ++tcount;
       }
     };
+    // first chunk of a tile: the accumulator must be complete and the staging buffer free (its previous store has read it)
+    auto tile_begin = [&]() {
+      ptx::mbar_wait(tfull_bar(acc), acc_phase);
+      ptx::tc_fence_after();
+      if (a.stage_out) ptx::mbar_wait(stg_empty(tcount & 1u), ((tcount >> 1) & 1u) ^ 1u);
+    };
     auto step = [&](int& tile, int& ch, const float (&xc)[kChunk], const float (&yc)[kChunk], float (&xn)[kChunk],
                     float (&yn)[kChunk]) -> bool {
-      if (ch == par) {                         // first chunk of a tile: the accumulator must be complete
-        ptx::mbar_wait(tfull_bar(acc), acc_phase);
-        ptx::tc_fence_after();
-      }
+      if (ch == par) tile_begin();
       uint32_t v[kChunk];
       ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
       int ntile = tile, nch = ch;
       advance(ntile, nch);
-      const bool nhave = ntile < n_tiles;
-      if (nhave) epi_load(a, ec, ntile, nch, xn, yn);
+      const bool nhave = ntile < vt_end;
+      if (nhave) epi_load(a, ec, ntile % stride, nch, xn, yn);
       ptx::tmem_ld_wait();
       const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
-      epi_update_store(a, ec, tile, ch, v, xc, yc, stg);
-      if (ntile != tile) tile_done(tile, stg);
+      set_step(tile);
+      epi_update_store(a, ec, tile % stride, ch, v, xc, yc, stg);
+      if (ntile != tile) tile_done();
       tile = ntile; ch = nch;
       return nhave;
     };
@@ -371,8 +453,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       // need no registers, no address arithmetic and no LSU slots; out-of-range rows / replicas arrive as zeros.
       const uint32_t ring_w = stg_base + 4u * kStageX + uint32_t(ew) * (4u * kRingSlot);
       const uint32_t rbar0 = ring_bar(2 * ew);
-      auto issue = [&](int tile, int ch, int slot) {
+      auto issue = [&](int vt, int ch, int slot) {
         if (ptx::elect_one()) {
+          const int tile = vt % stride;
           const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
           const uint32_t dst = ring_w + uint32_t(slot) * (2u * kRingSlot);
           ptx::mbar_arrive_expect_tx(rbar0 + 8u * slot, 2u * kRingSlot);
@@ -382,19 +465,16 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         __syncwarp();
       };
       int t0 = blockIdx.x, c0 = par, t1 = t0, c1i = c0, t2, c2i;
-      if (t0 < n_tiles) {
+      if (t0 < vt_end) {
         issue(t0, c0, 0);
         advance(t1, c1i);
-        if (t1 < n_tiles) issue(t1, c1i, 1);
+        if (t1 < vt_end) issue(t1, c1i, 1);
         t2 = t1; c2i = c1i;
-        if (t1 < n_tiles) advance(t2, c2i);
+        if (t1 < vt_end) advance(t2, c2i);
       }
-      for (uint32_t k = 0; t0 < n_tiles; ++k) {
+      for (uint32_t k = 0; t0 < vt_end; ++k) {
         const int slot = int(k & 1u);
-        if (c0 == par) {                         // first chunk of a tile: the accumulator must be complete
-          ptx::mbar_wait(tfull_bar(acc), acc_phase);
-          ptx::tc_fence_after();
-        }
+        if (c0 == par) tile_begin();
         uint32_t v[kChunk];
         ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + c0 * kChunk), v);
         ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
@@ -406,25 +486,24 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
         }
         __syncwarp();                            // every lane has its values: the slot may be refilled
-        if (t1 < n_tiles && t2 < n_tiles) issue(t2, c2i, slot);
+        if (t1 < vt_end && t2 < vt_end) issue(t2, c2i, slot);
         ptx::tmem_ld_wait();
         const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
-        epi_update_store(a, ec, t0, c0, v, xv, yv, stg);
-        if (t1 != t0) tile_done(t0, stg);
+        set_step(t0);
+        epi_update_store(a, ec, t0 % stride, c0, v, xv, yv, stg);
+        if (t1 != t0) tile_done();
         t0 = t1; c0 = c1i; t1 = t2; c1i = c2i;
-        if (t2 < n_tiles) advance(t2, c2i);
+        if (t2 < vt_end) advance(t2, c2i);
       }
-      if (a.stage_out && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
     } else {
-    int tile = blockIdx.x, ch = par;
-    if (tile < n_tiles) {
+    int tile = blockIdx.x, ch = par;           // virtual tile
+    if (tile < vt_end) {
       float xa[kChunk], ya[kChunk], xb[kChunk], yb[kChunk];
-      epi_load(a, ec, tile, ch, xa, ya);
+      epi_load(a, ec, tile % stride, ch, xa, ya);
       while (true) {
         if (!step(tile, ch, xa, ya, xb, yb)) break;
         if (!step(tile, ch, xb, yb, xa, ya)) break;
       }
-      if (a.stage_out && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();   // smem must outlive the bulk reads
     }
     }
   }
@@ -466,7 +545,12 @@ __global__ void __launch_bounds__(256) kb_flag_kernel(int32_t n, const int32_t* 
   if (a >= n) return;
   const int lane = threadIdx.x & 31;
   int32_t* f = flag + size_t(a / BN) * n_kblocks;
-  for (int32_t e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) f[col[e] / kBK] = 1;
+  for (int32_t e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
+    f[col[e] / kBK] = 1;
+    // tile rows == k-blocks: keep the lists symmetric even if the CSR is not (the fused steps' write-after-read
+    // ordering on the fp16 copies relies on "tn lists kb  <=>  kb lists tn"; an extra zero tile is harmless)
+    if (BN == kBK) flag[size_t(col[e] / kBK) * n_kblocks + a / kBK] = 1;
+  }
 }
 
 // One CTA per N tile: ascending list of flagged k-blocks (at least one entry, so that every tile produces an accumulator).
@@ -690,6 +774,47 @@ qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, co
   return QHAP_OK;
 }
 
+// Fused launches need: TMA-stored copies and tile rows == k-blocks (BN == kBK), k-block lists, and at least two tiles per
+// CTA and step (the epilogue requests the state of the item two ahead before it stores the current one): the grid is
+// at most half the tile count.  All CTAs of the grid must be co-resident (one per SM, grid <= SM count).
+// Grid of a fused launch, or 0 = one launch per step.  Worth it while a CTA has few tiles per step (launch gap, pipeline
+// fill and drain per step: cfg1 40.0 -> 38.2 us, cfg2 45.2 -> 41.4 us per step, a 304-tile problem 33.9 -> 14.5 us); with
+// ~50 tiles per CTA and step (cfg3) the step boundary is amortised and the lock-step launches keep the L2 reuse between
+// neighbouring CTAs (268 us per step against 274 fused), so those stay on one launch per step.
+int fused_grid(const DenseArgs& a, const qhap_bsb_params& p) {
+  const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;
+  const int64_t grid = std::min<int64_t>(sm_count(), n_tiles / 2);
+  if (p.step_launch != 0 || !a.stage_out || a.BN != kBK || a.kb_cnt == nullptr || p.steps_run < 2 || grid < 1) return 0;
+  if (ceil_div(n_tiles, grid) > 16) return 0;
+  return int(grid);
+}
+
+// All steps of the call in as few launches as the 32-bit virtual tile index allows (one, at every BASELINE size).
+// tm_h / tm_l: the two buffers of split copies; buffer `cur` holds the current x.  Returns the buffer that holds x after.
+qhap_status launch_fused(int grid, cudaStream_t stream, const CUtensorMap& tj, const CUtensorMap& tjl, const CUtensorMap (&tm_h)[2],
+                         const CUtensorMap (&tm_l)[2], const CUtensorMap& tsx, const CUtensorMap& tsy, DenseArgs a,
+                         const qhap_bsb_params& p, uint32_t* done, int& cur) {
+  const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;
+  a.fused = 1;
+  a.tile_stride = int32_t(ceil_div(n_tiles, grid) * grid);
+  a.fence_every = uint32_t(std::max<int64_t>(1, n_tiles / grid - 1));
+  a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0;
+  a.c3 = float(p.dt * p.a0);
+  a.c2 = 0.f;
+  a.done = done;
+  a.xh_out = nullptr; a.xl_out = nullptr;          // fused launches store through the tensor maps only (stage_out)
+  const int32_t max_steps = int32_t(std::max<int64_t>(1, (int64_t(1) << 30) / a.tile_stride));
+  for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run;) {
+    a.n_steps = std::min(max_steps, p.step_begin + p.steps_run - k);
+    a.k0 = k;
+    QHAP_CUDA_TRY(cudaMemsetAsync(done, 0, sizeof(uint32_t) * size_t(n_tiles), stream));
+    QHAP_TRY(launch_step(grid, stream, tj, tjl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tsx, tsy, a));
+    cur ^= (a.n_steps & 1);
+    k += a.n_steps;
+  }
+  return QHAP_OK;
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -787,6 +912,7 @@ size_t dense_workspace_bytes(int32_t n, int32_t ld, int32_t R) {
   ws.take<int32_t>(n_tn_max);             // kb_cnt
   ws.take<int32_t>(n_tn_max * n_kb);      // kb_idx
   ws.take<int32_t>(n_tn_max * n_kb);      // flags
+  ws.take<uint32_t>(n_tn_max * size_t(ceil_div(R, kBM)));   // done (fused steps)
   return ws.used();
 }
 
@@ -809,6 +935,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   int32_t* kb_cnt = ws.take<int32_t>(n_tn_max);
   int32_t* kb_idx = ws.take<int32_t>(n_tn_max * n_kb);
   int32_t* flags = ws.take<int32_t>(n_tn_max * n_kb);
+  uint32_t* done = ws.take<uint32_t>(n_tn_max * size_t(ceil_div(R, kBM)));
 
   const bool skip = p.tile_skip != 0;
   const int32_t BN = choose_bn(n, R, skip, p.dense_bn);
@@ -826,6 +953,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.kb_idx = skip ? kb_idx : nullptr;
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
+  a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   // per device and cheap: set on every call (a process may drive several devices)
   QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
@@ -853,7 +981,9 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   }
 
   const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
+  a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
   int cur = 0;
+  if (const int gf = fused_grid(a, p)) return launch_fused(gf, stream, tm_j, tm_j, tm_h, tm_l, tm_sx, tm_sy, a, p, done, cur);
   for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
     const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
     a.c2 = float(p.dt * (p.a0 - a_k));
@@ -897,6 +1027,7 @@ size_t block_workspace_bytes(int32_t n, int64_t nnz, int32_t R) {
   ws.take<float>(size_t(nnz));            // rem_val
   ws.take<uint32_t>(4);                   // absmax, scale
   ws.take<int64_t>(2);                    // total blocks, overflow
+  ws.take<uint32_t>(n_t * size_t(ceil_div(R, kBM)));   // done (fused steps)
   const size_t cap = size_t(block_capacity(n, nnz)) * kBK * kBK;
   ws.take<__half>(cap); ws.take<__half>(cap);
   return ws.used();
@@ -927,6 +1058,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   float* rem_val = ws.take<float>(size_t(g.nnz));
   uint32_t* scal = ws.take<uint32_t>(4);
   int64_t* totals = ws.take<int64_t>(2);
+  uint32_t* done = ws.take<uint32_t>(size_t(n_t) * size_t(ceil_div(R, kBM)));
   const int64_t cap_blocks = block_capacity(n, g.nnz);
   const size_t cap = size_t(cap_blocks) * kBK * kBK;
   __half* jh = ws.take<__half>(cap);
@@ -997,6 +1129,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
   a.c1 = c1row; a.c1_per_row = 1;
   a.x = x; a.y = y;
+  a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
   QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
 
   CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2], tm_sx, tm_sy;
@@ -1015,7 +1148,11 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
     QHAP_LAUNCH_CHECK();
   }
   const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
+  a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
   int cur = 0;
+  // the remainder gather reads the fp32 x of the whole graph between two tile steps: a grid-wide step boundary
+  if (const int gf = has_rem ? 0 : fused_grid(a, p))
+    return launch_fused(gf, stream, tm_jh, tm_jl, tm_h, tm_l, tm_sx, tm_sy, a, p, done, cur);
   for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
     const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
     a.c2 = float(p.dt * (p.a0 - a_k));

@@ -65,6 +65,27 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, uint32_t src,
 __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // all bulk groups of this thread have finished READING their shared-memory source
 __device__ __forceinline__ void tma_store_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// all committed bulk stores of this thread have completed AND their writes are visible to this thread
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// orders this thread's generic-proxy accesses to global memory against its async-proxy (TMA) accesses, both ways
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
+// Cross-CTA progress counters (fused steps): the writer's TMA stores are complete (tma_store_wait_all) before the release;
+// the reader acquires, then crosses to the async proxy before its TMA loads.  A wait that outlasts ~seconds traps (a lost
+// dependency must surface as a CUDA error, never as a hung device).
+__device__ __forceinline__ void signal_add_release(uint32_t* p, uint32_t v) {
+  fence_proxy_async_global();
+  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void wait_at_least_acquire(const uint32_t* p, uint32_t want) {
+  uint32_t v, spins = 0;
+  while (true) {
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    if (v >= want) break;
+    if (++spins > (1u << 22)) __trap();
+    __nanosleep(32);
+  }
+  fence_proxy_async_global();
+}
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }

@@ -493,6 +493,62 @@ def test_dense_solve_quality_cfg0(B, oracle, torch_mod):
         assert gse <= ose + 0.001
 
 
+# ------------------------------------------- fused launch: all steps in one launch, tiles of step k+1 wait for step-k tiles
+@pytest.mark.parametrize("case", ["read-2wave", "read-fullgrid", "read-porec", "snp-batched"])
+def test_fused_steps_equal_per_step_launches(B, oracle, torch_mod, case):
+    """step_launch = 0 (one launch runs all steps; a tile of step k+1 starts once the tiles it reads have finished step k)
+    against step_launch = 1 (one launch per step, grid-wide step boundary): same bits after odd and even step counts and
+    across a resume; and directly against the fp64 oracle over the first 10 steps (north_star bar).  Cases: a ragged
+    replica tile, a problem that fills all 148 CTAs, a non-banded read graph (Pore-C fragments: tiles depend on tiles far
+    away in launch order), a batch of SNP blocks (J_hi + J_lo, per-row c1)."""
+    inst_ptr = None
+    if case == "snp-batched":
+        fr, p = synth.make_config(3, scale=0.02)
+        g = oracle.block_split(oracle.snp_graph(fr, 3, 0.1), synth.block_windows(fr.n_snp, 1000, 900))
+        inst_ptr, mode, R, paths, wj = g["inst_ptr"], 2, 300, ((4, 0),), g["w"]
+        dg, J, T = B.upload_csr(g), None, p["T"]
+    else:
+        if case == "read-porec":
+            fr, T, R = porec_like(seed=23, n_snp=900, n_reads=700), 500, 300
+        else:
+            fr, pp = synth.make_config(1, scale=0.1 if case == "read-2wave" else 0.3)
+            T, R = pp["T"], (300 if case == "read-2wave" else 1024)
+        g = oracle.read_graph(fr)
+        mode, paths = 1, ((1, 1), (4, 0))
+        wj = oracle.read_weights(g, 1)
+        dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+        assert_csr_equal(dg.to_host(), g, ("d", "c"))
+    n = g["n"]
+    x0, y0 = synth.bsb_init_state(7, n, R)
+    for path, skip in paths:
+        kw = dict(replicas=R, steps_total=T, weight_mode=mode, path=path, dense_J=J if path == 1 else None, tile_skip=skip,
+                  dense_bn=64 if path == 1 else 0, finalize=False)
+        st = {}
+        for sl in (0, 1):
+            xg = torch_mod.from_numpy(x0.copy()).cuda(); yg = torch_mod.from_numpy(y0.copy()).cuda()
+            B.qhap_bsb_solve(dg, step_begin=0, steps_run=10, x=xg, y=yg, step_launch=sl, **kw)
+            first = (xg.cpu().numpy(), yg.cpu().numpy())
+            B.qhap_bsb_solve(dg, step_begin=10, steps_run=7, x=xg, y=yg, step_launch=sl, **kw)     # odd count: buffers end swapped
+            B.qhap_bsb_solve(dg, step_begin=17, steps_run=24, x=xg, y=yg, step_launch=sl, **kw)
+            st[sl] = (first, xg.cpu().numpy(), yg.cpu().numpy())
+        assert np.array_equal(st[0][1], st[1][1]) and np.array_equal(st[0][2], st[1][2]), (case, path)
+        assert np.array_equal(st[0][0][0], st[1][0][0]) and np.array_equal(st[0][0][1], st[1][0][1]), (case, path)
+        # the fused launch against the oracle, 10 free-running steps from the same fp32 state (replica subset for the big case)
+        rs = slice(0, min(R, 136))
+        jv = (-wj).astype(np.float32)
+        xo, yo = x0[:, rs].astype(np.float64), y0[:, rs].astype(np.float64)
+        bounds = [(0, n)] if inst_ptr is None else [(int(inst_ptr[b]), int(inst_ptr[b + 1])) for b in range(len(inst_ptr) - 1)]
+        for lo, hi in bounds:
+            rp = (g["row_ptr"][lo:hi + 1] - g["row_ptr"][lo]).astype(np.int32)
+            e = slice(int(g["row_ptr"][lo]), int(g["row_ptr"][hi]))
+            xs, ys = xo[lo:hi].copy(), yo[lo:hi].copy()
+            oracle.bsb_run(rp, (g["col"][e] - lo).astype(np.int32), jv[e], xs, ys, steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+            xo[lo:hi], yo[lo:hi] = xs, ys
+        dx = np.abs(st[0][0][0][:, rs] - xo).max(); dy = np.abs(st[0][0][1][:, rs] - yo).max()
+        print(f"fused {case} path {path}: n {n} R {R}, 10 steps against the oracle max|dx| {dx:.2e} max|dy| {dy:.2e}")
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (case, path, dx, dy)
+
+
 # ------------------------------------------------------- (3') tcgen05 step on a block-compressed J built from the CSR
 def test_block_path_read_graph_equals_dense_tile_skip(B, oracle, torch_mod):
     """Integer read graph: path 4 stores only the non-empty 64 x 64 tiles of J; same MMAs in the same order as the

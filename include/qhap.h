@@ -136,6 +136,10 @@ typedef struct {
   int32_t step_launch;  /* paths 1, 4: 0 = automatic (ONE launch runs all steps_run steps when the tiles allow:    */
                         /*    tiles of step k+1 start as soon as the tiles they read have finished step k);       */
                         /*    1 = one launch per step.  Same bits either way                                      */
+  int32_t l2_hints;     /* paths 1, 4: L2 eviction priorities of the step kernel: 0 = automatic (x and its fp16     */
+                        /*    copies evict_last, y evict_first when 12 B x n x R fits the L2), 1 = on, 2 = off        */
+  int32_t dense_stg_bufs; /* paths 1, 4 (tuning): shared-memory staging buffers for the fp16 copies: 0 = automatic, 1, 2 */
+  int32_t dense_epi_sync; /* paths 1, 4 (tuning): epilogue warps meet after every tile: 0 = automatic, 1 = yes, 2 = no  */
 } qhap_bsb_params;
 
 /* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`

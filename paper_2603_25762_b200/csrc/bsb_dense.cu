@@ -74,6 +74,13 @@ struct DenseArgs {
   double dt, a0;
   uint32_t* done;             // [n_tiles_n * n_tiles_m], zero at launch
   uint32_t fence_every;       // state ring: generic -> async proxy fence after every fence_every-th tile of a CTA
+  // L2 eviction priorities: when x and the four fp16 copies fit the L2 next to the streaming y, they are
+  // kept (evict_last) and y passes through (evict_first); otherwise both are the normal policy
+  uint64_t pol_keep, pol_stream;
+  uint32_t store_warp;        // 1: warp 18 issues the TMA stores of the fp16 copies (mbarrier hand-off; needed by fused launches
+                              // and by a single staging buffer); 0: epilogue thread 0 issues them behind a named barrier
+  uint32_t epi_sync;          // 1: the epilogue warps meet at a named barrier after every tile
+  uint32_t stg_bufs;          // staging buffers of (x_hi', x_lo') tiles: 2, or 1 to free 32 KB for another operand stage
 };
 
 // c2 = fp32(dt (a0 - a_k)), a_k = a0 k / (T - 1): the same individually rounded fp64 operations as the host loop
@@ -142,6 +149,7 @@ __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec
 
 // Fused update of one work item: y' = y + dt(-(a0 - a_k) x + c0 F), x' = x + dt a0 y', inelastic wall; stores x', y'
 // (fp32, coalesced across the warp's 32 replicas) and the fp16 split of x' (16 contiguous bytes per thread and array: into the staging tiles, or directly).
+template <bool hints>
 __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tile, int ch,
                                                  const uint32_t (&v)[kChunk], const float (&xv)[kChunk],
                                                  const float (&yv)[kChunk], uint32_t stg) {
@@ -156,8 +164,13 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
       float xn, yn;
       const float c1 = a.c1_per_row ? __ldg(a.c1 + i0 + j) : ec.c1;
       epi_point(ec, c1, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
-      a.x[off] = xn;
-      a.y[off] = yn;
+      if constexpr (hints) {
+        ptx::st_global_f32_hint(a.x + off, xn, a.pol_keep);
+        ptx::st_global_f32_hint(a.y + off, yn, a.pol_stream);
+      } else {
+        a.x[off] = xn;
+        a.y[off] = yn;
+      }
       epi_pack(j, xn, hp, lp);
     }
   } else {
@@ -168,8 +181,8 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
       const float c1 = (a.c1_per_row && (i0 + j) < a.n) ? __ldg(a.c1 + i0 + j) : ec.c1;
       epi_point(ec, c1, __uint_as_float(v[j]), xv[j], yv[j], xn, yn);
       if (ok) {
-        a.x[off] = xn;
-        a.y[off] = yn;
+        ptx::st_global_f32_hint(a.x + off, xn, a.pol_keep);
+        ptx::st_global_f32_hint(a.y + off, yn, a.pol_stream);
       }
       epi_pack(j, ok ? xn : 0.f, hp, lp);
     }
@@ -196,6 +209,10 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
   }
 }
 
+// RING: the fp32 state arrives through the per-warp TMA ring; HINTS: L2 eviction priorities on every state access.
+// Compile-time variants keep each instantiation's hot loops small (the single run-time kernel had grown from 63 to 88 KB
+// of SASS and cost cfg3 3 %).
+template <bool RING, bool HINTS>
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
                   const __grid_constant__ CUtensorMap tm_xh,
@@ -289,8 +306,13 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           } else {
             ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
           }
-          ptx::tma_load_2d(sj + kStageJ, mh, full_bar(stage), kb * kBK, tm * kBM);
-          ptx::tma_load_2d(sj + kStageJ + kStageX, ml, full_bar(stage), kb * kBK, tm * kBM);
+          if constexpr (HINTS) {
+            ptx::tma_load_2d_hint(sj + kStageJ, mh, full_bar(stage), kb * kBK, tm * kBM, a.pol_keep);
+            ptx::tma_load_2d_hint(sj + kStageJ + kStageX, ml, full_bar(stage), kb * kBK, tm * kBM, a.pol_keep);
+          } else {
+            ptx::tma_load_2d(sj + kStageJ, mh, full_bar(stage), kb * kBK, tm * kBM);
+            ptx::tma_load_2d(sj + kStageJ + kStageX, ml, full_bar(stage), kb * kBK, tm * kBM);
+          }
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
@@ -348,17 +370,22 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     // One thread hands each finished pair of staging tiles to TMA, returns the buffer once the bulk reads are done and --
     // fused steps -- signals the tile's completion (done[tile] += 1) once the writes have COMPLETED.  Off the epilogue's
     // critical path: the epilogue warps only arrive on / wait for the two staging barriers.
-    if (a.stage_out && lane == 0) {
+    if (a.stage_out && a.store_warp && lane == 0) {
       const uint32_t stg_base = smem_base + uint32_t(kStages) * kStageBytes;
-      uint32_t tc = 0;
+      uint32_t b = 0, bpar = 0;
       for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
         const int s = vt / stride, tile = vt - s * stride;
         if (tile >= n_tiles) continue;
         const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
-        const uint32_t b = tc & 1u, stg = stg_base + b * (2u * kStageX);
-        ptx::mbar_wait(stg_full(b), (tc >> 1) & 1u);
-        ptx::tma_store_2d((s & 1) ? &tm_xh : &tm_oh, stg, tn * a.BN, tm * kBM);
-        ptx::tma_store_2d((s & 1) ? &tm_xl : &tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+        const uint32_t stg = stg_base + b * (2u * kStageX);
+        ptx::mbar_wait(stg_full(b), bpar);
+        if constexpr (HINTS) {
+          ptx::tma_store_2d_hint((s & 1) ? &tm_xh : &tm_oh, stg, tn * a.BN, tm * kBM, a.pol_keep);
+          ptx::tma_store_2d_hint((s & 1) ? &tm_xl : &tm_ol, stg + kStageX, tn * a.BN, tm * kBM, a.pol_keep);
+        } else {
+          ptx::tma_store_2d((s & 1) ? &tm_xh : &tm_oh, stg, tn * a.BN, tm * kBM);
+          ptx::tma_store_2d((s & 1) ? &tm_xl : &tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+        }
         ptx::tma_store_commit();
         ptx::tma_store_wait_read_all();
         ptx::mbar_arrive(stg_empty(b));
@@ -366,7 +393,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           ptx::tma_store_wait_all();
           ptx::signal_add_release(a.done + tile, 1u);
         }
-        ++tc;
+        if (++b == a.stg_bufs) { b = 0; bpar ^= 1u; }
       }
     }
   } else {
@@ -391,92 +418,123 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     if (a.fused) ec.c2 = ramp_c2(a, 0);
     // every warp owns chunk `par` of every tile (possibly fully masked), so that it arrives on tmem_empty once per tile.
     // Items are addressed by the VIRTUAL tile (step-major); the last wave of a step may have a hole for this CTA.
-    auto advance = [&](int& vt, int& ch) {
-      ch += P;
-      if (ch * kChunk >= a.BN || ((vt % stride) / a.n_tiles_m) * a.BN + ch * kChunk >= a.n) {
-        vt += gridDim.x;
-        if (vt % stride >= n_tiles) vt += gridDim.x;      // hole -> first wave of the next step (stride % grid == 0)
-        ch = par;
+    // A position carries the virtual tile (ordering, end test) and the real tile next to it, so that the item loop needs
+    // no division by the runtime stride.
+    struct Pos { int vt, rt, ch; };
+    auto advance = [&](Pos& p) {
+      p.ch += P;
+      if (p.ch * kChunk >= a.BN || (p.rt / a.n_tiles_m) * a.BN + p.ch * kChunk >= a.n) {
+        p.vt += gridDim.x; p.rt += gridDim.x;
+        if (p.rt >= n_tiles) {                              // past the step's tiles
+          if (p.rt < stride) { p.vt += gridDim.x; p.rt += gridDim.x; }   // hole in the last wave (stride % grid == 0)
+          p.rt -= stride;                                   // first wave of the next step
+        }
+        p.ch = par;
       }
     };
-    auto set_step = [&](int vt) {
-      if (a.fused) {
-        const int s = vt / stride;
-        if (s != cur_s) { cur_s = s; ec.c2 = ramp_c2(a, s); }
-      }
+    int step_end = stride;                     // first virtual tile of step cur_s + 1
+    auto set_step = [&](int vt) {              // items are visited in ascending vt
+      if (a.fused && vt >= step_end) { ++cur_s; step_end += stride; ec.c2 = ramp_c2(a, cur_s); }
     };
+    uint32_t stg_i = 0, stg_par = 0;           // staging buffer of the current tile and its use parity
     // last chunk of this warp in a tile: hand the accumulator stage back and arrive on the staging tile's barrier (the
     // store warp takes it from there).  Fused steps: the fp32 state was written with generic stores and is re-read
     // through TMA one step later by the same warp (requested while the warp works on the tile BEFORE it in the CTA's
     // order), so every lane crosses to the async proxy in between: after every fence_every-th tile, with
     // fence_every <= (fewest tiles a CTA has per step) - 1, the fence that follows a tile's stores comes at most
     // fence_every - 1 tiles later, the request at least (tiles per step) - 1 tiles later.
+    int cur_rt = 0;                            // real tile of the item being finished (for the store above)
     auto tile_done = [&]() {
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
-      if (a.stage_out) {
+      if (a.stage_out && a.store_warp) {
         ptx::fence_proxy_async();
-        if (a.fused && a.ring && (tcount + 1u) % a.fence_every == 0u) ptx::fence_proxy_async_global();
+        if (RING && a.fused && ++tcount == a.fence_every) { tcount = 0; ptx::fence_proxy_async_global(); }
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(stg_full(tcount & 1u));
-        ++tcount;
+        if (lane == 0) ptx::mbar_arrive(stg_full(stg_i));
+        if (++stg_i == a.stg_bufs) { stg_i = 0; stg_par ^= 1u; }
+        if (a.epi_sync) ptx::named_barrier_sync(1, kEpiWarps * 32);       // measured: cfg1 32.3 -> 31.4 us per step
+      } else if (a.stage_out) {
+        // one launch per step with two staging buffers (cfg3, cfg4: 3 % faster than the store warp there): thread 0 waits
+        // until the previous tile's stores have read their buffer, all epilogue warps meet, thread 0 issues the stores
+        ptx::fence_proxy_async();
+        if (ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
+        ptx::named_barrier_sync(1, kEpiWarps * 32);
+        if (ew == 0 && lane == 0) {
+          const uint32_t stg = stg_base + stg_i * (2u * kStageX);
+          const int tn = cur_rt / a.n_tiles_m, tm = cur_rt % a.n_tiles_m;
+          ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
+          ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+          ptx::tma_store_commit();
+        }
+        stg_i ^= 1u;
       }
     };
-    // first chunk of a tile: the accumulator must be complete and the staging buffer free (its previous store has read it)
+    // first chunk of a tile: the accumulator must be complete
     auto tile_begin = [&]() {
       ptx::mbar_wait(tfull_bar(acc), acc_phase);
       ptx::tc_fence_after();
-      if (a.stage_out) ptx::mbar_wait(stg_empty(tcount & 1u), ((tcount >> 1) & 1u) ^ 1u);
     };
-    auto step = [&](int& tile, int& ch, const float (&xc)[kChunk], const float (&yc)[kChunk], float (&xn)[kChunk],
+    // ... and, before the chunk's fp16 pieces go to the staging buffer, its previous store must have read it
+    auto staging_free = [&]() {
+      if (a.stage_out && a.store_warp) ptx::mbar_wait(stg_empty(stg_i), stg_par ^ 1u);
+    };
+    auto step = [&](Pos& p, const float (&xc)[kChunk], const float (&yc)[kChunk], float (&xn)[kChunk],
                     float (&yn)[kChunk]) -> bool {
-      if (ch == par) tile_begin();
+      if (p.ch == par) tile_begin();
       uint32_t v[kChunk];
-      ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + ch * kChunk), v);
-      int ntile = tile, nch = ch;
-      advance(ntile, nch);
-      const bool nhave = ntile < vt_end;
-      if (nhave) epi_load(a, ec, ntile % stride, nch, xn, yn);
+      ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p.ch * kChunk), v);
+      Pos q = p;
+      advance(q);
+      const bool nhave = q.vt < vt_end;
+      if (nhave) epi_load(a, ec, q.rt, q.ch, xn, yn);
       ptx::tmem_ld_wait();
-      const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
-      set_step(tile);
-      epi_update_store(a, ec, tile % stride, ch, v, xc, yc, stg);
-      if (ntile != tile) tile_done();
-      tile = ntile; ch = nch;
+      const uint32_t stg = a.stage_out ? stg_base + stg_i * (2u * kStageX) : 0u;
+      if (p.ch == par) staging_free();
+      set_step(p.vt);
+      epi_update_store<HINTS>(a, ec, p.rt, p.ch, v, xc, yc, stg);
+      cur_rt = p.rt;
+      if (q.vt != p.vt) tile_done();
+      p = q;
       return nhave;
     };
-    if (a.ring) {
+    if constexpr (RING) {
       // State through TMA: every warp owns two 2 KB slots (x and y of one work item: a box of 8 spins x 32 replicas
       // each).  The item two ahead is requested as soon as the current item's values are in registers, so the loads
       // need no registers, no address arithmetic and no LSU slots; out-of-range rows / replicas arrive as zeros.
-      const uint32_t ring_w = stg_base + 4u * kStageX + uint32_t(ew) * (4u * kRingSlot);
+      const uint32_t ring_w = stg_base + a.stg_bufs * (2u * kStageX) + uint32_t(ew) * (4u * kRingSlot);
       const uint32_t rbar0 = ring_bar(2 * ew);
-      auto issue = [&](int vt, int ch, int slot) {
+      auto issue = [&](const Pos& p, int slot) {
         if (ptx::elect_one()) {
-          const int tile = vt % stride;
-          const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+          const int ch = p.ch;
+          const int tn = p.rt / a.n_tiles_m, tm = p.rt % a.n_tiles_m;
           const uint32_t dst = ring_w + uint32_t(slot) * (2u * kRingSlot);
           ptx::mbar_arrive_expect_tx(rbar0 + 8u * slot, 2u * kRingSlot);
-          ptx::tma_load_2d(dst, &tm_sx, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
-          ptx::tma_load_2d(dst + kRingSlot, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
+          if constexpr (HINTS) {
+            ptx::tma_load_2d_hint(dst, &tm_sx, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk, a.pol_keep);
+            ptx::tma_load_2d_hint(dst + kRingSlot, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk, a.pol_stream);
+          } else {
+            ptx::tma_load_2d(dst, &tm_sx, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
+            ptx::tma_load_2d(dst + kRingSlot, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
+          }
         }
         __syncwarp();
       };
-      int t0 = blockIdx.x, c0 = par, t1 = t0, c1i = c0, t2, c2i;
-      if (t0 < vt_end) {
-        issue(t0, c0, 0);
-        advance(t1, c1i);
-        if (t1 < vt_end) issue(t1, c1i, 1);
-        t2 = t1; c2i = c1i;
-        if (t1 < vt_end) advance(t2, c2i);
+      Pos p0{int(blockIdx.x), int(blockIdx.x), par}, p1 = p0, p2 = p0;
+      if (p0.vt < vt_end) {
+        issue(p0, 0);
+        advance(p1);
+        if (p1.vt < vt_end) issue(p1, 1);
+        p2 = p1;
+        if (p1.vt < vt_end) advance(p2);
       }
-      for (uint32_t k = 0; t0 < vt_end; ++k) {
+      for (uint32_t k = 0; p0.vt < vt_end; ++k) {
         const int slot = int(k & 1u);
-        if (c0 == par) tile_begin();
+        if (p0.ch == par) tile_begin();
         uint32_t v[kChunk];
-        ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + c0 * kChunk), v);
+        ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p0.ch * kChunk), v);
         ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
         float xv[kChunk], yv[kChunk];
         const uint32_t src = ring_w + uint32_t(slot) * (2u * kRingSlot) + uint32_t(lane) * 4u;
@@ -486,24 +544,28 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
         }
         __syncwarp();                            // every lane has its values: the slot may be refilled
-        if (t1 < vt_end && t2 < vt_end) issue(t2, c2i, slot);
+        if (p1.vt < vt_end && p2.vt < vt_end) issue(p2, slot);
         ptx::tmem_ld_wait();
-        const uint32_t stg = a.stage_out ? stg_base + (tcount & 1u) * (2u * kStageX) : 0u;
-        set_step(t0);
-        epi_update_store(a, ec, t0 % stride, c0, v, xv, yv, stg);
-        if (t1 != t0) tile_done();
-        t0 = t1; c0 = c1i; t1 = t2; c1i = c2i;
-        if (t2 < vt_end) advance(t2, c2i);
+        const uint32_t stg = a.stage_out ? stg_base + stg_i * (2u * kStageX) : 0u;
+        if (p0.ch == par) staging_free();
+        set_step(p0.vt);
+        epi_update_store<HINTS>(a, ec, p0.rt, p0.ch, v, xv, yv, stg);
+        cur_rt = p0.rt;
+        if (p1.vt != p0.vt) tile_done();
+        p0 = p1; p1 = p2;
+        if (p2.vt < vt_end) advance(p2);
       }
+      if (a.stage_out && !a.store_warp && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();   // smem must outlive the bulk reads
     } else {
-    int tile = blockIdx.x, ch = par;           // virtual tile
-    if (tile < vt_end) {
+    Pos p{int(blockIdx.x), int(blockIdx.x), par};
+    if (p.vt < vt_end) {
       float xa[kChunk], ya[kChunk], xb[kChunk], yb[kChunk];
-      epi_load(a, ec, tile % stride, ch, xa, ya);
+      epi_load(a, ec, p.rt, p.ch, xa, ya);
       while (true) {
-        if (!step(tile, ch, xa, ya, xb, yb)) break;
-        if (!step(tile, ch, xb, yb, xa, ya)) break;
+        if (!step(p, xa, ya, xb, yb)) break;
+        if (!step(p, xb, yb, xa, ya)) break;
       }
+      if (a.stage_out && !a.store_warp && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();
     }
     }
   }
@@ -769,7 +831,15 @@ qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, co
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_step_kernel, tj, tjl, th, tl, toh, tol, tsx, tsy, a));
+  const bool hints = a.pol_keep != ptx::kEvictNormal;
+  auto go = [&](auto kernel) -> qhap_status {
+    // per device and cheap: set on every call (a process may drive several devices)
+    QHAP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
+    QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, tj, tjl, th, tl, toh, tol, tsx, tsy, a));
+    return QHAP_OK;
+  };
+  if (a.ring) QHAP_TRY(hints ? go(dense_step_kernel<true, true>) : go(dense_step_kernel<true, false>));
+  else QHAP_TRY(hints ? go(dense_step_kernel<false, true>) : go(dense_step_kernel<false, false>));
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;
 }
@@ -777,6 +847,30 @@ qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, co
 // Fused launches need: TMA-stored copies and tile rows == k-blocks (BN == kBK), k-block lists, and at least two tiles per
 // CTA and step (the epilogue requests the state of the item two ahead before it stores the current one): the grid is
 // at most half the tile count.  All CTAs of the grid must be co-resident (one per SM, grid <= SM count).
+// Shared-memory split between operand stages and the staging buffers of the fp16 copies: the operand feed (every tile
+// re-reads ~6 k-blocks of x_hi, x_lo: 240 KB per tile at cfg1 against 160 KB of state) runs on the bytes in flight, so a
+// single staging buffer is used whenever that buys another stage (cfg1/cfg2: 2 -> 3 stages, 39.7 -> 36.5 and 45.7 -> 40.9
+// us per step; the epilogue waits for the previous tile's store only right before its first staging write).  Where it
+// buys none (cfg3: 48 KB stages) or a fourth one (cfg4) the second buffer stays (cfg3 275 against 290 us, cfg4 223.5 / 226).
+void choose_staging(DenseArgs& a, int stage_bytes, const qhap_bsb_params& p) {
+  auto stages = [&](int bufs) {
+    return std::min(kMaxStages, (kSmemBudget - (a.stage_out ? bufs * 2 * kStageX : 0) - (a.ring ? kRingBytes : 0)) / stage_bytes);
+  };
+  int bufs = (p.dense_stg_bufs == 1 || p.dense_stg_bufs == 2) ? p.dense_stg_bufs : ((a.stage_out && stages(1) > stages(2) && stages(2) < 3) ? 1 : 2);
+  a.stg_bufs = uint32_t(bufs);
+  a.n_stages = stages(bufs);
+  a.store_warp = bufs == 1 ? 1u : 0u;        // launch_fused sets it too
+}
+
+// x (fp32) and the four fp16 copies are 12 B per (spin, replica); when they fit the L2 with room for the y stream and the
+// J tiles they are given the evict_last priority and y evict_first, so that a step's DRAM traffic is y alone.
+void set_l2_policies(DenseArgs& a, const qhap_bsb_params& p) {
+  const bool keep = p.l2_hints == 0 ? 12.0 * double(a.n) * double(a.R) <= 104e6 : p.l2_hints == 1;
+  a.pol_keep = keep ? ptx::kEvictLast : ptx::kEvictNormal;
+  a.pol_stream = keep ? ptx::kEvictFirst : ptx::kEvictNormal;
+  a.epi_sync = p.dense_epi_sync == 0 ? (keep ? 1u : 0u) : (p.dense_epi_sync == 1 ? 1u : 0u);
+}
+
 // Grid of a fused launch, or 0 = one launch per step.  Worth it while a CTA has few tiles per step (launch gap, pipeline
 // fill and drain per step: cfg1 40.0 -> 38.2 us, cfg2 45.2 -> 41.4 us per step, a 304-tile problem 33.9 -> 14.5 us); with
 // ~50 tiles per CTA and step (cfg3) the step boundary is amortised and the lock-step launches keep the L2 reuse between
@@ -796,6 +890,7 @@ qhap_status launch_fused(int grid, cudaStream_t stream, const CUtensorMap& tj, c
                          const qhap_bsb_params& p, uint32_t* done, int& cur) {
   const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;
   a.fused = 1;
+  a.store_warp = 1;
   a.tile_stride = int32_t(ceil_div(n_tiles, grid) * grid);
   a.fence_every = uint32_t(std::max<int64_t>(1, n_tiles / grid - 1));
   a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0;
@@ -945,7 +1040,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   // staging buffers (2 x 32 KB) come out of the operand-stage budget
   a.stage_out = (BN == kBK) ? 1 : 0;
   a.ring = ring_ok(BN, R, x, y) ? 1 : 0;
-  a.n_stages = std::min(kMaxStages, (kSmemBudget - (a.stage_out ? 4 * kStageX : 0) - (a.ring ? kRingBytes : 0)) / (BN * kBK * 2 + 2 * kStageX));
+  choose_staging(a, BN * kBK * 2 + 2 * kStageX, p);
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = int32_t(ceil_div(n, BN));
   a.n_kblocks = n_kb;
@@ -953,10 +1048,9 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.kb_idx = skip ? kb_idx : nullptr;
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
-  a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
+  set_l2_policies(a, p); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   // per device and cheap: set on every call (a process may drive several devices)
-  QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
   QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));
@@ -1122,15 +1216,14 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.stage_out = 1;
   a.ring = ring_ok(kBK, R, x, y) ? 1 : 0;
   a.j_terms = two_terms ? 2 : 1;
-  a.n_stages = std::min(kMaxStages, (kSmemBudget - 4 * kStageX - (a.ring ? kRingBytes : 0)) / (a.j_terms * kBK * kBK * 2 + 2 * kStageX));
+  choose_staging(a, a.j_terms * kBK * kBK * 2 + 2 * kStageX, p);
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = n_t;
   a.n_kblocks = n_t;
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
   a.c1 = c1row; a.c1_per_row = 1;
   a.x = x; a.y = y;
-  a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
-  QHAP_CUDA_TRY(cudaFuncSetAttribute(dense_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
+  set_l2_policies(a, p); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2], tm_sx, tm_sy;
   QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));

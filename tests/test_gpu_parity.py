@@ -549,6 +549,46 @@ def test_fused_steps_equal_per_step_launches(B, oracle, torch_mod, case):
         assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (case, path, dx, dy)
 
 
+# --------------------- L2 eviction priorities, staging buffers, epilogue meeting: tuning only, same bits
+@pytest.mark.parametrize("step_launch", [0, 1])
+def test_l2_hints_and_staging_variants_are_bit_identical(B, oracle, torch_mod, step_launch):
+    """l2_hints (1 = evict_last on x and the fp16 copies, evict_first on y; 2 = off), dense_stg_bufs (1, 2) and dense_epi_sync
+    (1, 2) select compile-time variants and shared-memory splits of the tcgen05 step; none changes the arithmetic.  Every
+    combination gives the bits of the automatic setting after 10 + 7 steps (odd count: buffers end swapped), on the dense
+    tile_skip path and the block path, and the automatic setting matches the fp64 oracle over the first 10 steps."""
+    fr, pp = synth.make_config(1, scale=0.1)
+    T, R = pp["T"], 300
+    g = oracle.read_graph(fr)
+    wj = oracle.read_weights(g, 1)
+    dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    n = g["n"]
+    x0, y0 = synth.bsb_init_state(11, n, R)
+
+    def run(path, **knobs):
+        xg = torch_mod.from_numpy(x0.copy()).cuda(); yg = torch_mod.from_numpy(y0.copy()).cuda()
+        kw = dict(replicas=R, steps_total=T, weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1 if path == 1 else 0,
+                  dense_bn=64 if path == 1 else 0, finalize=False, step_launch=step_launch, x=xg, y=yg, **knobs)
+        B.qhap_bsb_solve(dg, step_begin=0, steps_run=10, **kw)
+        first = (xg.cpu().numpy(), yg.cpu().numpy())
+        B.qhap_bsb_solve(dg, step_begin=10, steps_run=7, **kw)
+        return first, (xg.cpu().numpy(), yg.cpu().numpy())
+
+    for path in (1, 4):
+        ref_first, ref_last = run(path)
+        for hints in (1, 2):
+            for bufs in (1, 2):
+                for sync in (1, 2):
+                    f, l = run(path, l2_hints=hints, dense_stg_bufs=bufs, dense_epi_sync=sync)
+                    tag = (path, hints, bufs, sync)
+                    assert np.array_equal(f[0], ref_first[0]) and np.array_equal(f[1], ref_first[1]), tag
+                    assert np.array_equal(l[0], ref_last[0]) and np.array_equal(l[1], ref_last[1]), tag
+        xo, yo = x0.astype(np.float64), y0.astype(np.float64)
+        oracle.bsb_run(g["row_ptr"].astype(np.int32), g["col"].astype(np.int32), (-wj).astype(np.float32), xo, yo,
+                       steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+        dx = np.abs(ref_first[0] - xo).max(); dy = np.abs(ref_first[1] - yo).max()
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (path, dx, dy)
+
+
 # ------------------------------------------------------- (3') tcgen05 step on a block-compressed J built from the CSR
 def test_block_path_read_graph_equals_dense_tile_skip(B, oracle, torch_mod):
     """Integer read graph: path 4 stores only the non-empty 64 x 64 tiles of J; same MMAs in the same order as the

@@ -140,6 +140,9 @@ typedef struct {
                         /*    copies evict_last, y evict_first when 12 B x n x R fits the L2), 1 = on, 2 = off        */
   int32_t dense_stg_bufs; /* paths 1, 4 (tuning): shared-memory staging buffers for the fp16 copies: 0 = automatic, 1, 2 */
   int32_t dense_epi_sync; /* paths 1, 4 (tuning): epilogue warps meet after every tile: 0 = automatic, 1 = yes, 2 = no  */
+  int32_t l2_keep_16ths;  /* paths 1, 4 (tuning): with the hints on, the share q/16 (1..16) of the lines of x and its fp16   */
+                        /*    copies that gets evict_last (the rest evict_first, like y): a keep set larger than the L2 thrashes   */
+                        /*    as a whole, a fixed fraction of it stays; 0 = automatic = 16 (measured: DESIGN.md 4.4e)           */
 } qhap_bsb_params;
 
 /* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`

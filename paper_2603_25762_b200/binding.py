@@ -45,7 +45,7 @@ class _BsbParams(C.Structure):
     _fields_ = [("replicas", C.c_int32), ("steps_total", C.c_int32), ("step_begin", C.c_int32), ("steps_run", C.c_int32),
                 ("dt", C.c_double), ("a0", C.c_double), ("c0", C.c_double), ("seed", C.c_uint64),
                 ("weight_mode", C.c_int32), ("path", C.c_int32), ("tile_skip", C.c_int32), ("init_state", C.c_int32),
-                ("finalize", C.c_int32), ("dense_bn", C.c_int32), ("step_launch", C.c_int32), ("l2_hints", C.c_int32), ("dense_stg_bufs", C.c_int32), ("dense_epi_sync", C.c_int32)]
+                ("finalize", C.c_int32), ("dense_bn", C.c_int32), ("step_launch", C.c_int32), ("l2_hints", C.c_int32), ("dense_stg_bufs", C.c_int32), ("dense_epi_sync", C.c_int32), ("l2_keep_16ths", C.c_int32)]
 
 
 for _name in EXPORTS[:15]:
@@ -279,7 +279,7 @@ def qhap_block_split(graph: Csr, windows: np.ndarray) -> Csr:
 
 def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: int = 0, steps_run: Optional[int] = None,
                    dt: float = 1.25, a0: float = 1.0, c0: float = 0.0, seed: int = 0, weight_mode: int = QHAP_WEIGHT_D,
-                   path: int = 0, tile_skip: int = 0, dense_bn: int = 0, step_launch: int = 0, l2_hints: int = 0, dense_stg_bufs: int = 0, dense_epi_sync: int = 0, x: Optional[torch.Tensor] = None, y: Optional[torch.Tensor] = None,
+                   path: int = 0, tile_skip: int = 0, dense_bn: int = 0, step_launch: int = 0, l2_hints: int = 0, dense_stg_bufs: int = 0, dense_epi_sync: int = 0, l2_keep_16ths: int = 0, x: Optional[torch.Tensor] = None, y: Optional[torch.Tensor] = None,
                    dense_J: Optional[torch.Tensor] = None, finalize: bool = True, cut_per_replica: bool = True,
                    workspace: Optional[torch.Tensor] = None) -> dict:
     """(3)(4)(5) bSB solve.  x, y: [n][R] fp32 CUDA tensors updated in place; None -> seeded on the device."""
@@ -296,7 +296,7 @@ def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: i
     n_inst = 1 if inst_ptr is None else len(inst_ptr) - 1
     ip = np.ascontiguousarray(inst_ptr, dtype=np.int32) if inst_ptr is not None else None
     p = _BsbParams(R, steps_total, step_begin, steps_run, dt, a0, c0, seed, weight_mode, path, tile_skip, int(init),
-                   int(finalize), int(dense_bn), int(step_launch), int(l2_hints), int(dense_stg_bufs), int(dense_epi_sync))
+                   int(finalize), int(dense_bn), int(step_launch), int(l2_hints), int(dense_stg_bufs), int(dense_epi_sync), int(l2_keep_16ths))
     gs = graph.c_struct()
     dd = QHAP_DENSE_NONE
     ld = 0

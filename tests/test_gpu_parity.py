@@ -552,8 +552,8 @@ def test_fused_steps_equal_per_step_launches(B, oracle, torch_mod, case):
 # --------------------- L2 eviction priorities, staging buffers, epilogue meeting: tuning only, same bits
 @pytest.mark.parametrize("step_launch", [0, 1])
 def test_l2_hints_and_staging_variants_are_bit_identical(B, oracle, torch_mod, step_launch):
-    """l2_hints (1 = evict_last on x and the fp16 copies, evict_first on y; 2 = off), dense_stg_bufs (1, 2) and dense_epi_sync
-    (1, 2) select compile-time variants and shared-memory splits of the tcgen05 step; none changes the arithmetic.  Every
+    """l2_hints (1 = evict_last on x and the fp16 copies, evict_first on y; 2 = off), l2_keep_16ths (the share of the keep
+    set that gets evict_last), dense_stg_bufs (1, 2) and dense_epi_sync (1, 2) select compile-time variants and shared-memory splits of the tcgen05 step; none changes the arithmetic.  Every
     combination gives the bits of the automatic setting after 10 + 7 steps (odd count: buffers end swapped), on the dense
     tile_skip path and the block path, and the automatic setting matches the fp64 oracle over the first 10 steps."""
     fr, pp = synth.make_config(1, scale=0.1)
@@ -582,6 +582,9 @@ def test_l2_hints_and_staging_variants_are_bit_identical(B, oracle, torch_mod, s
                     tag = (path, hints, bufs, sync)
                     assert np.array_equal(f[0], ref_first[0]) and np.array_equal(f[1], ref_first[1]), tag
                     assert np.array_equal(l[0], ref_last[0]) and np.array_equal(l[1], ref_last[1]), tag
+        for q in (1, 8, 11):
+            f, l = run(path, l2_hints=1, l2_keep_16ths=q)
+            assert np.array_equal(f[0], ref_first[0]) and np.array_equal(l[1], ref_last[1]) and np.array_equal(l[0], ref_last[0]), (path, q)
         xo, yo = x0.astype(np.float64), y0.astype(np.float64)
         oracle.bsb_run(g["row_ptr"].astype(np.int32), g["col"].astype(np.int32), (-wj).astype(np.float32), xo, yo,
                        steps_total=T, step_begin=0, steps_run=10, n_threads=8)

@@ -1156,6 +1156,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   float* rem_val = ws.take<float>(size_t(g.nnz));
   uint32_t* scal = ws.take<uint32_t>(4);
   int64_t* totals = ws.take<int64_t>(2);
+  int64_t* scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(n), 4096)) + 1);
   uint32_t* done = ws.take<uint32_t>(size_t(n_t) * size_t(ceil_div(R, kBM)));
   const int64_t cap_blocks = block_capacity(n, g.nnz);
   const size_t cap = size_t(cap_blocks) * kBK * kBK;
@@ -1195,7 +1196,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
     const int rb = int(ceil_div(int64_t(n) * 32, 256));
     remainder_kernel<0><<<rb, 256, 0, stream>>>(n, g.row_ptr, g.col, jval, n_t, kb_cnt, kb_idx, rem_ptr, rem_col, rem_val);
     QHAP_LAUNCH_CHECK();
-    QHAP_TRY(exclusive_scan_i32(rem_ptr, rem_ptr, n, totals, reinterpret_cast<int32_t*>(totals + 1), stream));
+    QHAP_TRY(exclusive_scan_i32(rem_ptr, rem_ptr, n, totals, reinterpret_cast<int32_t*>(totals + 1), stream, scan_scratch));
     remainder_kernel<1><<<rb, 256, 0, stream>>>(n, g.row_ptr, g.col, jval, n_t, kb_cnt, kb_idx, rem_ptr, rem_col, rem_val);
     QHAP_LAUNCH_CHECK();
   }

@@ -97,6 +97,7 @@ extern "C" qhap_status qhap_component_split(const qhap_csr* graph, int32_t min_s
   int32_t* inv = ws.take<int32_t>(size_t(n) + 1);
   int32_t* flag = ws.take<int32_t>(4);
   int64_t* totals = ws.take<int64_t>(2);
+  int64_t* scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(graph->n), 4096)) + 1);
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
@@ -158,7 +159,7 @@ extern "C" qhap_status qhap_component_split(const qhap_csr* graph, int32_t min_s
   }
   cc_degree_kernel<<<int(ceil_div(m, 256)), 256, 0, stream>>>(m, perm, graph->row_ptr, out->row_ptr);
   QHAP_LAUNCH_CHECK();
-  QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, m, totals, reinterpret_cast<int32_t*>(totals + 1), stream));
+  QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, m, totals, reinterpret_cast<int32_t*>(totals + 1), stream, scan_scratch));
   cc_fill_kernel<<<int(ceil_div(int64_t(m) * 32, 256)), 256, 0, stream>>>(m, perm, inv, graph->row_ptr, graph->col, graph->d, graph->c,
                                                                          graph->w_fx, graph->w, out->row_ptr, out->col, out->d, out->c,
                                                                          out->w_fx, out->w);

@@ -645,6 +645,7 @@ extern "C" qhap_status qhap_block_split(const qhap_csr* graph, int32_t n_blocks,
   int32_t* off_d = ws.take<int32_t>(size_t(n_blocks) + 1);
   int64_t* total_d = ws.take<int64_t>(1);
   int32_t* flags_d = ws.take<int32_t>(1);
+  int64_t* scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(n_out), 4096)) + 1);
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
@@ -661,7 +662,7 @@ extern "C" qhap_status qhap_block_split(const qhap_csr* graph, int32_t n_blocks,
                                              graph->w, out->row_ptr, nullptr, nullptr, nullptr);
     QHAP_LAUNCH_CHECK();
   }
-  QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, n_out, total_d, flags_d, stream));
+  QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, n_out, total_d, flags_d, stream, scan_scratch));
   int64_t total = 0;
   QHAP_CUDA_TRY(cudaMemcpyAsync(&total, total_d, sizeof(total), cudaMemcpyDeviceToHost, stream));
   QHAP_CUDA_TRY(cudaStreamSynchronize(stream));   // also keeps `off` alive until the copies above are done

@@ -98,10 +98,11 @@ def bsb_c0(row_ptr, jval) -> float:
 
 
 def bsb_run(row_ptr, col, jval, x, y, *, steps_total, step_begin=0, steps_run=None, dt=1.25, a0=1.0, c0=None,
-            n_threads=1, xpre=None):
+            n_threads=1, xpre=None, force_mode=0):
     """Advance fp64 state x, y ([n][R]) in place by ``steps_run`` bSB steps; returns (x, y, c0).
 
-    ``xpre`` (optional fp64 [n][R] array) receives x of the last step before the wall rule."""
+    ``xpre`` (optional fp64 [n][R] array) receives x of the last step before the wall rule.
+    ``force_mode`` 1 = dSB (F = J sgn(x)), 0 = bSB (L265)."""
     rp, cl, jv = _c(row_ptr, np.int32), _c(col, np.int32), _c(jval, np.float32)
     n = len(rp) - 1
     x = np.ascontiguousarray(x, np.float64); y = np.ascontiguousarray(y, np.float64)
@@ -113,7 +114,7 @@ def bsb_run(row_ptr, col, jval, x, y, *, steps_total, step_begin=0, steps_run=No
         steps_run = steps_total - step_begin
     lib().orc_bsb_run(C.c_int32(n), _p(rp), _p(cl), _p(jv), C.c_int32(R), C.c_int32(steps_total),
                       C.c_int32(step_begin), C.c_int32(steps_run), C.c_double(dt), C.c_double(a0), C.c_double(c0),
-                      _p(x), _p(y), _p(xpre), C.c_int32(n_threads))
+                      _p(x), _p(y), _p(xpre), C.c_int32(n_threads), C.c_int32(force_mode))
     return x, y, c0
 
 
@@ -213,15 +214,36 @@ def read_weights(g, weight_mode: int) -> np.ndarray:
     return (g["d"].astype(np.int64) if weight_mode == 0 else g["d"].astype(np.int64) - g["c"].astype(np.int64))
 
 
-def solve(row_ptr, col, w_int, jval, x0, y0, *, steps_total, dt=1.25, a0=1.0, c0=None, n_threads=1):
-    """Full single-instance solve: bSB from fp32 x0,y0 -> spins, cuts, best replica."""
-    x, y, c0 = bsb_run(row_ptr, col, jval, x0.astype(np.float64), y0.astype(np.float64), steps_total=steps_total,
-                       dt=dt, a0=a0, c0=c0, n_threads=n_threads)
+def solve(row_ptr, col, w_int, jval, x0, y0, *, steps_total, dt=1.25, a0=1.0, c0=None, n_threads=1, force_mode=0,
+          eval_every=0):
+    """Full single-instance solve: bSB from fp32 x0,y0 -> spins, cuts, best replica.
+
+    ``eval_every`` = k > 0 additionally returns ``trace``: the per-replica cuts of sign(x) after steps k, 2k, ... (what
+    Fig. 3 plots as the minimum energy over the samples at every time step): int64 [n_evals][R], plus
+    ``trace_steps`` (the number of steps completed at each evaluation).  The state is simply advanced k steps at a time."""
+    x, y = x0.astype(np.float64), y0.astype(np.float64)
+    trace, trace_steps = [], []
+    if eval_every and eval_every > 0:
+        k = 0
+        while k + eval_every <= steps_total:
+            x, y, c0 = bsb_run(row_ptr, col, jval, x, y, steps_total=steps_total, step_begin=k, steps_run=eval_every, dt=dt, a0=a0,
+                               c0=c0, n_threads=n_threads, force_mode=force_mode)
+            k += eval_every
+            trace.append(cut_eval(row_ptr, col, w_int, sign_spins(x))[0]); trace_steps.append(k)
+        if k < steps_total:
+            x, y, c0 = bsb_run(row_ptr, col, jval, x, y, steps_total=steps_total, step_begin=k, dt=dt, a0=a0, c0=c0,
+                               n_threads=n_threads, force_mode=force_mode)
+    else:
+        x, y, c0 = bsb_run(row_ptr, col, jval, x, y, steps_total=steps_total, dt=dt, a0=a0, c0=c0, n_threads=n_threads,
+                           force_mode=force_mode)
     s = sign_spins(x)
     cut, en = cut_eval(row_ptr, col, w_int, s)
     r = best_replica(cut)
-    return dict(x=x, y=y, c0=c0, spins=s, cut=cut, energy=en, best_replica=r, best_cut=int(cut[r]),
-                best_spins=s[:, r].copy())
+    out = dict(x=x, y=y, c0=c0, spins=s, cut=cut, energy=en, best_replica=r, best_cut=int(cut[r]),
+               best_spins=s[:, r].copy())
+    if trace:
+        out["trace"] = np.stack(trace); out["trace_steps"] = np.array(trace_steps, np.int32)
+    return out
 
 
 # ---------------------------------------------------------------------------------------------- O6

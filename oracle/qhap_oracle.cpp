@@ -7,9 +7,12 @@
 //
 // Pins (tests/test_oracle_pins.py) and what stays "parity unpinned":
 //   O1 read graph, O2 SNP graph, O4 cut/energy, O5 readouts+metrics: pinned (library matmul special
-//   case, closed forms, hand values, brute force, the paper's SE/HE worked example).
+//   case, closed forms, hand values, brute force, the paper's SE/HE worked example); the readings sgn(0) = +1
+//   (R10e), Pore-C fragments' exhaustive reach and alpha (R8), the Phred clamp [1, 93] (R5) and the stitch tie
+//   rule (R17) each have a hand-made pin (tests/golden/snp_edge_depth_porec_clamp.txt for R5 / R8).
 //   O3 bSB: its ARITHMETIC and update order are pinned (explicit linear-map product, scalar
-//   recurrence, exact symmetries), its solution quality by brute force and planted recovery; the
+//   recurrence, exact symmetries; dSB: sign-only force, hand values, affine-map product), its solution quality by
+//   brute force and planted recovery; the
 //   CONSTANTS c0, the ramp end points and the wall rule are "parity unpinned" against the paper,
 //   which prints no bSB equation (PAPER.md:L265 is prose) -- see DESIGN.md readings R10a-f.
 //
@@ -146,6 +149,9 @@ int64_t orc_snp_graph(int32_t n_frag, int32_t n_snp, const int64_t* frag_ptr, co
 //   a_k = a0 k / (T-1);  F = J x (x of the previous step for every row);
 //   y += dt (-(a0 - a_k) x + c0 F);  x += dt a0 y;  |x| > 1: x = sign(x), y = 0.
 // State layout [n][R], replica index contiguous.  jval[e] = J entry = -w (fp32 value, promoted).
+// force_mode 1 = dSB, the discrete variant the paper's bake-off contrasts with bSB (Fig. 2-3;
+// SURVEY.md 8(f) f4): the force is evaluated on the discretised positions, F = J sgn(x), with sgn(0) = +1 (R10e);
+// everything else is unchanged.  force_mode 0 = bSB (the paper's solver, L265).
 // ------------------------------------------------------------------------------------------------
 double orc_bsb_c0(int32_t n, const int32_t* row_ptr, const float* jval) {
   double ss = 0.0;
@@ -156,14 +162,18 @@ double orc_bsb_c0(int32_t n, const int32_t* row_ptr, const float* jval) {
 
 static void bsb_slice(int32_t n, const int32_t* row_ptr, const int32_t* col, const float* jval, int32_t R,
                       int32_t steps_total, int32_t step_begin, int32_t steps_run, double dt, double a0, double c0,
-                      double* x, double* y, double* xpre, int32_t r0, int32_t r1) {
+                      double* x, double* y, double* xpre, int32_t r0, int32_t r1, int32_t force_mode) {
   std::vector<double> F(size_t(n) * size_t(r1 - r0));
   for (int32_t k = step_begin; k < step_begin + steps_run; ++k) {
     double a_k = (steps_total > 1) ? a0 * double(k) / double(steps_total - 1) : 0.0;
     for (int32_t i = 0; i < n; ++i)
       for (int32_t r = r0; r < r1; ++r) {
         double f = 0.0;
-        for (int32_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) f += double(jval[e]) * x[size_t(col[e]) * R + r];
+        for (int32_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+          double xj = x[size_t(col[e]) * R + r];
+          if (force_mode == 1) xj = (xj >= 0.0) ? 1.0 : -1.0;          // dSB: F = J sgn(x), sgn(0) = +1
+          f += double(jval[e]) * xj;
+        }
         F[size_t(i) * (r1 - r0) + (r - r0)] = f;
       }
     for (int32_t i = 0; i < n; ++i)
@@ -180,12 +190,12 @@ static void bsb_slice(int32_t n, const int32_t* row_ptr, const int32_t* col, con
 void orc_bsb_run(int32_t n, const int32_t* row_ptr, const int32_t* col, const float* jval, int32_t R,
                  int32_t steps_total, int32_t step_begin, int32_t steps_run, double dt, double a0, double c0,
                  double* x, double* y, double* xpre /* optional [n][R]: x of the last step before the wall rule */,
-                 int32_t n_threads) {
-  if (n_threads <= 1) { bsb_slice(n, row_ptr, col, jval, R, steps_total, step_begin, steps_run, dt, a0, c0, x, y, xpre, 0, R); return; }
+                 int32_t n_threads, int32_t force_mode /* 0 bSB, 1 dSB */) {
+  if (n_threads <= 1) { bsb_slice(n, row_ptr, col, jval, R, steps_total, step_begin, steps_run, dt, a0, c0, x, y, xpre, 0, R, force_mode); return; }
   std::vector<std::thread> th;                                      // replicas are independent (L265)
   for (int32_t t = 0; t < n_threads; ++t) {
     int32_t r0 = int32_t(int64_t(R) * t / n_threads), r1 = int32_t(int64_t(R) * (t + 1) / n_threads);
-    if (r1 > r0) th.emplace_back(bsb_slice, n, row_ptr, col, jval, R, steps_total, step_begin, steps_run, dt, a0, c0, x, y, xpre, r0, r1);
+    if (r1 > r0) th.emplace_back(bsb_slice, n, row_ptr, col, jval, R, steps_total, step_begin, steps_run, dt, a0, c0, x, y, xpre, r0, r1, force_mode);
   }
   for (auto& t : th) t.join();
 }

@@ -244,8 +244,35 @@ def test_cut_eval_empty_graph(B, torch_mod):
 
 
 # ------------------------------------------------------------------------------------------ (3)(4) bSB steps
+_RECORDS = []            # one entry per compare_trajectory call; rewritten to RECORD_FILE after every call
+
+
+def _record_file():
+    import os
+    from pathlib import Path
+    p = os.environ.get("QHAP_PARITY_RECORD")
+    if p:
+        return Path(p)
+    d = Path(__file__).resolve().parent.parent / "gpurun_out"
+    return d / "parity_horizons.json"
+
+
+def _record(entry):
+    """Per-case record of what the trajectory comparison really asserted: written as JSON next to the
+    GPU run's other outputs; profiles/r2_parity_horizons.json is a copy of the file the committed tests wrote on the B200."""
+    import json
+    _RECORDS.append(entry)
+    try:
+        f = _record_file()
+        f.parent.mkdir(parents=True, exist_ok=True)
+        f.write_text(json.dumps(_RECORDS, indent=1))
+    except OSError:
+        pass
+
+
 def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, steps=50, path=2, dense_J=None, inst_ptr=None,
-                       c0=None, tile_skip=0, expect_full=False, min_horizon=MIN_HORIZON):
+                       c0=None, tile_skip=0, expect_full=False, min_horizon=MIN_HORIZON, case="", sample=None, strict=True,
+                       force_mode=0, max_tainted=None, **solve_kw):
     """Trajectory parity over the first `steps` steps from identical fp32 initial states (R18).
 
     (a) RESYNCHRONISED: at every step k the GPU starts from fp32(oracle state after k steps) and takes ONE step; the oracle
@@ -255,11 +282,18 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         ulp) has drifted more than TWIN_TOL from it -- past that step the recurrence has amplified an input rounding a
         thousandfold and no fp32-state implementation can track the fp64 one.  expect_full=True asserts all steps.
     A (spin, replica) whose oracle pre-clamp |x| lies within WALL_BAND of 1 may take the other wall decision; its y is
-    excluded for that step (x still agrees to ~WALL_BAND).  Returns a dict of maxima, the horizon and the excluded count."""
+    excluded for that step (x still agrees to ~WALL_BAND).
+    `sample`: replica indices the oracle follows (full-size cases: replicas are independent trajectories, so the oracle runs
+    exactly those columns; the GPU runs all R).  `strict=False` records without asserting the free-running bar (probes).
+    Every call appends its record (horizon, per-step maxima, first step beyond the bar, tainted / excluded counts) to the
+    JSON file of `_record`.  Returns the record."""
     jval = (-(g["w"] if mode == 2 else w_int)).astype(np.float32)
     x0, y0 = synth.bsb_init_state(seed, n, R)
+    cols = np.arange(R) if sample is None else np.asarray(sample)
+    Rs = len(cols)
     dg = B.upload_csr(dict(g, inst_ptr=inst_ptr))
     xg = torch_mod.from_numpy(x0.copy()).cuda(); yg = torch_mod.from_numpy(y0.copy()).cuda()
+    cols_t = torch_mod.from_numpy(cols).cuda()
     ws = None
     if inst_ptr is None:
         inst = [(0, n)]
@@ -270,47 +304,57 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         rp = (g["row_ptr"][lo:hi + 1] - g["row_ptr"][lo]).astype(np.int32)
         sl = slice(int(g["row_ptr"][lo]), int(g["row_ptr"][hi]))
         subs.append((rp, (g["col"][sl] - lo).astype(np.int32), jval[sl]))
+    okw = dict(force_mode=force_mode) if force_mode else {}
 
     def oracle_step(x, y, k):
         x, y = x.copy(), y.copy()
         xpre = np.zeros_like(x)
         for (lo, hi), (rp, cl, jv) in zip(inst, subs):
-            xs, ys, xp = x[lo:hi].copy(), y[lo:hi].copy(), np.zeros((hi - lo, R))
-            oracle.bsb_run(rp, cl, jv, xs, ys, steps_total=T, step_begin=k, steps_run=1, n_threads=8, xpre=xp, c0=c0)
+            xs, ys, xp = x[lo:hi].copy(), y[lo:hi].copy(), np.zeros((hi - lo, Rs))
+            oracle.bsb_run(rp, cl, jv, xs, ys, steps_total=T, step_begin=k, steps_run=1, n_threads=8, xpre=xp, c0=c0, **okw)
             x[lo:hi], y[lo:hi], xpre[lo:hi] = xs, ys, xp
         return x, y, xpre
 
     def gpu_step(xt, yt, k):
         nonlocal ws
         res = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, step_begin=k, steps_run=1, weight_mode=mode, path=path, x=xt, y=yt,
-                               dense_J=dense_J, finalize=False, workspace=ws, c0=c0 or 0.0, tile_skip=tile_skip)
+                               dense_J=dense_J, finalize=False, workspace=ws, c0=c0 or 0.0, tile_skip=tile_skip,
+                               **(dict(force_mode=force_mode) if force_mode else {}), **solve_kw)
         ws = res["workspace"]
-        return xt.cpu().numpy().astype(np.float64), yt.cpu().numpy().astype(np.float64)
+        return xt[:, cols_t].cpu().numpy().astype(np.float64), yt[:, cols_t].cpu().numpy().astype(np.float64)
 
     def diff(xh, yh, xo, yo, xpre):
         marginal = np.abs(np.abs(xpre) - 1.0) < WALL_BAND
-        return np.abs(xh - xo).max(), np.abs(np.where(marginal, 0.0, yh - yo)).max(), int(marginal.sum())
+        return float(np.abs(xh - xo).max()), float(np.abs(np.where(marginal, 0.0, yh - yo)).max()), int(marginal.sum())
 
-    xo = x0.astype(np.float64); yo = y0.astype(np.float64)
+    xo = np.ascontiguousarray(x0[:, cols], np.float64); yo = np.ascontiguousarray(y0[:, cols], np.float64)
     xt = xo * (1.0 + 2.0 ** -23); yt = yo * (1.0 + 2.0 ** -23)        # the oracle's twin, one fp32 ulp away
-    out = dict(free_dx=0.0, free_dy=0.0, resync_dx=0.0, resync_dy=0.0, horizon=steps, excluded=0, tail_dx=0.0)
+    twin_tol = TWIN_TOL_TC if path in (1, 4) else TWIN_TOL
+    out = dict(case=case, path=path, n=int(n), R=int(R), replicas_compared=int(Rs), steps=int(steps), expect_full=bool(expect_full),
+               twin_tol=twin_tol, free_dx=0.0, free_dy=0.0, resync_dx=0.0, resync_dy=0.0, horizon=steps, excluded=0, tail_dx=0.0,
+               first_exceed=None, twin_at_first_exceed=None, series_dx=[], series_dy=[], series_twin=[])
     horizon_open = True
-    tainted = np.zeros(R, bool)
+    tainted = np.zeros(Rs, bool)
     for k in range(steps):
         # (a) resynchronised single step from the oracle's current state rounded to fp32
-        xs32, ys32 = xo.astype(np.float32), yo.astype(np.float32)
+        xs32, ys32 = np.ascontiguousarray(xo, np.float32), np.ascontiguousarray(yo, np.float32)
         xr, yr, xrpre = oracle_step(xs32.astype(np.float64), ys32.astype(np.float64), k)
-        xh, yh = gpu_step(torch_mod.from_numpy(xs32).cuda(), torch_mod.from_numpy(ys32).cuda(), k)
+        if sample is None:
+            xs_t, ys_t = torch_mod.from_numpy(xs32).cuda(), torch_mod.from_numpy(ys32).cuda()
+        else:                                  # the other replicas keep the free-running GPU state (independent trajectories)
+            xs_t, ys_t = xg.clone(), yg.clone()
+            xs_t[:, cols_t] = torch_mod.from_numpy(xs32).cuda(); ys_t[:, cols_t] = torch_mod.from_numpy(ys32).cuda()
+        xh, yh = gpu_step(xs_t, ys_t, k)
         dx, dy, exc = diff(xh, yh, xr, yr, xrpre)
         out["resync_dx"], out["resync_dy"] = max(out["resync_dx"], dx), max(out["resync_dy"], dy)
         out["excluded"] += exc
-        assert dx <= RESYNC_TOL and dy <= RESYNC_TOL, f"resync step {k}: max|dx| {dx:.3e}, max|dy| {dy:.3e}"
+        assert dx <= RESYNC_TOL and dy <= RESYNC_TOL, f"{case}: resync step {k}: max|dx| {dx:.3e}, max|dy| {dy:.3e}"
         # (b) free-running
         xo, yo, xpre = oracle_step(xo, yo, k)
         xt, yt, _ = oracle_step(xt, yt, k)
         xh, yh = gpu_step(xg, yg, k)
-        twin = max(np.abs(xt - xo).max(), np.abs(yt - yo).max())
-        if horizon_open and twin > (TWIN_TOL_TC if path in (1, 4) else TWIN_TOL) and not expect_full:
+        twin = float(max(np.abs(xt - xo).max(), np.abs(yt - yo).max()))
+        if horizon_open and twin > twin_tol and not expect_full:
             out["horizon"], horizon_open = k, False
         # a replica whose GPU run took the OTHER wall decision at a marginal pre-clamp |x| (within WALL_BAND of 1) follows a
         # legitimately different trajectory from then on (the wall is a discontinuity; replicas are independent): it leaves
@@ -319,23 +363,30 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         flipped = marginal & ((yh == 0.0) != (yo == 0.0))
         tainted |= flipped.any(axis=0)
         keep = ~tainted
-        dx, dy, exc = diff(xh[:, keep], yh[:, keep], xo[:, keep], yo[:, keep], xpre[:, keep])
+        dx, dy, exc = diff(xh[:, keep], yh[:, keep], xo[:, keep], yo[:, keep], xpre[:, keep]) if keep.any() else (0.0, 0.0, 0)
+        out["series_dx"].append(dx); out["series_dy"].append(dy); out["series_twin"].append(twin)
+        if out["first_exceed"] is None and (dx > TRAJ_TOL or dy > TRAJ_TOL):
+            out["first_exceed"], out["twin_at_first_exceed"] = k, twin
         if horizon_open:
             out["free_dx"], out["free_dy"] = max(out["free_dx"], dx), max(out["free_dy"], dy)
             out["excluded"] += exc
-            assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, f"free-running step {k} (twin drift {twin:.1e}): max|dx| {dx:.3e}, max|dy| {dy:.3e}"
+            if strict:
+                assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, f"{case}: free-running step {k} (twin drift {twin:.1e}): max|dx| {dx:.3e}, max|dy| {dy:.3e}"
         else:
             out["tail_dx"] = max(out["tail_dx"], dx)
     out["tainted"] = int(tainted.sum())
-    assert out["tainted"] <= max(2, 0.5 * R), out     # the free-running check must not become vacuous
-    assert out["excluded"] <= 1e-3 * n * R * steps * 2
-    assert out["horizon"] >= min(steps, min_horizon), out
+    _record(out)
+    cap = max(2, 0.5 * Rs) if max_tainted is None else max_tainted
+    assert out["tainted"] <= cap, {k: v for k, v in out.items() if not k.startswith("series")}     # the free-running check must not become vacuous
+    assert out["excluded"] <= 1e-3 * n * Rs * steps * 2
+    if strict:
+        assert out["horizon"] >= min(steps, min_horizon), {k: v for k, v in out.items() if not k.startswith("series")}
     return out
 
 
 def fmt_traj(o):
     return (f"free-running max|dx| {o['free_dx']:.2e} max|dy| {o['free_dy']:.2e} over {o['horizon']} steps "
-            f"(after the horizon: {o['tail_dx']:.1e}); resync max|dx| {o['resync_dx']:.2e} max|dy| {o['resync_dy']:.2e}; "
+            f"(after the horizon: {o['tail_dx']:.1e}; first step beyond 1e-3: {o['first_exceed']}); resync max|dx| {o['resync_dx']:.2e} max|dy| {o['resync_dy']:.2e}; "
             f"excluded {o['excluded']}, replicas dropped after a marginal wall flip {o.get('tainted', 0)}")
 
 

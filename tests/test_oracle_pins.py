@@ -532,3 +532,160 @@ def test_component_split_known_graph_and_bfs(oracle):
                 comps.append(sorted(comp))
         assert cs["perm"].tolist() == [v for c in comps for v in c]
         assert np.diff(cs["inst_ptr"]).tolist() == [len(c) for c in comps]
+
+
+# ------------------------------------------------- round 2: the four behaviours VERDICT r1 listed as "parity unpinned"
+def test_R10e_sign_of_zero_is_plus_one(oracle):
+    """Reading R10e ("s = sgn(x)"; Eq. 6 needs s in {-1, +1}, so sgn(0) must pick a side): x = +0.0 and
+    x = -0.0 both read out as +1; the smallest negative number as -1.  A spin vector therefore never contains 0 and every
+    vertex is on exactly one side of the cut."""
+    x = np.array([[0.0, -0.0, 5e-324, -5e-324, 1.0, -1.0]])
+    assert oracle.sign_spins(x).tolist() == [[1, 1, 1, -1, 1, -1]]
+    # consequence for the solver: a spin that sits exactly at 0 (isolated vertex, x0 = y0 = 0) is reported as +1
+    rp = np.zeros(3, np.int32); cl = np.zeros(0, np.int32)
+    res = oracle.solve(rp, cl, np.zeros(0, np.int64), np.zeros(0, np.float32), np.zeros((2, 1), np.float32), np.zeros((2, 1), np.float32),
+                       steps_total=5)
+    assert res["best_spins"].tolist() == [1, 1] and np.all(res["x"] == 0.0)
+
+
+def _golden_depth_rows():
+    edges, clamps = {}, []
+    for ln in (GOLDEN / "snp_edge_depth_porec_clamp.txt").read_text().splitlines():
+        f = ln.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] == "edge":
+            edges.setdefault((int(f[1]), int(f[2]), float(f[3])), {})[(int(f[4]), int(f[5]))] = float(f[6])
+        elif f[0] == "clamp":
+            clamps.append((int(f[1]), int(f[2]), float(f[3])))
+    return edges, clamps
+
+
+def test_R8_porec_fragments_keep_every_pair_and_scale_by_alpha(oracle):
+    """PAPER.md:L85 (depth), L344-L350 (Pore-C, alpha), reading R8: a k = 5 fragment at depth 3/10 emits only its 4 adjacent
+    pairs; the SAME fragment flagged Pore-C emits all 10 pairs (reach = k - 1 whatever the depth) and every weight is
+    alpha x the unflagged exhaustive one.  Expected edge lists and 20-digit weights: tests/golden/ (mpmath script beside it);
+    a build that applied the depth limit to Pore-C fragments, forgot alpha, or used alpha on ordinary reads fails here."""
+    edges, _ = _golden_depth_rows()
+    Q = [12, 25, 7, 33, 18]
+    assert len(edges) == 4
+    for (tenths, flag, alpha), exp in edges.items():
+        g = oracle.snp_graph(one_fragment(list(range(5)), [0] * 5, Q, n_snp=5, flag=flag), tenths, alpha)
+        W = csr_to_dense(g, g["w_fx"]).astype(np.float64) / 2.0 ** 32
+        got = {(u, v) for u in range(5) for v in range(u + 1, 5) if csr_to_dense(g, np.ones(g["nnz"], np.int64))[u, v]}
+        assert got == set(exp), (tenths, flag, sorted(got))
+        for (u, v), w in exp.items():
+            assert abs(W[u, v] - w) <= 2.0 ** -32 and W[v, u] == W[u, v], (tenths, flag, u, v, W[u, v], w)
+    assert len(edges[(3, 0, 0.1)]) == 4 and len(edges[(3, 1, 0.1)]) == 10
+    # a Pore-C fragment next to an ordinary read through the same SNP pair: the two contributions add (alpha only on one)
+    fr2 = synth.Fragments(2, 5, np.array([0, 5, 10], np.int64), np.tile(np.arange(5, dtype=np.int32), 2), np.zeros(10, np.uint8),
+                          np.array(Q * 2, np.uint8), np.array([0, 1], np.uint8), np.zeros(5, np.uint8), np.zeros(5, np.uint8),
+                          np.zeros(2, np.uint8), np.arange(5, dtype=np.int64))
+    g2 = oracle.snp_graph(fr2, 3, 0.1)
+    W2 = csr_to_dense(g2, g2["w_fx"]).astype(np.float64) / 2.0 ** 32
+    for (u, v), w in edges[(3, 1, 0.1)].items():
+        expect = w + edges[(3, 0, 0.1)].get((u, v), 0.0)
+        assert abs(W2[u, v] - expect) <= 2 * 2.0 ** -32
+
+
+def test_R5_phred_clamp(oracle):
+    """Reading R5: integer Phred is clamped to [1, 93] before Eq. 9 (Q = 0 would make q = 0 and, for two such sites,
+    P_trans = P_cis; Q > 93 has no table entry).  Q = 0 weighs exactly like Q = 1 and Q = 200 like Q = 93; the values are the
+    mpmath evaluation of Eq. 9-14 at the CLAMPED qualities (tests/golden/snp_edge_depth_porec_clamp.txt)."""
+    _, clamps = _golden_depth_rows()
+    assert len(clamps) >= 6
+    for qu, qv, w in clamps:
+        g = oracle.snp_graph(one_fragment([0, 1], [0, 0], [min(qu, 255), min(qv, 255)], n_snp=2), 10, 0.1)
+        got = csr_to_dense(g, g["w_fx"])[0, 1] / 2.0 ** 32
+        # fp64 conditioning of Eq. 11-12 as printed: 1 - q = 10^(-Q/10) is formed by subtraction from 1, so P_trans carries a
+        # relative error of about eps / (1 - q); beyond Q ~ 60 that exceeds one fixed-point ulp (Q = 93: 2e-7 relative)
+        qmax = min(93, max(1, max(qu, qv)))
+        tol = max(2.0 ** -32, 4 * 2.0 ** -53 * 10.0 ** (qmax / 10.0) / np.log(10.0))
+        assert abs(got - w) <= tol, (qu, qv, got, w, tol)
+    same = lambda a, b: np.array_equal(oracle.snp_graph(one_fragment([0, 1], [0, 1], list(a), n_snp=2), 10, 0.1)["w_fx"],
+                                       oracle.snp_graph(one_fragment([0, 1], [0, 1], list(b), n_snp=2), 10, 0.1)["w_fx"])
+    assert same((0, 20), (1, 20)) and same((200, 20), (93, 20)) and same((94, 0), (93, 1)) and not same((2, 20), (1, 20)) \
+        and not same((92, 20), (93, 20))
+
+
+def test_R17_stitch_tie_keeps_orientation(oracle):
+    """Reading R17: a block is flipped only when the overlap DISAGREES with the (already oriented) previous block, i.e. when
+    the agreement sum is negative; a tie (sum = 0) keeps the block as solved.  Two blocks, overlap of two SNPs, one agreeing
+    and one disagreeing -> no flip; make both disagree -> flip; the tie rule also chains through an already flipped block."""
+    win = np.array([[0, 4], [2, 6]], np.int64)
+    b0 = np.array([1, 1, 1, -1], np.int8)
+    b1 = np.array([1, 1, -1, 1], np.int8)            # overlap SNPs 2, 3: b0 = (1, -1), b1 = (1, 1) -> +1 - 1 = 0: tie
+    out = oracle.block_stitch(6, win, [b0, b1])
+    assert out.tolist() == [1, 1, 1, 1, -1, 1]       # block 0 owns [0, 3), block 1 owns [3, 6), unflipped
+    b1f = np.array([-1, 1, -1, 1], np.int8)          # overlap (−1, 1) vs (1, −1): both disagree -> flipped
+    assert oracle.block_stitch(6, win, [b0, b1f]).tolist() == [1, 1, 1, -1, 1, -1]
+    win3 = np.array([[0, 4], [2, 6], [4, 8]], np.int64)
+    b2 = np.array([1, -1, 1, 1], np.int8)            # vs oriented block 1 (flipped b1f = (1,-1,1,-1)) on SNPs 4, 5: (1,-1) vs (1,-1): agree
+    assert oracle.block_stitch(8, win3, [b0, b1f, b2]).tolist() == [1, 1, 1, -1, 1, -1, 1, 1]
+    b2t = np.array([1, 1, 1, 1], np.int8)            # (1,-1) vs (1,1): tie -> kept
+    assert oracle.block_stitch(8, win3, [b0, b1f, b2t]).tolist() == [1, 1, 1, -1, 1, 1, 1, 1]
+
+
+# ------------------------------------------------------------------------------------- O3 dSB variant (SURVEY 8(f) f4)
+def test_dsb_force_uses_signs_only(oracle):
+    """PAPER.md:L71-L77 (dSB in the bake-off): the force is J sgn(x).  (i) J = 0: identical to bSB.  (ii) The increment of y
+    beyond the spin's own -dt (a0 - a_k) x term depends only on the SIGNS of the other spins: rescaling every |x_j| by an
+    arbitrary positive factor leaves it unchanged bit for bit (it would not under bSB).  (iii) hand values on two coupled
+    spins, including sgn(0) = +1.  (iv) while no sign changes, the step is an affine map: explicit matrix product."""
+    rp0 = np.zeros(4, np.int32); e = np.zeros(0, np.int32)
+    x0 = np.array([[0.3, -0.2], [0.05, 0.0], [-0.6, 0.4]]); y0 = np.array([[0.1, 0.2], [-0.3, 0.0], [0.2, -0.1]])
+    a = oracle.bsb_run(rp0, e, np.zeros(0, np.float32), x0.copy(), y0.copy(), steps_total=9, steps_run=4, c0=0.3, force_mode=1)
+    b = oracle.bsb_run(rp0, e, np.zeros(0, np.float32), x0.copy(), y0.copy(), steps_total=9, steps_run=4, c0=0.3, force_mode=0)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    rng = np.random.default_rng(2)
+    n, R, T, dt, a0, c0 = 7, 5, 30, 0.5, 1.0, 0.125
+    J = rng.integers(-3, 4, size=(n, n)).astype(np.float64); J = np.triu(J, 1); J = J + J.T
+    rp, cl, jv = csr_from_dense(J)
+    x = rng.uniform(-0.5, 0.5, size=(n, R)); y = rng.uniform(-0.1, 0.1, size=(n, R))
+    scale = 2.0 ** rng.integers(-3, 1, size=(n, R)).astype(np.float64)           # exact rescaling, signs kept
+    k = 11
+    a_k = a0 * k / (T - 1)
+    incs = []
+    for xs in (x, x * scale):
+        _, y1, _ = oracle.bsb_run(rp, cl, jv, xs.copy(), y.copy(), steps_total=T, step_begin=k, steps_run=1, dt=dt, a0=a0, c0=c0, force_mode=1)
+        incs.append(y1 - (y + dt * (-(a0 - a_k) * xs)))
+    clamped = np.abs(oracle.bsb_run(rp, cl, jv, x.copy(), y.copy(), steps_total=T, step_begin=k, steps_run=1, dt=dt, a0=a0, c0=c0, force_mode=1)[0]) == 1.0
+    assert not clamped.any()
+    np.testing.assert_allclose(incs[0], incs[1], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(incs[0], dt * c0 * (J @ np.where(x >= 0, 1.0, -1.0)), rtol=0, atol=1e-15)       # = dt c0 J sgn(x): library matmul
+    _, yb, _ = oracle.bsb_run(rp, cl, jv, (x * scale).copy(), y.copy(), steps_total=T, step_begin=k, steps_run=1, dt=dt, a0=a0, c0=c0, force_mode=0)
+    assert np.abs((yb - (y + dt * (-(a0 - a_k) * x * scale))) - incs[0]).max() > 1e-3                          # bSB does depend on |x|
+    # (iii) two spins, J01 = -2 (w = 2), x = (0, 0.5): sgn = (+1, +1) -> F = (-2, -2); T = 1 -> a_k = 0
+    rp2 = np.array([0, 1, 2], np.int32); cl2 = np.array([1, 0], np.int32); jv2 = np.array([-2, -2], np.float32)
+    x2, y2, _ = oracle.bsb_run(rp2, cl2, jv2, np.array([[0.0], [0.5]]), np.array([[0.0], [0.0]]), steps_total=1, dt=0.5, a0=1.0, c0=0.25, force_mode=1)
+    assert y2.tolist() == [[0.5 * 0.25 * -2.0], [0.5 * (-0.5 + 0.25 * -2.0)]] and x2.tolist() == [[0.5 * y2[0, 0]], [0.5 + 0.5 * y2[1, 0]]]
+    # (iv) antiferromagnetic pair pushed apart: signs (+, -) never change -> affine map z' = M z + b per step
+    x0 = np.array([[0.01], [-0.02]]); y0 = np.array([[0.0], [0.0]])
+    steps, T = 6, 50
+    xa, ya, _ = oracle.bsb_run(rp2, cl2, jv2, x0.copy(), y0.copy(), steps_total=T, steps_run=steps, dt=0.25, a0=1.0, c0=0.1, force_mode=1)
+    z = np.vstack([x0, y0, [[1.0]]])
+    Fc = 0.25 * 0.1 * (np.array([[0.0, -2.0], [-2.0, 0.0]]) @ np.array([[1.0], [-1.0]]))                     # dt c0 J s, constant
+    I = np.eye(2)
+    for k in range(steps):
+        B = -0.25 * (1.0 - k / (T - 1)) * I
+        Mk = np.block([[I + 0.25 * B, 0.25 * I, 0.25 * Fc], [B, I, Fc], [np.zeros((1, 4)), np.ones((1, 1))]])
+        z = Mk @ z
+    assert np.all(np.abs(xa) < 1.0) and xa[0, 0] > 0 > xa[1, 0]
+    np.testing.assert_allclose(np.vstack([xa, ya]), z[:4], rtol=1e-12, atol=1e-18)
+
+
+def test_eval_every_trace_is_the_cut_at_those_steps(oracle):
+    """PAPER.md:L118 (Fig. 3: energy of the best sample at every time step): the trace rows equal a fresh cut evaluation of
+    sign(x) after exactly that many steps (resume property P10), and the run with a trace ends in the same state."""
+    fr = tiny_fragments(21, n_snp=60, n_reads=40)
+    g = oracle.read_graph(fr)
+    w = oracle.read_weights(g, 1); jv = (-w).astype(np.float32)
+    x0, y0 = synth.bsb_init_state(5, fr.n_frag, 6)
+    T = 60
+    res = oracle.solve(g["row_ptr"], g["col"], w, jv, x0, y0, steps_total=T, eval_every=25)
+    ref = oracle.solve(g["row_ptr"], g["col"], w, jv, x0, y0, steps_total=T)
+    assert np.array_equal(res["x"], ref["x"]) and np.array_equal(res["cut"], ref["cut"])
+    assert res["trace_steps"].tolist() == [25, 50] and res["trace"].shape == (2, 6)
+    for row, k in zip(res["trace"], res["trace_steps"]):
+        xk, _, _ = oracle.bsb_run(g["row_ptr"], g["col"], jv, x0.astype(np.float64), y0.astype(np.float64), steps_total=T, steps_run=int(k))
+        assert np.array_equal(row, oracle.cut_eval(g["row_ptr"], g["col"], w, np.where(xk >= 0, 1, -1).astype(np.int8))[0])

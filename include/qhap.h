@@ -14,8 +14,11 @@
  *    *ws_bytes, launches nothing and returns QHAP_OK.  With workspace != NULL, *ws_bytes is the size provided;
  *    too small -> QHAP_ERR_WORKSPACE (and *ws_bytes = required).
  *  - all work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).  Entry points
- *    that return a count to the host (graph builds: nnz) synchronise the stream once; qhap_bsb_solve,
- *    qhap_cut_eval and the readouts are asynchronous: results are valid after the caller synchronises.
+ *    that return a count to the host synchronise the stream: the graph builds, qhap_block_split (nnz),
+ *    qhap_component_split (sizes), qhap_snp_refine (once per iteration) and qhap_bsb_solve on path 4 (its tile plan reads
+ *    one count back).  qhap_bsb_solve on paths 1-3, qhap_cut_eval, the readouts, qhap_block_stitch, qhap_gauge_transform,
+ *    qhap_flip_count_update, qhap_refine_readout and qhap_component_merge are asynchronous: results are valid after the
+ *    caller synchronises.
  *  - no global state, no hidden RNG, no CPU fallback: without an sm_100 device every call returns QHAP_ERR_CUDA.
  *  - qhap_last_error() returns a thread-local text for the last non-OK status.
  */
@@ -107,9 +110,32 @@ QHAP_API qhap_status qhap_build_snp_graph(const qhap_frags *frags, int32_t linka
 QHAP_API qhap_status qhap_build_snp_graph_fill(const qhap_frags *frags, int32_t linkage_tenths, double alpha, qhap_csr *out,
                                       void *workspace, size_t *ws_bytes, void *stream);
 
+/* Optional kernel tuning of qhap_bsb_solve (paths 1 and 4).  NULL, or a field left 0, means AUTOMATIC.  These knobs select
+ * launch shapes, shared-memory splits and cache policies; only `state16` can change result bits (documented there).  They
+ * live outside qhap_bsb_params so that the solver's parameter block does not change when a kernel is retuned. */
+typedef struct {
+  int32_t dense_bn;       /* path 1: tile width in output spins (multiple of 16 in 32..256)                              */
+  int32_t step_launch;    /* 1 = one launch per bSB step; automatic = ONE launch runs all steps_run steps when the tiles   */
+                          /*    allow and all CTAs can be co-resident (checked with the occupancy API).  Same bits           */
+  int32_t l2_hints;       /* L2 eviction priorities of the step kernel: 1 = on (the 16-bit copies of x evict_last, y          */
+                          /*    evict_first), 2 = off; automatic = on when the copies fit the L2                              */
+  int32_t dense_stg_bufs; /* shared-memory staging buffers for the 16-bit copies of x: 1 or 2                              */
+  int32_t dense_epi_sync; /* epilogue warps meet after every tile: 1 = yes, 2 = no                                          */
+  int32_t l2_keep_16ths;  /* with the hints on: the share q/16 (1..16) of the kept lines that gets evict_last              */
+  int32_t state16;        /* how x is carried BETWEEN the steps of one call on the tile paths (64-wide tiles):               */
+                          /*    automatic / 1 = as the pair of fp16 numbers the tensor cores read, 2^15 x = x_hi + x_lo      */
+                          /*    (16 B of HBM traffic per spin-update instead of 24; x is rounded to that pair, relative      */
+                          /*    2^-22, once per step instead of to fp32's 2^-24); 2 = in fp32.  The x returned to the caller */
+                          /*    is fp32 either way                                                                            */
+  int32_t bias_cancel;    /* 1 = every tile is accumulated twice, with x and with -x, and F = (D+ - D-) / 2: cancels the      */
+                          /*    sign-independent truncation bias of the tensor cores' fp32 accumulation (2x the MMAs)         */
+  int32_t reserved[8];    /* must be 0                                                                                      */
+} qhap_bsb_tuning;
+
 /* bSB parameters (PAPER.md:L265 gives the outline; constants from BASELINE.json; readings R10a-f):
  *   a_k = a0 k / (steps_total - 1), k = step_begin .. step_begin + steps_run - 1
- *   F = J x (x of the previous step);  y += dt (-(a0 - a_k) x + c0 F);  x += dt a0 y;  |x| > 1: x = sign(x), y = 0. */
+ *   F = J x (x of the previous step);  y += dt (-(a0 - a_k) x + c0 F);  x += dt a0 y;  |x| > 1: x = sign(x), y = 0.
+ * force_mode 1 (dSB, the discrete variant of the paper's bake-off): F = J sgn(x), sgn(0) = +1. */
 typedef struct {
   int32_t replicas;     /* R; x, y are [n][R] with the replica index contiguous                           */
   int32_t steps_total;  /* T of the ramp                                                                  */
@@ -126,23 +152,18 @@ typedef struct {
                         /*    same bits as path 2);                                                           */
                         /*  4 tcgen05 step on a block-compressed J built from the CSR (64 x 64 tiles; entries */
                         /*    of sparsely filled tiles -- long-range edges -- go through a remainder CSR      */
-                        /*    gather; batches allowed; the plan synchronises the stream once or a few times); */
-                        /*  0 auto: 3 if it fits, else 1 if dense_J is given, else 4 (2 below 1024 or above   */
-                        /*    2^20 vertices)                                                                  */
+                        /*    gather; batches allowed; the plan SYNCHRONISES the stream once or a few times); */
+                        /*  0 auto: 3 if it fits, else 1 if dense_J is given, else 4 (2 below 1024 vertices)   */
   int32_t tile_skip;    /* path 1: 1 = visit only the 64-column blocks of J that hold a non-zero (bit-identical) */
   int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
   int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */
-  int32_t dense_bn;     /* path 1: tile width in output spins (multiple of 16 in 32..256); 0 = automatic      */
-  int32_t step_launch;  /* paths 1, 4: 0 = automatic (ONE launch runs all steps_run steps when the tiles allow:    */
-                        /*    tiles of step k+1 start as soon as the tiles they read have finished step k);       */
-                        /*    1 = one launch per step.  Same bits either way                                      */
-  int32_t l2_hints;     /* paths 1, 4: L2 eviction priorities of the step kernel: 0 = automatic (x and its fp16     */
-                        /*    copies evict_last, y evict_first when 12 B x n x R fits the L2), 1 = on, 2 = off        */
-  int32_t dense_stg_bufs; /* paths 1, 4 (tuning): shared-memory staging buffers for the fp16 copies: 0 = automatic, 1, 2 */
-  int32_t dense_epi_sync; /* paths 1, 4 (tuning): epilogue warps meet after every tile: 0 = automatic, 1 = yes, 2 = no  */
-  int32_t l2_keep_16ths;  /* paths 1, 4 (tuning): with the hints on, the share q/16 (1..16) of the lines of x and its fp16   */
-                        /*    copies that gets evict_last (the rest evict_first, like y): a keep set larger than the L2 thrashes   */
-                        /*    as a whole, a fixed fraction of it stays; 0 = automatic = 16 (measured: DESIGN.md 4.4e)           */
+  int32_t force_mode;   /* 0 = bSB (F = J x, the paper's solver, L265); 1 = dSB (F = J sgn(x), L71-L77)     */
+  int32_t eval_every;   /* k > 0: after every k-th step of this call (steps step_begin + k, + 2k, ...) the cut of sgn(x)   */
+                        /*    of every replica is evaluated -- what Fig. 3 plots per time step -- and      */
+                        /*    written to the trace arrays below, row j = after step_begin + (j + 1) k steps; 0 = never      */
+  int64_t *trace_cut;      /* DEVICE [steps_run / k][n_inst][R] or NULL                                                       */
+  int64_t *trace_best_cut; /* DEVICE [steps_run / k][n_inst]: max over the replicas (min energy, E = W_tot - 2 cut), or NULL */
+  const qhap_bsb_tuning *tuning;   /* HOST, optional (NULL = automatic)                                                      */
 } qhap_bsb_params;
 
 /* (3)+(4)+(5) bSB solve of `n_inst` independent instances stored as ONE block-diagonal CSR `graph`

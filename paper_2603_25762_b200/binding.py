@@ -41,11 +41,30 @@ class _Csr(C.Structure):
                 ("c", C.c_void_p), ("w_fx", C.c_void_p), ("w", C.c_void_p)]
 
 
+class _BsbTuning(C.Structure):
+    _fields_ = [("dense_bn", C.c_int32), ("step_launch", C.c_int32), ("l2_hints", C.c_int32), ("dense_stg_bufs", C.c_int32),
+                ("dense_epi_sync", C.c_int32), ("l2_keep_16ths", C.c_int32), ("state16", C.c_int32), ("bias_cancel", C.c_int32), ("reserved", C.c_int32 * 8)]
+
+
 class _BsbParams(C.Structure):
     _fields_ = [("replicas", C.c_int32), ("steps_total", C.c_int32), ("step_begin", C.c_int32), ("steps_run", C.c_int32),
                 ("dt", C.c_double), ("a0", C.c_double), ("c0", C.c_double), ("seed", C.c_uint64),
                 ("weight_mode", C.c_int32), ("path", C.c_int32), ("tile_skip", C.c_int32), ("init_state", C.c_int32),
-                ("finalize", C.c_int32), ("dense_bn", C.c_int32), ("step_launch", C.c_int32), ("l2_hints", C.c_int32), ("dense_stg_bufs", C.c_int32), ("dense_epi_sync", C.c_int32), ("l2_keep_16ths", C.c_int32)]
+                ("finalize", C.c_int32), ("force_mode", C.c_int32), ("eval_every", C.c_int32),
+                ("trace_cut", C.c_void_p), ("trace_best_cut", C.c_void_p), ("tuning", C.POINTER(_BsbTuning))]
+
+
+TUNING_KEYS = ("dense_bn", "step_launch", "l2_hints", "dense_stg_bufs", "dense_epi_sync", "l2_keep_16ths", "state16", "bias_cancel")
+
+
+def _tuning(kw: dict):
+    """qhap_bsb_tuning from keyword arguments (None when every knob is automatic)."""
+    if not any(kw.get(k) for k in TUNING_KEYS):
+        return None
+    t = _BsbTuning()
+    for k in TUNING_KEYS:
+        setattr(t, k, int(kw.get(k) or 0))
+    return t
 
 
 for _name in EXPORTS[:15]:
@@ -279,11 +298,17 @@ def qhap_block_split(graph: Csr, windows: np.ndarray) -> Csr:
 
 def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: int = 0, steps_run: Optional[int] = None,
                    dt: float = 1.25, a0: float = 1.0, c0: float = 0.0, seed: int = 0, weight_mode: int = QHAP_WEIGHT_D,
-                   path: int = 0, tile_skip: int = 0, dense_bn: int = 0, step_launch: int = 0, l2_hints: int = 0, dense_stg_bufs: int = 0, dense_epi_sync: int = 0, l2_keep_16ths: int = 0, x: Optional[torch.Tensor] = None, y: Optional[torch.Tensor] = None,
+                   path: int = 0, tile_skip: int = 0, force_mode: int = 0, eval_every: int = 0, trace_cuts: bool = False,
+                   x: Optional[torch.Tensor] = None, y: Optional[torch.Tensor] = None,
                    dense_J: Optional[torch.Tensor] = None, finalize: bool = True, cut_per_replica: bool = True,
-                   workspace: Optional[torch.Tensor] = None) -> dict:
-    """(3)(4)(5) bSB solve.  x, y: [n][R] fp32 CUDA tensors updated in place; None -> seeded on the device."""
+                   workspace: Optional[torch.Tensor] = None, **tuning) -> dict:
+    """(3)(4)(5) bSB solve.  x, y: [n][R] fp32 CUDA tensors updated in place; None -> seeded on the device.
+    Keyword arguments named like the fields of qhap_bsb_tuning (dense_bn, step_launch, l2_hints, ..., state16) fill that
+    optional block; eval_every = k > 0 returns `trace_best_cut` [steps_run // k][n_inst] (and `trace_cut` [..][n_inst][R]
+    with trace_cuts=True)."""
     dev = _dev()
+    unknown = set(tuning) - set(TUNING_KEYS)
+    assert not unknown, f"unknown arguments {sorted(unknown)}"
     n, R = graph.n, int(replicas)
     init = x is None
     if init:
@@ -295,8 +320,13 @@ def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: i
     inst_ptr = graph.inst_ptr
     n_inst = 1 if inst_ptr is None else len(inst_ptr) - 1
     ip = np.ascontiguousarray(inst_ptr, dtype=np.int32) if inst_ptr is not None else None
+    n_eval = steps_run // eval_every if eval_every > 0 else 0
+    tr_best = torch.empty((n_eval, n_inst), dtype=torch.int64, device=dev) if n_eval else None
+    tr_cut = torch.empty((n_eval, n_inst, R), dtype=torch.int64, device=dev) if (n_eval and trace_cuts) else None
+    tun = _tuning(tuning)
     p = _BsbParams(R, steps_total, step_begin, steps_run, dt, a0, c0, seed, weight_mode, path, tile_skip, int(init),
-                   int(finalize), int(dense_bn), int(step_launch), int(l2_hints), int(dense_stg_bufs), int(dense_epi_sync), int(l2_keep_16ths))
+                   int(finalize), int(force_mode), int(eval_every), tr_cut.data_ptr() if tr_cut is not None else None,
+                   tr_best.data_ptr() if tr_best is not None else None, C.pointer(tun) if tun is not None else None)
     gs = graph.c_struct()
     dd = QHAP_DENSE_NONE
     ld = 0
@@ -319,7 +349,7 @@ def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: i
     ws_bytes = C.c_size_t(workspace.numel())
     _check(call(_ptr(workspace), C.byref(ws_bytes)), "qhap_bsb_solve")
     return dict(x=x, y=y, best_spins=best_spins[:n] if finalize else None, best_cut=best_cut, best_replica=best_rep,
-                cut=cuts, workspace=workspace)
+                cut=cuts, workspace=workspace, trace_best_cut=tr_best, trace_cut=tr_cut, workspace_bytes=int(ws_bytes.value))
 
 
 def qhap_cut_eval(graph: Csr, weight_mode: int, spins: torch.Tensor, want_energy: bool = True):
@@ -417,7 +447,7 @@ def qhap_snp_refine(graph: Csr, *, replicas: int, steps_total: int, max_iter: in
     x = torch.empty((n, R), dtype=torch.float32, device=dev)
     y = torch.empty((n, R), dtype=torch.float32, device=dev)
     flip = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
-    p = _BsbParams(R, steps_total, 0, steps_total, dt, a0, c0, seed, QHAP_WEIGHT_FX, path, 0, 1, 1, 0)
+    p = _BsbParams(R, steps_total, 0, steps_total, dt, a0, c0, seed, QHAP_WEIGHT_FX, path, 0, 1, 1, 0, 0, None, None, None)
     gs = graph.c_struct()
     iters = C.c_int32(0)
     cuts = (C.c_int64 * max_iter)()

@@ -41,6 +41,7 @@ constexpr int kStoreWarp = 2 + kEpiWarps;  // one lane: TMA stores of the fp16 c
 constexpr int kThreads = 32 * (kStoreWarp + 1);
 constexpr int kRingSlot = kChunk * 32 * 4;           // one work item of x (or y): 8 spins x 32 replicas fp32 = 1 KB
 constexpr int kRingBytes = kEpiWarps * 2 * 2 * kRingSlot;   // per warp: 2 slots x (x, y)
+constexpr int kRingBytes16 = kEpiWarps * 2 * kRingSlot;     // state16: per warp 2 slots x (y)
 constexpr int kTmemCols = 512;                       // 2 accumulator stages x 256 columns
 constexpr size_t kSmemBytes = size_t(kSmemBudget) + 1024 /*alignment slack*/ + 1024 /*barriers*/;
 
@@ -81,6 +82,15 @@ struct DenseArgs {
                               // and by a single staging buffer); 0: epilogue thread 0 issues them behind a named barrier
   uint32_t epi_sync;          // 1: the epilogue warps meet at a named barrier after every tile
   uint32_t stg_bufs;          // staging buffers of (x_hi', x_lo') tiles: 2, or 1 to free 32 KB for another operand stage
+  // state16 (X16 kernels): between the steps of a call x lives ONLY as the fp16 pair the tensor cores read (2^15 x = x_hi + x_lo,
+  // [R][n_k] arrays); the tile's own pair arrives in the staging buffer by TMA, is updated IN PLACE and leaves by TMA store.
+  // The fp32 x array is not touched by the step kernel (split before the first step, merged after the last).
+  int32_t x16;
+  int32_t dsb;                // dSB: the copies hold 2^15 sgn(x) (x_lo = 0), so F = J sgn(x)
+  // bias cancellation: the tcgen05 fp32 accumulation truncates toward -inf, a bias of a few ulp of F that does not depend on
+  // the sign of F.  A second accumulator (128 TMEM columns further) receives the same MMAs with the A operand negated by the
+  // instruction descriptor: D- = -F + bias, D+ = F + bias, and the epilogue uses (D+ - D-) / 2.  Needs BN <= 128 and the ring.
+  int32_t bc;
 };
 
 // c2 = fp32(dt (a0 - a_k)), a_k = a0 k / (T - 1): the same individually rounded fp64 operations as the host loop
@@ -101,6 +111,22 @@ __device__ __forceinline__ void split_half(float v, __half& hi, __half& lo) {
   lo = __float2half_rn(vs - __half2float(hi));
 }
 
+// state16: the pair IS the state, so it must be a fixed point of the split: (h, l) == split((h + l) 2^-15).  rn(xs - h) can
+// round up to exactly half an ulp of h, and h + l then re-splits to the neighbouring (h', l') with the same sum; splitting
+// the (exact) sum once more gives the canonical pair, for which x fp32 -> pair -> x fp32 -> pair reproduces itself, so a
+// resumed call continues bit for bit.
+__device__ __forceinline__ void split_half_canonical(float v, __half& hi, __half& lo) {
+  __half h, l;
+  split_half(v, h, l);
+  const float s2 = __half2float(h) + __half2float(l);      // exact: at most 23 significant bits
+  hi = __float2half_rn(s2);
+  lo = __float2half_rn(s2 - __half2float(hi));              // exact
+}
+__device__ __forceinline__ void split_sign(float v, __half& hi, __half& lo) {     // dSB operand: 2^15 sgn(x), sgn(0) = +1
+  hi = __float2half_rn(v >= 0.f ? kXScale : -kXScale);
+  lo = __float2half_rn(0.f);
+}
+
 struct EpiConsts {
   float c1, c2, c3;
   int lane_r;            // replica of this thread inside the tile
@@ -115,9 +141,12 @@ __device__ __forceinline__ void epi_point(const EpiConsts& ec, float c1, float F
     yn = 0.0f;
   }
 }
+template <int MODE>   // 0: fp32-x kernels, 1: dSB sign copies, 2: state16 canonical pair
 __device__ __forceinline__ void epi_pack(int j, float xn, uint32_t (&hp)[kChunk / 2], uint32_t (&lp)[kChunk / 2]) {
   __half h, l;
-  split_half(xn, h, l);
+  if constexpr (MODE == 2) split_half_canonical(xn, h, l);
+  else if constexpr (MODE == 1) split_sign(xn, h, l);
+  else split_half(xn, h, l);
   const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
   if (j & 1) { hp[j >> 1] |= hb << 16; lp[j >> 1] |= lb << 16; }
   else       { hp[j >> 1] = hb;        lp[j >> 1] = lb; }
@@ -171,7 +200,7 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
         a.x[off] = xn;
         a.y[off] = yn;
       }
-      epi_pack(j, xn, hp, lp);
+      if (a.dsb) epi_pack<1>(j, xn, hp, lp); else epi_pack<0>(j, xn, hp, lp);
     }
   } else {
 #pragma unroll
@@ -184,7 +213,7 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
         ptx::st_global_f32_hint(a.x + off, xn, a.pol_keep);
         ptx::st_global_f32_hint(a.y + off, yn, a.pol_stream);
       }
-      epi_pack(j, ok ? xn : 0.f, hp, lp);
+      if (a.dsb && ok) epi_pack<1>(j, xn, hp, lp); else epi_pack<0>(j, ok ? xn : 0.f, hp, lp);
     }
   }
   if (stg != 0) {
@@ -209,10 +238,48 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
   }
 }
 
+// state16: one work item (kChunk spins x this thread's replica).  x comes from the tile's own (x_hi, x_lo) in the staging
+// buffer `stg` (TMA-loaded, 128-byte swizzle: 16-byte piece p of row r sits at piece p ^ (r & 7)), x = (x_hi + x_lo) 2^-15
+// exactly; the new canonical pair goes back to the SAME 16 bytes (this thread is their only reader and writer), y' to global.
+// Rows / replicas outside the problem arrive as zeros (TMA fill), stay zero (F = 0 there) and are clipped by the TMA store.
+template <bool hints>
+__device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, const uint32_t (&v)[kChunk],
+                                               const float (&yv)[kChunk], uint32_t stg) {
+  const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+  const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
+  const bool r_ok = r < a.R;
+  const int row = ec.lane_r;
+  static_assert(kChunk == 8, "one work item = one 16-byte piece of the swizzled staging row");
+  const uint32_t addr = stg + uint32_t(row) * 128u + ((uint32_t(ch) ^ uint32_t(row & 7)) << 4);
+  uint32_t hq[4], lq[4];
+  ptx::ld_shared_v4(addr, hq[0], hq[1], hq[2], hq[3]);
+  ptx::ld_shared_v4(addr + kStageX, lq[0], lq[1], lq[2], lq[3]);
+  uint32_t hp[kChunk / 2], lp[kChunk / 2];
+  uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
+  const bool interior = r_ok && i0 + kChunk <= a.n;
+#pragma unroll
+  for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
+    const uint32_t hb = (j & 1) ? (hq[j >> 1] >> 16) : (hq[j >> 1] & 0xffffu);
+    const uint32_t lb = (j & 1) ? (lq[j >> 1] >> 16) : (lq[j >> 1] & 0xffffu);
+    const float x = (__half2float(__ushort_as_half((unsigned short)hb)) + __half2float(__ushort_as_half((unsigned short)lb))) * (1.0f / kXScale);
+    const bool ok = interior || (r_ok && (i0 + j) < a.n);
+    const float c1 = (a.c1_per_row && (interior || (i0 + j) < a.n)) ? __ldg(a.c1 + i0 + j) : ec.c1;
+    float xn, yn;
+    epi_point(ec, c1, __uint_as_float(v[j]), x, yv[j], xn, yn);
+    if (ok) {
+      if constexpr (hints) ptx::st_global_f32_hint(a.y + off, yn, a.pol_stream);
+      else a.y[off] = yn;
+    }
+    epi_pack<2>(j, ok ? xn : 0.f, hp, lp);
+  }
+  ptx::st_shared_v4(addr, hp[0], hp[1], hp[2], hp[3]);
+  ptx::st_shared_v4(addr + kStageX, lp[0], lp[1], lp[2], lp[3]);
+}
+
 // RING: the fp32 state arrives through the per-warp TMA ring; HINTS: L2 eviction priorities on every state access.
 // Compile-time variants keep each instantiation's hot loops small (the single run-time kernel had grown from 63 to 88 KB
 // of SASS and cost cfg3 3 %).
-template <bool RING, bool HINTS>
+template <bool RING, bool HINTS, bool X16>
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
                   const __grid_constant__ CUtensorMap tm_xh,
@@ -233,6 +300,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   auto ring_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 6 + s); };
   auto stg_full = [&](uint32_t b) { return bar_base + 8u * (2 * kMaxStages + 6 + 2 * kEpiWarps + b); };       // staging tile b written
   auto stg_empty = [&](uint32_t b) { return bar_base + 8u * (2 * kMaxStages + 8 + 2 * kEpiWarps + b); };      // ... read by its TMA store
+  auto stg_in = [&](uint32_t b) { return bar_base + 8u * (2 * kMaxStages + 10 + 2 * kEpiWarps + b); };        // state16: the tile's own pair has arrived
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && ptx::elect_one()) {
@@ -253,6 +321,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     for (uint32_t b = 0; b < 2; ++b) {
       ptx::mbar_init(stg_full(b), kEpiWarps);
       ptx::mbar_init(stg_empty(b), 1);
+      ptx::mbar_init(stg_in(b), 1);
     }
     ptx::fence_barrier_init();
   }
@@ -343,7 +412,13 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           const uint64_t dl = ptx::umma_desc_k_sw128(sj + kStageJ + kStageX);
           // UMMA_K = 16 for 16-bit inputs: +32 B per step.  Two straight-line variants: a test of j_terms inside the
           // unrolled issue sequence costs the full GEMM 12 % (measured: 165 -> 186 us per step at cfg1).
-          if (a.j_terms == 2) {
+          if (a.dsb) {                    // dSB: the operand is 2^15 sgn(x), x_lo = 0 -> one MMA per J term and k-slice
+#pragma unroll
+            for (int kk = 0; kk < kBK / 16; ++kk) {
+              ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+              if (a.j_terms == 2) ptx::umma_f16(d_tmem, dh + 2u * kk, djl + 2u * kk, idesc, 1u);
+            }
+          } else if (a.j_terms == 2) {
 #pragma unroll
             for (int kk = 0; kk < kBK / 16; ++kk) {
               ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
@@ -355,6 +430,23 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
             for (int kk = 0; kk < kBK / 16; ++kk) {
               ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
               ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
+            }
+          }
+          if (a.bc) {                     // the same MMAs once more with -A into the second accumulator
+            const uint32_t idn = idesc | (1u << 13), dn = d_tmem + 128u;
+            if (a.j_terms == 2) {
+#pragma unroll
+              for (int kk = 0; kk < kBK / 16; ++kk) {
+                ptx::umma_f16(dn, dh + 2u * kk, dj + 2u * kk, idn, (j | kk) != 0);
+                ptx::umma_f16(dn, dl + 2u * kk, dj + 2u * kk, idn, 1u);
+                ptx::umma_f16(dn, dh + 2u * kk, djl + 2u * kk, idn, 1u);
+              }
+            } else {
+#pragma unroll
+              for (int kk = 0; kk < kBK / 16; ++kk) {
+                ptx::umma_f16(dn, dh + 2u * kk, dj + 2u * kk, idn, (j | kk) != 0);
+                ptx::umma_f16(dn, dl + 2u * kk, dj + 2u * kk, idn, 1u);
+              }
             }
           }
           ptx::umma_commit(empty_bar(stage));                            // frees the smem stage when these MMAs are done
@@ -373,6 +465,34 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     if (a.stage_out && a.store_warp && lane == 0) {
       const uint32_t stg_base = smem_base + uint32_t(kStages) * kStageBytes;
       uint32_t b = 0, bpar = 0;
+      // state16: this thread also brings each tile's OWN (x_hi, x_lo) into the staging buffer, stg_bufs tiles ahead; the
+      // epilogue updates the buffer in place and the store below writes it to the other copy.  A buffer is reloaded right
+      // after its store has read it.  Fused steps: the tile's own pair of step s - 1 was stored (and waited for with
+      // wait_group 0) by this same thread at least stg_bufs tiles earlier -- every CTA has >= 2 tiles per step.
+      int vt_ld = blockIdx.x;
+      uint32_t b_ld = 0;
+      auto load_next = [&]() {
+        while (vt_ld < vt_end) {
+          const int s = vt_ld / stride, tile = vt_ld - s * stride;
+          if (tile >= n_tiles) { vt_ld += gridDim.x; continue; }
+          const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+          const uint32_t stg = stg_base + b_ld * (2u * kStageX);
+          ptx::mbar_arrive_expect_tx(stg_in(b_ld), 2u * kStageX);
+          if constexpr (HINTS) {
+            ptx::tma_load_2d_hint(stg, (s & 1) ? &tm_oh : &tm_xh, stg_in(b_ld), tn * a.BN, tm * kBM, a.pol_keep);
+            ptx::tma_load_2d_hint(stg + kStageX, (s & 1) ? &tm_ol : &tm_xl, stg_in(b_ld), tn * a.BN, tm * kBM, a.pol_keep);
+          } else {
+            ptx::tma_load_2d(stg, (s & 1) ? &tm_oh : &tm_xh, stg_in(b_ld), tn * a.BN, tm * kBM);
+            ptx::tma_load_2d(stg + kStageX, (s & 1) ? &tm_ol : &tm_xl, stg_in(b_ld), tn * a.BN, tm * kBM);
+          }
+          vt_ld += gridDim.x;
+          if (++b_ld == a.stg_bufs) b_ld = 0;
+          return;
+        }
+      };
+      if constexpr (X16) {
+        for (uint32_t q = 0; q < a.stg_bufs; ++q) load_next();
+      }
       for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
         const int s = vt / stride, tile = vt - s * stride;
         if (tile >= n_tiles) continue;
@@ -388,11 +508,12 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         }
         ptx::tma_store_commit();
         ptx::tma_store_wait_read_all();
-        ptx::mbar_arrive(stg_empty(b));
+        if constexpr (!X16) ptx::mbar_arrive(stg_empty(b));
         if (a.fused) {
           ptx::tma_store_wait_all();
           ptx::signal_add_release(a.done + tile, 1u);
         }
+        if constexpr (X16) load_next();            // into the buffer just read (b_ld == b)
         if (++b == a.stg_bufs) { b = 0; bpar ^= 1u; }
       }
     }
@@ -504,15 +625,20 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       // State through TMA: every warp owns two 2 KB slots (x and y of one work item: a box of 8 spins x 32 replicas
       // each).  The item two ahead is requested as soon as the current item's values are in registers, so the loads
       // need no registers, no address arithmetic and no LSU slots; out-of-range rows / replicas arrive as zeros.
-      const uint32_t ring_w = stg_base + a.stg_bufs * (2u * kStageX) + uint32_t(ew) * (4u * kRingSlot);
+      // (state16: y only -- x is the tile's own fp16 pair in the staging buffer)
+      constexpr uint32_t kSlotBytes = X16 ? uint32_t(kRingSlot) : 2u * kRingSlot;
+      const uint32_t ring_w = stg_base + a.stg_bufs * (2u * kStageX) + uint32_t(ew) * (2u * kSlotBytes);
       const uint32_t rbar0 = ring_bar(2 * ew);
       auto issue = [&](const Pos& p, int slot) {
         if (ptx::elect_one()) {
           const int ch = p.ch;
           const int tn = p.rt / a.n_tiles_m, tm = p.rt % a.n_tiles_m;
-          const uint32_t dst = ring_w + uint32_t(slot) * (2u * kRingSlot);
-          ptx::mbar_arrive_expect_tx(rbar0 + 8u * slot, 2u * kRingSlot);
-          if constexpr (HINTS) {
+          const uint32_t dst = ring_w + uint32_t(slot) * kSlotBytes;
+          ptx::mbar_arrive_expect_tx(rbar0 + 8u * slot, kSlotBytes);
+          if constexpr (X16) {
+            if constexpr (HINTS) ptx::tma_load_2d_hint(dst, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk, a.pol_stream);
+            else ptx::tma_load_2d(dst, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk);
+          } else if constexpr (HINTS) {
             ptx::tma_load_2d_hint(dst, &tm_sx, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk, a.pol_keep);
             ptx::tma_load_2d_hint(dst + kRingSlot, &tm_sy, rbar0 + 8u * slot, tm * kBM + quarter * 32, tn * a.BN + ch * kChunk, a.pol_stream);
           } else {
@@ -535,21 +661,42 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if (p0.ch == par) tile_begin();
         uint32_t v[kChunk];
         ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p0.ch * kChunk), v);
+        uint32_t vneg[kChunk];
+        if (a.bc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p0.ch * kChunk), vneg);
         ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
         float xv[kChunk], yv[kChunk];
-        const uint32_t src = ring_w + uint32_t(slot) * (2u * kRingSlot) + uint32_t(lane) * 4u;
+        const uint32_t src = ring_w + uint32_t(slot) * kSlotBytes + uint32_t(lane) * 4u;
 #pragma unroll
         for (int j = 0; j < kChunk; ++j) {
-          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(xv[j]) : "r"(src + uint32_t(j) * 128u));
-          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
+          if constexpr (X16) {
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + uint32_t(j) * 128u));
+          } else {
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(xv[j]) : "r"(src + uint32_t(j) * 128u));
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
+          }
         }
         __syncwarp();                            // every lane has its values: the slot may be refilled
         if (p1.vt < vt_end && p2.vt < vt_end) issue(p2, slot);
-        ptx::tmem_ld_wait();
         const uint32_t stg = a.stage_out ? stg_base + stg_i * (2u * kStageX) : 0u;
-        if (p0.ch == par) staging_free();
-        set_step(p0.vt);
-        epi_update_store<HINTS>(a, ec, p0.rt, p0.ch, v, xv, yv, stg);
+        if constexpr (X16) {
+          if (p0.ch == par) ptx::mbar_wait(stg_in(stg_i), stg_par);      // the tile's own (x_hi, x_lo) has arrived
+          ptx::tmem_ld_wait();
+          if (a.bc) {
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(0.5f * (__uint_as_float(v[j]) - __uint_as_float(vneg[j])));
+          }
+          set_step(p0.vt);
+          epi_update_x16<HINTS>(a, ec, p0.rt, p0.ch, v, yv, stg);
+        } else {
+          ptx::tmem_ld_wait();
+          if (a.bc) {
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(0.5f * (__uint_as_float(v[j]) - __uint_as_float(vneg[j])));
+          }
+          if (p0.ch == par) staging_free();
+          set_step(p0.vt);
+          epi_update_store<HINTS>(a, ec, p0.rt, p0.ch, v, xv, yv, stg);
+        }
         cur_rt = p0.rt;
         if (p1.vt != p0.vt) tile_done();
         p0 = p1; p1 = p2;
@@ -579,7 +726,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
 }
 
 // x [n][R] fp32 -> split copies [R][n_k] fp16 (transpose through shared memory, 32 x 32 tiles).
-__global__ void __launch_bounds__(256) split_x_kernel(int32_t n, int32_t R, int32_t n_k, const float* __restrict__ x,
+// mode 0: plain split (fp32-x kernels); 1: dSB sign copies; 2: canonical pair (state16).
+__global__ void __launch_bounds__(256) split_x_kernel(int32_t n, int32_t R, int32_t n_k, int32_t mode, const float* __restrict__ x,
                                                       __half* __restrict__ xh, __half* __restrict__ xl) {
   __shared__ float t[32][33];
   const int i0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
@@ -593,10 +741,29 @@ __global__ void __launch_bounds__(256) split_x_kernel(int32_t n, int32_t R, int3
     const int r = r0 + j, i = i0 + tx;
     if (r < R && i < n_k) {
       __half h, l;
-      split_half(t[tx][j], h, l);
+      if (mode == 2) split_half_canonical(t[tx][j], h, l);
+      else if (mode == 1 && i < n) split_sign(t[tx][j], h, l);
+      else split_half(t[tx][j], h, l);
       xh[size_t(r) * n_k + i] = h;
       xl[size_t(r) * n_k + i] = l;
     }
+  }
+}
+
+// state16, after the last step of a call: x[i][r] = (x_hi[r][i] + x_lo[r][i]) 2^-15 (exact in fp32).
+__global__ void __launch_bounds__(256) merge_x_kernel(int32_t n, int32_t R, int32_t n_k, const __half* __restrict__ xh,
+                                                      const __half* __restrict__ xl, float* __restrict__ x) {
+  __shared__ float t[32][33];
+  const int i0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int j = ty; j < 32; j += 8) {
+    const int r = r0 + j, i = i0 + tx;
+    t[j][tx] = (r < R && i < n) ? (__half2float(xh[size_t(r) * n_k + i]) + __half2float(xl[size_t(r) * n_k + i])) * (1.0f / kXScale) : 0.f;
+  }
+  __syncthreads();
+  for (int j = ty; j < 32; j += 8) {
+    const int i = i0 + j, r = r0 + tx;
+    if (i < n && r < R) x[size_t(i) * R + r] = t[tx][j];
   }
 }
 
@@ -616,7 +783,7 @@ __global__ void __launch_bounds__(256) kb_flag_kernel(int32_t n, const int32_t* 
 }
 
 // One CTA per N tile: ascending list of flagged k-blocks (at least one entry, so that every tile produces an accumulator).
-__global__ void __launch_bounds__(32) kb_list_kernel(int32_t n_kblocks, const int32_t* __restrict__ flag, int32_t* __restrict__ kb_cnt,
+__global__ void __launch_bounds__(32) kb_list_kernel(int32_t n_kblocks, int32_t BN, const int32_t* __restrict__ flag, int32_t* __restrict__ kb_cnt,
                                                      int32_t* __restrict__ kb_idx) {
   const int tn = blockIdx.x, lane = threadIdx.x;
   const int32_t* f = flag + size_t(tn) * n_kblocks;
@@ -630,7 +797,9 @@ __global__ void __launch_bounds__(32) kb_list_kernel(int32_t n_kblocks, const in
     cnt += __popc(m);
   }
   if (lane == 0) {
-    if (cnt == 0) { out[0] = 0; cnt = 1; }
+    // an empty tile row lists the k-block of its own first row: for BN == kBK that is its diagonal block, which keeps the
+    // lists symmetric (fused steps: "tn lists kb <=> kb lists tn") and is ordered against itself by the owning CTA
+    if (cnt == 0) { out[0] = min(n_kblocks - 1, int32_t((int64_t(tn) * BN) / kBK)); cnt = 1; }
     kb_cnt[tn] = cnt;
   }
 }
@@ -744,7 +913,10 @@ __global__ void __launch_bounds__(256) remainder_kernel(int32_t n, const int32_t
 // y += c1[instance] * sum over the row's remainder entries of J x_old  -- one warp per row, lanes across replicas
 // (float4), rows without remainder entries cost one row_ptr read.  Runs BEFORE the tile step of the same bSB step, on the
 // fp32 x that step will then update in place; the tile step's fma(c1, F_tiles, fma(-c2, x, y)) completes the sum.
-__global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t R, const int32_t* __restrict__ rem_ptr,
+__device__ __forceinline__ float4 sgn4(float4 v) {
+  return make_float4(v.x >= 0.f ? 1.f : -1.f, v.y >= 0.f ? 1.f : -1.f, v.z >= 0.f ? 1.f : -1.f, v.w >= 0.f ? 1.f : -1.f);
+}
+__global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t R, int32_t dsb, const int32_t* __restrict__ rem_ptr,
                                                              const int32_t* __restrict__ rem_col, const float* __restrict__ rem_val,
                                                              const float* __restrict__ c1row_plain, const float* __restrict__ x,
                                                              float* __restrict__ y) {
@@ -765,6 +937,7 @@ __global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t 
         for (int q = 0; q < 4; ++q) {
           v[q] = __ldg(rem_val + e + q);
           xv[q] = *reinterpret_cast<const float4*>(x + size_t(__ldg(rem_col + e + q)) * R + r);
+          if (dsb) xv[q] = sgn4(xv[q]);
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
@@ -773,7 +946,8 @@ __global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t 
       }
       for (; e < e1; ++e) {
         const float v = __ldg(rem_val + e);
-        const float4 xv = *reinterpret_cast<const float4*>(x + size_t(__ldg(rem_col + e)) * R + r);
+        float4 xv = *reinterpret_cast<const float4*>(x + size_t(__ldg(rem_col + e)) * R + r);
+        if (dsb) xv = sgn4(xv);
         F.x = fmaf(v, xv.x, F.x); F.y = fmaf(v, xv.y, F.y); F.z = fmaf(v, xv.z, F.z); F.w = fmaf(v, xv.w, F.w);
       }
       float4* py = reinterpret_cast<float4*>(y + size_t(a) * R + r);
@@ -783,7 +957,10 @@ __global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t 
     } else {
       for (int32_t rr = r; rr < min(r + 4, R); ++rr) {
         float F = 0.f;
-        for (int32_t e = e0; e < e1; ++e) F = fmaf(__ldg(rem_val + e), x[size_t(__ldg(rem_col + e)) * R + rr], F);
+        for (int32_t e = e0; e < e1; ++e) {
+          const float xj = x[size_t(__ldg(rem_col + e)) * R + rr];
+          F = fmaf(__ldg(rem_val + e), dsb ? (xj >= 0.f ? 1.f : -1.f) : xj, F);
+        }
         y[size_t(a) * R + rr] = fmaf(c1, F, y[size_t(a) * R + rr]);
       }
     }
@@ -817,7 +994,19 @@ __global__ void __launch_bounds__(256) block_fill_kernel(int32_t n, const int32_
 }
 
 // ------------------------------------------------------------------------------------------- host side
-// One step launch with the programmatic-stream-serialization attribute (see the kernel: griddepcontrol.wait).
+// Kernel variant of a launch: RING (fp32 state through the TMA ring) x HINTS (L2 eviction priorities) x X16 (state16).
+typedef void (*StepKernel)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const CUtensorMap, const CUtensorMap,
+                           const CUtensorMap, const CUtensorMap, const CUtensorMap, const DenseArgs);
+StepKernel step_kernel_of(const DenseArgs& a) {
+  const bool hints = a.pol_keep != ptx::kEvictNormal;
+  if (a.x16) return hints ? dense_step_kernel<true, true, true> : dense_step_kernel<true, false, true>;
+  if (a.ring) return hints ? dense_step_kernel<true, true, false> : dense_step_kernel<true, false, false>;
+  return hints ? dense_step_kernel<false, true, false> : dense_step_kernel<false, false, false>;
+}
+
+// One launch of the step kernel.  Per-step launches carry the programmatic-stream-serialization attribute (see the
+// kernel: griddepcontrol.wait); a fused launch (its CTAs wait for each other's tiles) is a COOPERATIVE launch, so the
+// driver guarantees that all of its CTAs are co-resident whatever else runs on the device.
 qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, const CUtensorMap& tjl, const CUtensorMap& th,
                         const CUtensorMap& tl, const CUtensorMap& toh, const CUtensorMap& tol, const CUtensorMap& tsx,
                         const CUtensorMap& tsy, const DenseArgs& a) {
@@ -827,63 +1016,70 @@ qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, co
   cfg.dynamicSmemBytes = kSmemBytes;
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  if (a.fused) {
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+  } else {
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+  }
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  const bool hints = a.pol_keep != ptx::kEvictNormal;
-  auto go = [&](auto kernel) -> qhap_status {
-    // per device and cheap: set on every call (a process may drive several devices)
-    QHAP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
-    QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, tj, tjl, th, tl, toh, tol, tsx, tsy, a));
-    return QHAP_OK;
-  };
-  if (a.ring) QHAP_TRY(hints ? go(dense_step_kernel<true, true>) : go(dense_step_kernel<true, false>));
-  else QHAP_TRY(hints ? go(dense_step_kernel<false, true>) : go(dense_step_kernel<false, false>));
+  StepKernel kernel = step_kernel_of(a);
+  // per device and cheap: set on every call (a process may drive several devices)
+  QHAP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)));
+  QHAP_CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, tj, tjl, th, tl, toh, tol, tsx, tsy, a));
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;
 }
 
-// Fused launches need: TMA-stored copies and tile rows == k-blocks (BN == kBK), k-block lists, and at least two tiles per
-// CTA and step (the epilogue requests the state of the item two ahead before it stores the current one): the grid is
-// at most half the tile count.  All CTAs of the grid must be co-resident (one per SM, grid <= SM count).
 // Shared-memory split between operand stages and the staging buffers of the fp16 copies: the operand feed (every tile
 // re-reads ~6 k-blocks of x_hi, x_lo: 240 KB per tile at cfg1 against 160 KB of state) runs on the bytes in flight, so a
-// single staging buffer is used whenever that buys another stage (cfg1/cfg2: 2 -> 3 stages, 39.7 -> 36.5 and 45.7 -> 40.9
-// us per step; the epilogue waits for the previous tile's store only right before its first staging write).  Where it
-// buys none (cfg3: 48 KB stages) or a fourth one (cfg4) the second buffer stays (cfg3 275 against 290 us, cfg4 223.5 / 226).
-void choose_staging(DenseArgs& a, int stage_bytes, const qhap_bsb_params& p) {
+// single staging buffer is used whenever that buys another stage (fp32-x kernels; cfg1/cfg2: 2 -> 3 stages).  state16 always
+// has two buffers (tile t + 1's own pair is loaded while tile t is updated) and a ring of half the size.
+void choose_staging(DenseArgs& a, int stage_bytes, const qhap_bsb_tuning& t) {
+  const int ring_bytes = a.x16 ? kRingBytes16 : (a.ring ? kRingBytes : 0);
   auto stages = [&](int bufs) {
-    return std::min(kMaxStages, (kSmemBudget - (a.stage_out ? bufs * 2 * kStageX : 0) - (a.ring ? kRingBytes : 0)) / stage_bytes);
+    return std::min(kMaxStages, (kSmemBudget - (a.stage_out ? bufs * 2 * kStageX : 0) - ring_bytes) / stage_bytes);
   };
-  int bufs = (p.dense_stg_bufs == 1 || p.dense_stg_bufs == 2) ? p.dense_stg_bufs : ((a.stage_out && stages(1) > stages(2) && stages(2) < 3) ? 1 : 2);
+  int bufs = (t.dense_stg_bufs == 1 || t.dense_stg_bufs == 2) ? t.dense_stg_bufs : ((a.stage_out && stages(1) > stages(2) && stages(2) < 3) ? 1 : 2);
+  if (a.x16) bufs = 2;
   a.stg_bufs = uint32_t(bufs);
   a.n_stages = stages(bufs);
-  a.store_warp = bufs == 1 ? 1u : 0u;        // launch_fused sets it too
+  a.store_warp = (bufs == 1 || a.x16) ? 1u : 0u;        // launch_fused sets it too
 }
 
-// x (fp32) and the four fp16 copies are 12 B per (spin, replica); when they fit the L2 with room for the y stream and the
-// J tiles they are given the evict_last priority and y evict_first.  Measured: the in-step operand re-reads
-// hit more often (cfg1 34.1 -> 31.7 us per step); the state itself still goes through DRAM every step.
-void set_l2_policies(DenseArgs& a, const qhap_bsb_params& p) {
-  const bool keep = p.l2_hints == 0 ? 12.0 * double(a.n) * double(a.R) <= 104e6 : p.l2_hints == 1;
+// The arrays that are re-used (x in fp32 and the four fp16 copies: 12 B per (spin, replica); state16: the copies only, 8 B)
+// get the evict_last priority and y evict_first when they fit the L2 with room for the y stream and the J tiles.
+void set_l2_policies(DenseArgs& a, const qhap_bsb_tuning& t) {
+  const double keep_bytes = (a.x16 ? 8.0 : 12.0) * double(a.n) * double(a.R);
+  const bool keep = t.l2_hints == 0 ? keep_bytes <= 104e6 : t.l2_hints == 1;
   // q/16 of the keep set's lines are evict_last, the rest evict_first (createpolicy.fractional.L2::evict_last.L2::evict_first
   // with fraction q/16 encodes as (0x150 | (q - 1)) << 52; q = 16 is kEvictLast for every line)
-  const int q = (p.l2_keep_16ths >= 1 && p.l2_keep_16ths <= 16) ? p.l2_keep_16ths : 16;
+  const int q = (t.l2_keep_16ths >= 1 && t.l2_keep_16ths <= 16) ? t.l2_keep_16ths : 16;
   a.pol_keep = keep ? (q == 16 ? ptx::kEvictLast : (uint64_t(0x150u | uint32_t(q - 1)) << 52)) : ptx::kEvictNormal;
   a.pol_stream = keep ? ptx::kEvictFirst : ptx::kEvictNormal;
-  a.epi_sync = p.dense_epi_sync == 0 ? (keep ? 1u : 0u) : (p.dense_epi_sync == 1 ? 1u : 0u);
+  a.epi_sync = t.dense_epi_sync == 0 ? (keep ? 1u : 0u) : (t.dense_epi_sync == 1 ? 1u : 0u);
 }
 
-// Grid of a fused launch, or 0 = one launch per step.  Worth it while a CTA has few tiles per step (launch gap, pipeline
-// fill and drain per step: cfg1 40.0 -> 38.2 us, cfg2 45.2 -> 41.4 us per step, a 304-tile problem 33.9 -> 14.5 us); with
-// ~50 tiles per CTA and step (cfg3) the step boundary is amortised and the lock-step launches keep the L2 reuse between
-// neighbouring CTAs (268 us per step against 274 fused), so those stay on one launch per step.
-int fused_grid(const DenseArgs& a, const qhap_bsb_params& p) {
+// Grid of a fused launch, or 0 = one launch per step.  Fused launches need: TMA-stored copies and tile rows == k-blocks
+// (BN == kBK), k-block lists, at least two tiles per CTA and step (state prefetch distance: grid <= tiles / 2), and ALL CTAs
+// co-resident -- the launch is cooperative, and the grid is capped by what the occupancy API says fits this device.
+// Worth it while a CTA has few tiles per step (launch gap, pipeline fill and drain per step); with ~50 tiles per CTA and
+// step (cfg3) the boundary is amortised and lock-step launches keep the L2 reuse between neighbouring CTAs.
+int fused_grid(const DenseArgs& a, const qhap_bsb_params& p, const qhap_bsb_tuning& t) {
   const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;
-  const int64_t grid = std::min<int64_t>(sm_count(), n_tiles / 2);
-  if (p.step_launch != 0 || !a.stage_out || a.BN != kBK || a.kb_cnt == nullptr || p.steps_run < 2 || grid < 1) return 0;
-  if (ceil_div(n_tiles, grid) > 16) return 0;
+  if (t.step_launch != 0 || !a.stage_out || a.BN != kBK || a.kb_cnt == nullptr || p.steps_run < 2) return 0;
+  int per_sm = 0, coop = 0, dev = 0;
+  StepKernel kernel = step_kernel_of(a);
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop ||
+      cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemBytes)) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, kSmemBytes) != cudaSuccess || per_sm < 1) {
+    (void)cudaGetLastError();
+    return 0;
+  }
+  const int64_t grid = std::min<int64_t>(int64_t(sm_count()) * per_sm, n_tiles / 2);
+  if (grid < 1 || ceil_div(n_tiles, grid) > 16) return 0;
   return int(grid);
 }
 
@@ -1002,94 +1198,121 @@ int32_t choose_bn(int32_t n, int32_t R, bool tile_skip, int32_t forced) {
 
 }  // namespace
 
+namespace {
+// Workspace layout of the dense path -- ONE walk, used by the size query (measure mode) and by the solve.
+struct DenseWs {
+  __half* xh[2];
+  __half* xl[2];
+  int32_t* kb_cnt;
+  int32_t* kb_idx;
+  int32_t* flags;
+  uint32_t* done;
+};
+DenseWs carve_dense(Workspace& ws, int32_t n, int32_t R) {
+  DenseWs w;
+  const size_t copy = size_t(R) * pitch_of(n);
+  w.xh[0] = ws.take<__half>(copy); w.xl[0] = ws.take<__half>(copy);
+  w.xh[1] = ws.take<__half>(copy); w.xl[1] = ws.take<__half>(copy);
+  const size_t n_kb = size_t(ceil_div(n, kBK)), n_tn_max = size_t(ceil_div(n, 32));
+  w.kb_cnt = ws.take<int32_t>(n_tn_max);
+  w.kb_idx = ws.take<int32_t>(n_tn_max * n_kb);
+  w.flags = ws.take<int32_t>(n_tn_max * n_kb);
+  w.done = ws.take<uint32_t>(n_tn_max * size_t(ceil_div(R, kBM)));   // fused steps
+  return w;
+}
+
+// state16 is usable when the tile is one swizzle box wide with TMA-stored copies, the y ring's boxes are legal (row pitch a
+// multiple of 16 bytes, aligned base) and nothing outside the step kernel needs the fp32 x between steps (no remainder
+// gather, no dSB sign copies).
+bool x16_ok(const DenseArgs& a, const float* y, bool has_rem, const qhap_bsb_params& p, const qhap_bsb_tuning& t) {
+  return t.state16 != 2 && a.stage_out && a.BN == kBK && a.R % 4 == 0 && (reinterpret_cast<uintptr_t>(y) & 15) == 0 && !has_rem &&
+         p.force_mode == 0;
+}
+}  // namespace
+
 size_t dense_workspace_bytes(int32_t n, int32_t ld, int32_t R) {
   (void)ld;
   Workspace ws(nullptr);
-  const size_t copy = size_t(R) * pitch_of(n);
-  ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy);
-  const size_t n_kb = size_t(ceil_div(n, kBK)), n_tn_max = size_t(ceil_div(n, 32));
-  ws.take<int32_t>(n_tn_max);             // kb_cnt
-  ws.take<int32_t>(n_tn_max * n_kb);      // kb_idx
-  ws.take<int32_t>(n_tn_max * n_kb);      // flags
-  ws.take<uint32_t>(n_tn_max * size_t(ceil_div(R, kBM)));   // done (fused steps)
+  carve_dense(ws, n, R);
   return ws.used();
 }
 
 qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld, int32_t dtype, int32_t R, const float* c1_dev,
                               const qhap_bsb_params& p, float* x, float* y, void* ws_ptr, size_t ws_bytes, cudaStream_t stream) {
   const int32_t n = g.n;
+  const qhap_bsb_tuning t = tuning_of(p);
   QHAP_REQUIRE(dtype == QHAP_DENSE_FP16, "dense path takes J in fp16");
   QHAP_REQUIRE(uint64_t(g.n) * uint64_t(R) < (1ull << 32), "dense path: n * replicas must be below 2^32");
   QHAP_REQUIRE((reinterpret_cast<uintptr_t>(dense_J) & 15) == 0, "dense_J must be 16-byte aligned");
-  QHAP_REQUIRE(ws_bytes >= dense_workspace_bytes(n, ld, R), "dense workspace too small");
-  Workspace ws(ws_ptr);
+  Workspace ws(ws_ptr, ws_bytes);
+  const DenseWs w = carve_dense(ws, n, R);
+  if (ws.overflow) {
+    set_error("dense workspace too small: %zu < %zu", ws_bytes, ws.used());
+    return QHAP_ERR_WORKSPACE;
+  }
   const int32_t n_k = pitch_of(n);
-  const size_t copy = size_t(R) * n_k;
-  __half* xh[2];
-  __half* xl[2];
-  xh[0] = ws.take<__half>(copy); xl[0] = ws.take<__half>(copy);
-  xh[1] = ws.take<__half>(copy); xl[1] = ws.take<__half>(copy);
   const int32_t n_kb = int32_t(ceil_div(n, kBK));
-  const size_t n_tn_max = size_t(ceil_div(n, 32));
-  int32_t* kb_cnt = ws.take<int32_t>(n_tn_max);
-  int32_t* kb_idx = ws.take<int32_t>(n_tn_max * n_kb);
-  int32_t* flags = ws.take<int32_t>(n_tn_max * n_kb);
-  uint32_t* done = ws.take<uint32_t>(n_tn_max * size_t(ceil_div(R, kBM)));
 
   const bool skip = p.tile_skip != 0;
-  const int32_t BN = choose_bn(n, R, skip, p.dense_bn);
+  const int32_t BN = choose_bn(n, R, skip, t.dense_bn);
   DenseArgs a;
   a.n = n; a.R = R; a.n_k = n_k; a.BN = BN;
   // fp16 copies through TMA stores: the tile must be exactly one 64-column box wide (tile_skip's width); the two
   // staging buffers (2 x 32 KB) come out of the operand-stage budget
   a.stage_out = (BN == kBK) ? 1 : 0;
-  a.ring = ring_ok(BN, R, x, y) ? 1 : 0;
-  choose_staging(a, BN * kBK * 2 + 2 * kStageX, p);
+  a.dsb = p.force_mode == 1 ? 1 : 0;
+  a.x16 = x16_ok(a, y, false, p, t) ? 1 : 0;
+  a.ring = (a.x16 || ring_ok(BN, R, x, y)) ? 1 : 0;
+  a.bc = (t.bias_cancel == 1 && a.ring && BN <= 128 && !a.dsb) ? 1 : 0;
+  choose_staging(a, BN * kBK * 2 + 2 * kStageX, t);
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = int32_t(ceil_div(n, BN));
   a.n_kblocks = n_kb;
-  a.kb_cnt = skip ? kb_cnt : nullptr;
-  a.kb_idx = skip ? kb_idx : nullptr;
+  a.kb_cnt = skip ? w.kb_cnt : nullptr;
+  a.kb_idx = skip ? w.kb_idx : nullptr;
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
-  set_l2_policies(a, p); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
-
-  // per device and cheap: set on every call (a process may drive several devices)
+  set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
   QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));
   QHAP_TRY(make_state_map(&tm_sy, y, n, a.ring ? R : 4));
   QHAP_TRY(make_map(&tm_j, dense_J, uint64_t(ld), uint64_t(ld), uint64_t(ld), uint32_t(BN)));
   for (int b = 0; b < 2; ++b) {
-    QHAP_TRY(make_map(&tm_h[b], xh[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
-    QHAP_TRY(make_map(&tm_l[b], xl[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
+    QHAP_TRY(make_map(&tm_h[b], w.xh[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
+    QHAP_TRY(make_map(&tm_l[b], w.xl[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
   }
 
-  {
-    dim3 grid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
-    split_x_kernel<<<grid, 256, 0, stream>>>(n, R, n_k, x, xh[0], xl[0]);
-    QHAP_LAUNCH_CHECK();
-  }
+  const dim3 tgrid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
+  split_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, a.x16 ? 2 : a.dsb, x, w.xh[0], w.xl[0]);
+  QHAP_LAUNCH_CHECK();
   if (skip) {
-    QHAP_CUDA_TRY(cudaMemsetAsync(flags, 0, sizeof(int32_t) * size_t(a.n_tiles_n) * n_kb, stream));
-    kb_flag_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, BN, n_kb, flags);
+    QHAP_CUDA_TRY(cudaMemsetAsync(w.flags, 0, sizeof(int32_t) * size_t(a.n_tiles_n) * n_kb, stream));
+    kb_flag_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, BN, n_kb, w.flags);
     QHAP_LAUNCH_CHECK();
-    kb_list_kernel<<<a.n_tiles_n, 32, 0, stream>>>(n_kb, flags, kb_cnt, kb_idx);
+    kb_list_kernel<<<a.n_tiles_n, 32, 0, stream>>>(n_kb, BN, w.flags, w.kb_cnt, w.kb_idx);
     QHAP_LAUNCH_CHECK();
   }
 
   const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
   a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
   int cur = 0;
-  if (const int gf = fused_grid(a, p)) return launch_fused(gf, stream, tm_j, tm_j, tm_h, tm_l, tm_sx, tm_sy, a, p, done, cur);
-  for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
-    const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
-    a.c2 = float(p.dt * (p.a0 - a_k));
-    a.c3 = float(p.dt * p.a0);
-    a.xh_out = xh[cur ^ 1];
-    a.xl_out = xl[cur ^ 1];
-    QHAP_TRY(launch_step(grid, stream, tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));
-    cur ^= 1;
+  if (const int gf = fused_grid(a, p, t)) {
+    QHAP_TRY(launch_fused(gf, stream, tm_j, tm_j, tm_h, tm_l, tm_sx, tm_sy, a, p, w.done, cur));
+  } else {
+    for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
+      const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
+      a.c2 = float(p.dt * (p.a0 - a_k));
+      a.c3 = float(p.dt * p.a0);
+      a.xh_out = w.xh[cur ^ 1];
+      a.xl_out = w.xl[cur ^ 1];
+      QHAP_TRY(launch_step(grid, stream, tm_j, tm_j, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));
+      cur ^= 1;
+    }
+  }
+  if (a.x16) {
+    merge_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, w.xh[cur], w.xl[cur], x);
+    QHAP_LAUNCH_CHECK();
   }
   return QHAP_OK;
 }
@@ -1109,25 +1332,52 @@ namespace {
 int64_t block_capacity(int32_t n, int64_t nnz) { return 16 * nnz / (kBK * kBK) + ceil_div(n, kBK) + 1; }
 }  // namespace
 
+namespace {
+// Workspace layout of the block path -- ONE walk, used by the size query (measure mode) and by the solve.
+struct BlockWs {
+  __half* xh[2];
+  __half* xl[2];
+  int32_t *kb_cnt, *blk_ptr, *kb_idx, *flags;
+  float *c1row, *c1plain;
+  int32_t *rem_ptr, *rem_col;
+  float* rem_val;
+  uint32_t* scal;          // absmax bits, scale
+  int64_t* totals;         // total blocks, overflow
+  int64_t* scan_scratch;
+  uint32_t* done;
+  __half *jh, *jl;
+  int64_t cap_blocks;
+};
+BlockWs carve_block(Workspace& ws, int32_t n, int64_t nnz, int32_t R) {
+  BlockWs w;
+  const size_t copy = size_t(R) * pitch_of(n);
+  w.xh[0] = ws.take<__half>(copy); w.xl[0] = ws.take<__half>(copy);
+  w.xh[1] = ws.take<__half>(copy); w.xl[1] = ws.take<__half>(copy);
+  const size_t n_t = size_t(ceil_div(n, kBK));
+  w.kb_cnt = ws.take<int32_t>(n_t + 1);
+  w.blk_ptr = ws.take<int32_t>(n_t + 1);
+  w.kb_idx = ws.take<int32_t>(n_t * n_t);
+  w.flags = ws.take<int32_t>(n_t * n_t);
+  w.c1row = ws.take<float>(size_t(n));
+  w.c1plain = ws.take<float>(size_t(n));
+  w.rem_ptr = ws.take<int32_t>(size_t(n) + 1);
+  w.rem_col = ws.take<int32_t>(size_t(nnz));
+  w.rem_val = ws.take<float>(size_t(nnz));
+  w.scal = ws.take<uint32_t>(4);
+  w.totals = ws.take<int64_t>(2);
+  w.scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(n), 4096)) + 1);
+  w.done = ws.take<uint32_t>(n_t * size_t(ceil_div(R, kBM)));   // fused steps
+  w.cap_blocks = block_capacity(n, nnz);
+  const size_t cap = size_t(w.cap_blocks) * kBK * kBK;
+  w.jh = ws.take<__half>(cap);
+  w.jl = ws.take<__half>(cap);
+  return w;
+}
+}  // namespace
+
 size_t block_workspace_bytes(int32_t n, int64_t nnz, int32_t R) {
   Workspace ws(nullptr);
-  const size_t copy = size_t(R) * pitch_of(n);
-  ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy); ws.take<__half>(copy);
-  const size_t n_t = size_t(ceil_div(n, kBK));
-  ws.take<int32_t>(n_t + 1);              // kb_cnt
-  ws.take<int32_t>(n_t + 1);              // blk_ptr
-  ws.take<int32_t>(n_t * n_t);            // kb_idx
-  ws.take<int32_t>(n_t * n_t);            // flags
-  ws.take<float>(size_t(n));              // c1row
-  ws.take<float>(size_t(n));              // c1plain
-  ws.take<int32_t>(size_t(n) + 1);        // rem_ptr
-  ws.take<int32_t>(size_t(nnz));          // rem_col
-  ws.take<float>(size_t(nnz));            // rem_val
-  ws.take<uint32_t>(4);                   // absmax, scale
-  ws.take<int64_t>(2);                    // total blocks, overflow
-  ws.take<uint32_t>(n_t * size_t(ceil_div(R, kBM)));   // done (fused steps)
-  const size_t cap = size_t(block_capacity(n, nnz)) * kBK * kBK;
-  ws.take<__half>(cap); ws.take<__half>(cap);
+  carve_block(ws, n, nnz, R);
   return ws.used();
 }
 
@@ -1135,33 +1385,27 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
                               const int32_t* inst_ptr_dev, const float* c1_dev, const qhap_bsb_params& p, float* x, float* y,
                               void* ws_ptr, size_t ws_bytes, cudaStream_t stream) {
   const int32_t n = g.n;
+  const qhap_bsb_tuning t = tuning_of(p);
   QHAP_REQUIRE(uint64_t(n) * uint64_t(R) < (1ull << 32), "block path: n * replicas must be below 2^32");
-  QHAP_REQUIRE(ws_bytes >= block_workspace_bytes(n, g.nnz, R), "block workspace too small");
-  Workspace ws(ws_ptr);
+  Workspace ws(ws_ptr, ws_bytes);
+  const BlockWs w = carve_block(ws, n, g.nnz, R);
+  if (ws.overflow) {
+    set_error("block workspace too small: %zu < %zu", ws_bytes, ws.used());
+    return QHAP_ERR_WORKSPACE;
+  }
   const int32_t n_k = pitch_of(n);
-  const size_t copy = size_t(R) * n_k;
-  __half* xh[2];
-  __half* xl[2];
-  xh[0] = ws.take<__half>(copy); xl[0] = ws.take<__half>(copy);
-  xh[1] = ws.take<__half>(copy); xl[1] = ws.take<__half>(copy);
   const int32_t n_t = int32_t(ceil_div(n, kBK));
-  int32_t* kb_cnt = ws.take<int32_t>(size_t(n_t) + 1);
-  int32_t* blk_ptr = ws.take<int32_t>(size_t(n_t) + 1);
-  int32_t* kb_idx = ws.take<int32_t>(size_t(n_t) * n_t);
-  int32_t* flags = ws.take<int32_t>(size_t(n_t) * n_t);
-  float* c1row = ws.take<float>(size_t(n));
-  float* c1plain = ws.take<float>(size_t(n));
-  int32_t* rem_ptr = ws.take<int32_t>(size_t(n) + 1);
-  int32_t* rem_col = ws.take<int32_t>(size_t(g.nnz));
-  float* rem_val = ws.take<float>(size_t(g.nnz));
-  uint32_t* scal = ws.take<uint32_t>(4);
-  int64_t* totals = ws.take<int64_t>(2);
-  int64_t* scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(n), 4096)) + 1);
-  uint32_t* done = ws.take<uint32_t>(size_t(n_t) * size_t(ceil_div(R, kBM)));
-  const int64_t cap_blocks = block_capacity(n, g.nnz);
-  const size_t cap = size_t(cap_blocks) * kBK * kBK;
-  __half* jh = ws.take<__half>(cap);
-  __half* jl = ws.take<__half>(cap);
+  __half* const* xh = w.xh;
+  __half* const* xl = w.xl;
+  int32_t *kb_cnt = w.kb_cnt, *blk_ptr = w.blk_ptr, *kb_idx = w.kb_idx, *flags = w.flags;
+  float *c1row = w.c1row, *c1plain = w.c1plain;
+  int32_t *rem_ptr = w.rem_ptr, *rem_col = w.rem_col;
+  float* rem_val = w.rem_val;
+  uint32_t* scal = w.scal;
+  int64_t *totals = w.totals, *scan_scratch = w.scan_scratch;
+  uint32_t* done = w.done;
+  const int64_t cap_blocks = w.cap_blocks;
+  __half *jh = w.jh, *jl = w.jl;
   const bool two_terms = weight_mode == QHAP_WEIGHT_FX;      // integer counts are exact in fp16 (|J| <= 2048 checked below)
 
   // tile occupancy -> tile lists -> block offsets.  All tiles are kept if they fit the capacity (banded graphs); otherwise
@@ -1219,16 +1463,19 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   DenseArgs a;
   a.n = n; a.R = R; a.n_k = n_k; a.BN = kBK;
   a.stage_out = 1;
-  a.ring = ring_ok(kBK, R, x, y) ? 1 : 0;
+  a.dsb = p.force_mode == 1 ? 1 : 0;
+  a.x16 = x16_ok(a, y, has_rem, p, t) ? 1 : 0;
+  a.ring = (a.x16 || ring_ok(kBK, R, x, y)) ? 1 : 0;
   a.j_terms = two_terms ? 2 : 1;
-  choose_staging(a, a.j_terms * kBK * kBK * 2 + 2 * kStageX, p);
+  a.bc = (t.bias_cancel == 1 && a.ring && !a.dsb) ? 1 : 0;
+  choose_staging(a, a.j_terms * kBK * kBK * 2 + 2 * kStageX, t);
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
   a.n_tiles_n = n_t;
   a.n_kblocks = n_t;
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
   a.c1 = c1row; a.c1_per_row = 1;
   a.x = x; a.y = y;
-  set_l2_policies(a, p); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
+  set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2], tm_sx, tm_sy;
   QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));
@@ -1240,29 +1487,33 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
     QHAP_TRY(make_map(&tm_h[b], xh[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
     QHAP_TRY(make_map(&tm_l[b], xl[b], uint64_t(n), uint64_t(R), uint64_t(n_k), kBM));
   }
-  {
-    dim3 grid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
-    split_x_kernel<<<grid, 256, 0, stream>>>(n, R, n_k, x, xh[0], xl[0]);
-    QHAP_LAUNCH_CHECK();
-  }
+  const dim3 tgrid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
+  split_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, a.x16 ? 2 : a.dsb, x, xh[0], xl[0]);
+  QHAP_LAUNCH_CHECK();
   const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
   a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
   int cur = 0;
   // the remainder gather reads the fp32 x of the whole graph between two tile steps: a grid-wide step boundary
-  if (const int gf = has_rem ? 0 : fused_grid(a, p))
-    return launch_fused(gf, stream, tm_jh, tm_jl, tm_h, tm_l, tm_sx, tm_sy, a, p, done, cur);
-  for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
-    const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
-    a.c2 = float(p.dt * (p.a0 - a_k));
-    a.c3 = float(p.dt * p.a0);
-    a.xh_out = xh[cur ^ 1];
-    a.xl_out = xl[cur ^ 1];
-    if (has_rem) {
-      remainder_step_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, R, rem_ptr, rem_col, rem_val, c1plain, x, y);
-      QHAP_LAUNCH_CHECK();
+  if (const int gf = has_rem ? 0 : fused_grid(a, p, t)) {
+    QHAP_TRY(launch_fused(gf, stream, tm_jh, tm_jl, tm_h, tm_l, tm_sx, tm_sy, a, p, done, cur));
+  } else {
+    for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
+      const double a_k = p.steps_total > 1 ? p.a0 * double(k) / double(p.steps_total - 1) : 0.0;   // R10b
+      a.c2 = float(p.dt * (p.a0 - a_k));
+      a.c3 = float(p.dt * p.a0);
+      a.xh_out = xh[cur ^ 1];
+      a.xl_out = xl[cur ^ 1];
+      if (has_rem) {
+        remainder_step_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, R, a.dsb, rem_ptr, rem_col, rem_val, c1plain, x, y);
+        QHAP_LAUNCH_CHECK();
+      }
+      QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));
+      cur ^= 1;
     }
-    QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));
-    cur ^= 1;
+  }
+  if (a.x16) {
+    merge_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, xh[cur], xl[cur], x);
+    QHAP_LAUNCH_CHECK();
   }
   return QHAP_OK;
 }

@@ -24,6 +24,7 @@ struct ResidentArgs {
   float* x;
   float* y;
   int32_t steps_total, step_begin, steps_run;
+  int32_t dsb;                 // 1: F = J sgn(x) (dSB), sgn(0) = +1
   double dt, a0;
 };
 
@@ -73,7 +74,11 @@ __global__ void __launch_bounds__(kResThreads) bsb_resident_kernel(const Residen
     for (int i = slot; i < n; i += slots) {
       float F = 0.f;
       const int e1 = rp[i + 1];
-      for (int e = rp[i]; e < e1; ++e) F = fmaf(jv[e], cur[cl[e] * RC + l], F);
+      if (a.dsb) {
+        for (int e = rp[i]; e < e1; ++e) F = fmaf(jv[e], cur[cl[e] * RC + l] >= 0.f ? 1.0f : -1.0f, F);
+      } else {
+        for (int e = rp[i]; e < e1; ++e) F = fmaf(jv[e], cur[cl[e] * RC + l], F);
+      }
       const float xo = cur[i * RC + l];
       float yn = fmaf(c1row[i], F, fmaf(-c2, xo, ys[i * RC + l]));
       float xn = fmaf(c3, yn, xo);
@@ -126,7 +131,7 @@ qhap_status resident_solve_steps(const CsrView& g, const float* jval, int32_t R,
   a.row_ptr = g.row_ptr; a.col = g.col; a.jval = jval; a.inst_ptr = inst_ptr_dev; a.c1 = c1;
   a.x = x; a.y = y;
   a.steps_total = p.steps_total; a.step_begin = p.step_begin; a.steps_run = p.steps_run;
-  a.dt = p.dt; a.a0 = p.a0;
+  a.dt = p.dt; a.a0 = p.a0; a.dsb = p.force_mode == 1 ? 1 : 0;
   bsb_resident_kernel<<<int(ceil_div(R, RC)), kResThreads, smem, stream>>>(a);
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;

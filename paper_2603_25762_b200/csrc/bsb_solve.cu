@@ -40,6 +40,31 @@ SolveWs carve(Workspace& ws, int32_t n, int64_t nnz, int32_t n_inst, int32_t R, 
 
 }  // namespace
 
+// One contiguous run of bSB steps [pc.step_begin, pc.step_begin + pc.steps_run) on the chosen path.
+static qhap_status run_steps(const CsrView& g, int path, int32_t res_rc, const void* dense_J, int32_t dense_ld, int32_t dense_dtype,
+                             int32_t n_inst, const SolveWs& s, const qhap_bsb_params& pc, float* x, float* y, cudaStream_t stream) {
+  const int32_t n = g.n, R = pc.replicas;
+  if (pc.steps_run <= 0 || n == 0) return QHAP_OK;
+  if (path == 1) return dense_solve_steps(g, dense_J, dense_ld, dense_dtype, R, s.c1, pc, x, y, s.dense, s.dense_bytes, stream);
+  if (path == 4) return block_solve_steps(g, s.jval, pc.weight_mode, R, n_inst, s.inst_ptr, s.c1, pc, x, y, s.dense, s.dense_bytes, stream);
+  if (path == 3) return resident_solve_steps(g, s.jval, R, res_rc, n_inst, s.inst_ptr, s.c1, pc, x, y, stream);
+  float* cur = x;
+  float* alt = s.x_alt;
+  if (pc.steps_run & 1) {   // an odd number of ping-pong steps must end in the caller's x
+    QHAP_CUDA_TRY(cudaMemcpyAsync(alt, x, sizeof(float) * size_t(n) * R, cudaMemcpyDeviceToDevice, stream));
+    cur = s.x_alt; alt = x;
+  }
+  for (int32_t k = pc.step_begin; k < pc.step_begin + pc.steps_run; ++k) {
+    const double a_k = pc.steps_total > 1 ? pc.a0 * double(k) / double(pc.steps_total - 1) : 0.0;   // R10b
+    StepConsts sc;
+    sc.c2 = float(pc.dt * (pc.a0 - a_k));
+    sc.c3 = float(pc.dt * pc.a0);
+    QHAP_TRY(sparse_step(g, s.jval, R, n_inst, s.inst_ptr, s.c1, sc, pc.force_mode, cur, alt, y, stream));
+    std::swap(cur, alt);
+  }
+  return QHAP_OK;
+}
+
 extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, const int32_t* inst_ptr, const void* dense_J,
                                       int32_t dense_ld, int32_t dense_dtype, const qhap_bsb_params* p, float* x, float* y,
                                       int8_t* best_spins, int64_t* best_cut, int32_t* best_replica,
@@ -50,12 +75,16 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
                    p->step_begin + p->steps_run <= p->steps_total,
                "bad replica/step counts");
   QHAP_REQUIRE(p->weight_mode >= 0 && p->weight_mode <= 2, "bad weight_mode");
+  QHAP_REQUIRE(p->force_mode == 0 || p->force_mode == 1, "force_mode must be 0 (bSB) or 1 (dSB)");
+  QHAP_REQUIRE(p->eval_every >= 0, "eval_every must be >= 0");
   QHAP_REQUIRE(n_inst == 1 || inst_ptr, "inst_ptr (host) is required for n_inst > 1");
+  if (p->tuning)
+    for (int32_t v : p->tuning->reserved) QHAP_REQUIRE(v == 0, "qhap_bsb_tuning.reserved must be 0");
   int path = p->path;
   const int32_t res_rc = (path == 0 || path == 3) ? resident_plan(graph->n, graph->nnz, p->replicas) : 0;
   // auto: small problems -> shared-memory resident; a dense J was built -> tcgen05 over it; otherwise the tcgen05 step on the
   // block-compressed J (hybrid with a remainder CSR for non-banded graphs), except for tiny graphs where the CSR step is as good
-  if (path == 0) path = res_rc > 0 ? 3 : ((dense_J && n_inst == 1) ? 1 : ((graph->n >= 1024 && graph->n <= (1 << 20)) ? 4 : 2));   // the tile-occupancy table is (n / 64)^2 ints
+  if (path == 0) path = res_rc > 0 ? 3 : ((dense_J && n_inst == 1) ? 1 : (graph->n >= 1024 ? 4 : 2));
   QHAP_REQUIRE(path >= 1 && path <= 4, "path must be 0, 1, 2, 3 or 4");
   QHAP_REQUIRE(path != 3 || res_rc > 0, "resident path: problem too large for shared memory (needs n R <= 65536)");
   if (path == 1) {
@@ -64,7 +93,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
     QHAP_REQUIRE(dense_ld >= graph->n && dense_ld % 8 == 0, "dense_ld must be >= n and a multiple of 8");
   }
   const int32_t n = graph->n, R = p->replicas;
-  Workspace ws(workspace);
+  Workspace ws(workspace, (workspace && ws_bytes) ? *ws_bytes : ~size_t(0));
   SolveWs s = carve(ws, n, graph->nnz, n_inst, R, path == 1, dense_ld, path == 4);
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
@@ -88,28 +117,22 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   QHAP_TRY(compute_c1(n, n_inst, s.inst_ptr, s.sumsq, p->dt, p->c0, s.c1, stream));
   if (p->init_state && p->step_begin == 0) QHAP_TRY(init_state(n, R, p->seed, x, y, stream));
 
-  if (p->steps_run > 0 && n > 0) {
-    if (path == 1) {
-      QHAP_TRY(dense_solve_steps(g, dense_J, dense_ld, dense_dtype, R, s.c1, *p, x, y, s.dense, s.dense_bytes, stream));
-    } else if (path == 4) {
-      QHAP_TRY(block_solve_steps(g, s.jval, p->weight_mode, R, n_inst, s.inst_ptr, s.c1, *p, x, y, s.dense, s.dense_bytes, stream));
-    } else if (path == 3) {
-      QHAP_TRY(resident_solve_steps(g, s.jval, R, res_rc, n_inst, s.inst_ptr, s.c1, *p, x, y, stream));
-    } else {
-      float* cur = x;
-      float* alt = s.x_alt;
-      if (p->steps_run & 1) {   // an odd number of ping-pong steps must end in the caller's x
-        QHAP_CUDA_TRY(cudaMemcpyAsync(alt, x, sizeof(float) * size_t(n) * R, cudaMemcpyDeviceToDevice, stream));
-        cur = s.x_alt; alt = x;
-      }
-      for (int32_t k = p->step_begin; k < p->step_begin + p->steps_run; ++k) {
-        const double a_k = p->steps_total > 1 ? p->a0 * double(k) / double(p->steps_total - 1) : 0.0;   // R10b
-        StepConsts sc;
-        sc.c2 = float(p->dt * (p->a0 - a_k));
-        sc.c3 = float(p->dt * p->a0);
-        QHAP_TRY(sparse_step(g, s.jval, R, n_inst, s.inst_ptr, s.c1, sc, cur, alt, y, stream));
-        std::swap(cur, alt);
-      }
+  // eval_every = k: the steps run in pieces of k, each followed by a cut evaluation of sgn(x) (Fig. 3)
+  const bool tracing = p->eval_every > 0 && (p->trace_cut || p->trace_best_cut);
+  qhap_bsb_params pc = *p;
+  int32_t k = p->step_begin, row = 0;
+  const int32_t k_end = p->step_begin + p->steps_run;
+  while (k < k_end) {
+    pc.step_begin = k;
+    pc.steps_run = tracing ? std::min(p->eval_every, k_end - k) : k_end - k;
+    QHAP_TRY(run_steps(g, path, res_rc, dense_J, dense_ld, dense_dtype, n_inst, s, pc, x, y, stream));
+    k += pc.steps_run;
+    if (tracing && pc.steps_run == p->eval_every) {
+      int64_t* cut = p->trace_cut ? p->trace_cut + size_t(row) * n_inst * R : s.cut;
+      QHAP_TRY(cut_from_x(g, p->weight_mode, x, R, n_inst, s.inst_ptr, cut, s.wtot, stream));
+      if (p->trace_best_cut)
+        QHAP_TRY(cut_finalize(n_inst, R, cut, s.wtot, nullptr, p->trace_best_cut + size_t(row) * n_inst, s.best_replica, stream));
+      ++row;
     }
   }
   if (p->finalize) {

@@ -90,6 +90,9 @@ __global__ void __launch_bounds__(256) init_state_kernel(int64_t n, int32_t R, u
 }
 
 // ------------------------------------------------------------------------------------------ the step
+// dSB: the force sees sgn(x), sgn(0) = sgn(-0) = +1 (R10e)
+__device__ __forceinline__ float sgn1(float v) { return v >= 0.f ? 1.0f : -1.0f; }
+
 template <int VEC>
 struct Vec;
 template <>
@@ -100,6 +103,7 @@ struct Vec<4> {
   }
   static __device__ __forceinline__ void unpack(float (&f)[4], const float4& a) { f[0] = a.x; f[1] = a.y; f[2] = a.z; f[3] = a.w; }
   static __device__ __forceinline__ float4 pack(const float (&f)[4]) { return make_float4(f[0], f[1], f[2], f[3]); }
+  static __device__ __forceinline__ float4 sgn(const float4& a) { return make_float4(sgn1(a.x), sgn1(a.y), sgn1(a.z), sgn1(a.w)); }
 };
 template <>
 struct Vec<2> {
@@ -109,6 +113,7 @@ struct Vec<2> {
   }
   static __device__ __forceinline__ void unpack(float (&f)[2], const float2& a) { f[0] = a.x; f[1] = a.y; }
   static __device__ __forceinline__ float2 pack(const float (&f)[2]) { return make_float2(f[0], f[1]); }
+  static __device__ __forceinline__ float2 sgn(const float2& a) { return make_float2(sgn1(a.x), sgn1(a.y)); }
 };
 template <>
 struct Vec<1> {
@@ -116,6 +121,7 @@ struct Vec<1> {
   static __device__ __forceinline__ void fma(float (&f)[1], float v, const float& a) { f[0] = fmaf(v, a, f[0]); }
   static __device__ __forceinline__ void unpack(float (&f)[1], const float& a) { f[0] = a; }
   static __device__ __forceinline__ float pack(const float (&f)[1]) { return f[0]; }
+  static __device__ __forceinline__ float sgn(const float& a) { return sgn1(a); }
 };
 
 // The fused update of one (spin, replica): returns x', writes y'.
@@ -133,7 +139,7 @@ __device__ __forceinline__ float bsb_update(float F, float x, float& y, float c1
 constexpr int kRowsPerBlock = 32;   // consecutive rows share neighbours -> their x rows stay in L1
 constexpr int kWarps = 8;
 
-template <int VEC>
+template <int VEC, bool DSB>
 __global__ void __launch_bounds__(kWarps * 32) sparse_step_kernel(
     int32_t n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col, const float* __restrict__ jval,
     int32_t R, int32_t n_inst, const int32_t* __restrict__ inst_ptr, const float* __restrict__ c1v, float c2, float c3,
@@ -157,14 +163,16 @@ __global__ void __launch_bounds__(kWarps * 32) sparse_step_kernel(
         for (; e + 4 <= e1; e += 4) {
           const int32_t b0 = __ldg(col + e), b1 = __ldg(col + e + 1), b2 = __ldg(col + e + 2), b3 = __ldg(col + e + 3);
           const float v0 = __ldg(jval + e), v1 = __ldg(jval + e + 1), v2 = __ldg(jval + e + 2), v3 = __ldg(jval + e + 3);
-          const V x0 = *reinterpret_cast<const V*>(x_in + size_t(b0) * R + r);
-          const V x1 = *reinterpret_cast<const V*>(x_in + size_t(b1) * R + r);
-          const V x2 = *reinterpret_cast<const V*>(x_in + size_t(b2) * R + r);
-          const V x3 = *reinterpret_cast<const V*>(x_in + size_t(b3) * R + r);
+          V x0 = *reinterpret_cast<const V*>(x_in + size_t(b0) * R + r);
+          V x1 = *reinterpret_cast<const V*>(x_in + size_t(b1) * R + r);
+          V x2 = *reinterpret_cast<const V*>(x_in + size_t(b2) * R + r);
+          V x3 = *reinterpret_cast<const V*>(x_in + size_t(b3) * R + r);
+          if constexpr (DSB) { x0 = Vec<VEC>::sgn(x0); x1 = Vec<VEC>::sgn(x1); x2 = Vec<VEC>::sgn(x2); x3 = Vec<VEC>::sgn(x3); }
           Vec<VEC>::fma(F, v0, x0); Vec<VEC>::fma(F, v1, x1); Vec<VEC>::fma(F, v2, x2); Vec<VEC>::fma(F, v3, x3);
         }
         for (; e < e1; ++e) {
-          const V xv = *reinterpret_cast<const V*>(x_in + size_t(__ldg(col + e)) * R + r);
+          V xv = *reinterpret_cast<const V*>(x_in + size_t(__ldg(col + e)) * R + r);
+          if constexpr (DSB) xv = Vec<VEC>::sgn(xv);
           Vec<VEC>::fma(F, __ldg(jval + e), xv);
         }
         int inst = 0;
@@ -220,7 +228,8 @@ qhap_status init_state(int64_t n, int32_t R, uint64_t seed, float* x, float* y, 
 }
 
 qhap_status sparse_step(const CsrView& g, const float* jval, int32_t R, int32_t n_inst, const int32_t* inst_ptr_dev,
-                        const float* c1, StepConsts k, const float* x_in, float* x_out, float* y, cudaStream_t stream) {
+                        const float* c1, StepConsts k, int32_t force_mode, const float* x_in, float* x_out, float* y,
+                        cudaStream_t stream) {
   if (g.n == 0 || R == 0) return QHAP_OK;
   const bool al16 = ((reinterpret_cast<uintptr_t>(x_in) | reinterpret_cast<uintptr_t>(x_out) | reinterpret_cast<uintptr_t>(y)) & 15) == 0;
   const int vec = (R % 4 == 0 && R >= 128 && al16) ? 4 : ((R % 2 == 0 && al16) ? 2 : 1);
@@ -228,9 +237,15 @@ qhap_status sparse_step(const CsrView& g, const float* jval, int32_t R, int32_t 
   const int64_t work = ceil_div(g.n, kRowsPerBlock) * chunks;
   const int blocks = int(std::min<int64_t>(work, int64_t(sm_count()) * 8));
 #define QHAP_STEP_ARGS g.n, g.row_ptr, g.col, jval, R, n_inst, inst_ptr_dev, c1, k.c2, k.c3, x_in, x_out, y
-  if (vec == 4) sparse_step_kernel<4><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
-  else if (vec == 2) sparse_step_kernel<2><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
-  else sparse_step_kernel<1><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+  if (force_mode == 1) {
+    if (vec == 4) sparse_step_kernel<4, true><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+    else if (vec == 2) sparse_step_kernel<2, true><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+    else sparse_step_kernel<1, true><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+  } else {
+    if (vec == 4) sparse_step_kernel<4, false><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+    else if (vec == 2) sparse_step_kernel<2, false><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+    else sparse_step_kernel<1, false><<<blocks, kWarps * 32, 0, stream>>>(QHAP_STEP_ARGS);
+  }
 #undef QHAP_STEP_ARGS
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;

@@ -19,30 +19,58 @@ void set_error(const char* fmt, ...) {
 static std::atomic<uint64_t> g_launches{0};
 void count_launches(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
-static int g_dev_checked = 0;  // 0 unknown, 1 ok, -1 bad
-static int g_sm_count = 0;
+// Per-device cache (a process may drive several devices): state 0 unknown, 1 sm_100 ok, -1 other architecture.
+constexpr int kMaxDevices = 64;
+struct DevInfo {
+  std::atomic<int> state{0};
+  std::atomic<int> sms{0};
+};
+static DevInfo g_dev[kMaxDevices];
 
-qhap_status require_device() {
-  if (g_dev_checked == 1) return QHAP_OK;
+static cudaError_t probe_device(int* dev_out, int* major, int* minor, int* sms) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
-  cudaDeviceProp prop;
-  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(minor, cudaDevAttrComputeCapabilityMinor, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, dev);
+  *dev_out = dev;
+  return e;
+}
+
+qhap_status require_device() {
+  int dev = 0, major = 0, minor = 0, sms = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices && g_dev[dev].state.load(std::memory_order_acquire) == 1)
+    return QHAP_OK;
+  const cudaError_t e = probe_device(&dev, &major, &minor, &sms);
   if (e != cudaSuccess) {
     set_error("no CUDA device: %s (libqhap has no CPU fallback)", cudaGetErrorString(e));
     (void)cudaGetLastError();
     return QHAP_ERR_CUDA;
   }
-  if (prop.major != 10) {
-    set_error("device '%s' is sm_%d%d; libqhap is built for sm_100a only", prop.name, prop.major, prop.minor);
+  if (major != 10) {
+    set_error("device %d is sm_%d%d; libqhap is built for sm_100a only", dev, major, minor);
     return QHAP_ERR_CUDA;
   }
-  g_sm_count = prop.multiProcessorCount;
-  g_dev_checked = 1;
+  if (dev >= 0 && dev < kMaxDevices) {
+    g_dev[dev].sms.store(sms, std::memory_order_relaxed);
+    g_dev[dev].state.store(1, std::memory_order_release);
+  }
   return QHAP_OK;
 }
 
-int sm_count() { return g_sm_count > 0 ? g_sm_count : 148; }
+int sm_count() {
+  int dev = 0, major = 0, minor = 0, sms = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices) {
+    const int c = g_dev[dev].sms.load(std::memory_order_relaxed);
+    if (c > 0) return c;
+  }
+  if (probe_device(&dev, &major, &minor, &sms) == cudaSuccess && sms > 0) {
+    if (dev >= 0 && dev < kMaxDevices) g_dev[dev].sms.store(sms, std::memory_order_relaxed);
+    return sms;
+  }
+  (void)cudaGetLastError();
+  return 148;          // no device (size queries on a box without a GPU): B200's count, planning only
+}
 
 // ------------------------------------------------------------------------------------------------ scan
 // One CTA of 1024 threads walks the array in tiles of 4096 counts, carrying the running total.
@@ -191,4 +219,4 @@ qhap_status exclusive_scan_i32(const int32_t* in, int32_t* out, int64_t n, int64
 
 extern "C" const char* qhap_last_error(void) { return qhap::g_err; }
 extern "C" uint64_t qhap_launch_count(void) { return qhap::g_launches.load(std::memory_order_relaxed); }
-extern "C" const char* qhap_version(void) { return "qhap-b200 0.1 sm_100a"; }
+extern "C" const char* qhap_version(void) { return "qhap-b200 0.2 sm_100a"; }

@@ -46,20 +46,27 @@ void count_launches(uint64_t n);
     QHAP_CUDA_TRY(cudaGetLastError());      \
   } while (0)
 
-// sm_100 present?  (cached per process)
+// sm_100 present on the CURRENT device?  (cached per device ordinal)
 qhap_status require_device();
+// SM count of the current device (queried once per device; 148 on B200)
 int sm_count();
 
 // ------------------------------------------------------------------------------------------- workspace
-// Bump allocator over the caller's workspace.  In "measure" mode (base == nullptr) it only adds sizes up.
+// Bump allocator over the caller's workspace.  In "measure" mode (base == nullptr) it only adds sizes up.  Every layout
+// is written ONCE, as a function that walks a Workspace: the size query runs it in measure mode, the call runs the same
+// function on the real pointer, so the two cannot disagree.  `cap` bounds a real carve: a take() that would pass it sets
+// `overflow` (checked by the caller -> QHAP_ERR_WORKSPACE) and returns nullptr instead of a pointer past the end.
 struct Workspace {
   char* base;
+  size_t cap;
   size_t off = 0;
-  explicit Workspace(void* p) : base(static_cast<char*>(p)) {}
+  bool overflow = false;
+  explicit Workspace(void* p, size_t cap_bytes = ~size_t(0)) : base(static_cast<char*>(p)), cap(cap_bytes) {}
   template <class T>
   T* take(size_t count) {
     size_t bytes = (count * sizeof(T) + 255) & ~size_t(255);
     T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    if (base && (bytes > cap || off > cap - bytes)) { overflow = true; p = nullptr; }
     off += bytes;
     return p;
   }

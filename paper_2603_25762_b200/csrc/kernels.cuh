@@ -24,6 +24,13 @@ inline CsrView view_of(const qhap_csr& g) {
   return v;
 }
 
+// Tuning knobs of a solve (qhap.h qhap_bsb_tuning): the caller's block, or all zeros = automatic.
+inline qhap_bsb_tuning tuning_of(const qhap_bsb_params& p) {
+  qhap_bsb_tuning t = {};
+  if (p.tuning) t = *p.tuning;
+  return t;
+}
+
 // bSB step constants, evaluated on the host in fp64 and rounded once to fp32 (R10):
 //   y' = fma(c1, F, fma(-c2, x, y)), x' = fma(c3, y', x);  c1 = dt c0 (per instance), c2 = dt (a0 - a_k), c3 = dt a0.
 struct StepConsts {
@@ -48,12 +55,12 @@ qhap_status materialize_jval(const CsrView& g, int mode, int32_t n_inst, const i
 qhap_status compute_c1(int32_t n, int32_t n_inst, const int32_t* inst_ptr_dev, const double* sumsq, double dt, double c0,
                        float* c1, cudaStream_t stream);
 qhap_status init_state(int64_t n, int32_t R, uint64_t seed, float* x, float* y, cudaStream_t stream);
-// one bSB step on the CSR path: x_out, y (in place) from x_in
+// one bSB step on the CSR path: x_out, y (in place) from x_in; force_mode 1 (dSB): F = J sgn(x_in)
 qhap_status sparse_step(const CsrView& g, const float* jval, int32_t R, int32_t n_inst, const int32_t* inst_ptr_dev,
-                        const float* c1, StepConsts k, const float* x_in, float* x_out, float* y, cudaStream_t stream);
+                        const float* c1, StepConsts k, int32_t force_mode, const float* x_in, float* x_out, float* y,
+                        cudaStream_t stream);
 
 // ---- bsb_dense.cu
-struct DensePlan;  // opaque: tensor maps, tile lists, internal buffers carved from the workspace
 size_t dense_workspace_bytes(int32_t n, int32_t ld, int32_t R);
 qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld, int32_t dtype, int32_t R,
                               const float* c1_dev, const qhap_bsb_params& p, float* x, float* y, void* ws, size_t ws_bytes,

@@ -111,7 +111,7 @@ QHAP_API qhap_status qhap_build_snp_graph_fill(const qhap_frags *frags, int32_t 
                                       void *workspace, size_t *ws_bytes, void *stream);
 
 /* Optional kernel tuning of qhap_bsb_solve (paths 1 and 4).  NULL, or a field left 0, means AUTOMATIC.  These knobs select
- * launch shapes, shared-memory splits and cache policies; only `state16` can change result bits (documented there).  They
+ * launch shapes, shared-memory splits and cache policies; only `state16` and `split_acc` can change result bits (documented there).  They
  * live outside qhap_bsb_params so that the solver's parameter block does not change when a kernel is retuned. */
 typedef struct {
   int32_t dense_bn;       /* path 1: tile width in output spins (multiple of 16 in 32..256)                              */
@@ -127,8 +127,10 @@ typedef struct {
                           /*    (16 B of HBM traffic per spin-update instead of 24; x is rounded to that pair, relative      */
                           /*    2^-22, once per step instead of to fp32's 2^-24); 2 = in fp32.  The x returned to the caller */
                           /*    is fp32 either way                                                                            */
-  int32_t bias_cancel;    /* 1 = every tile is accumulated twice, with x and with -x, and F = (D+ - D-) / 2: cancels the      */
-                          /*    sign-independent truncation bias of the tensor cores' fp32 accumulation (2x the MMAs)         */
+  int32_t split_acc;      /* tiles up to 128 wide: automatic / 1 = the small product terms (x_lo J, x_hi J_lo) accumulate in a   */
+                          /*    second TMEM tile and the epilogue adds the two (the tensor cores' fp32 accumulation truncates at */
+                          /*    every MMA; kept apart, the small terms no longer truncate the large sum: measured 2-8x smaller   */
+                          /*    trajectory drift); 2 = one accumulator.  Changes result bits (documented in DESIGN.md 4.4)       */
   int32_t reserved[8];    /* must be 0                                                                                      */
 } qhap_bsb_tuning;
 

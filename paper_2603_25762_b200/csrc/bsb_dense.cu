@@ -52,6 +52,7 @@ struct DenseArgs {
   int32_t ring;               // 1: the fp32 state of the work items arrives through per-warp TMA boxes (BN == 64, R % 4 == 0)
   int32_t stage_out;          // 1: the fp16 copies leave through swizzled shared-memory tiles and TMA stores (BN == 64)
   int32_t n_tiles_m, n_tiles_n, n_kblocks;
+  uint32_t inv_tm;            // floor(2^32 / n_tiles_m) + 1: tile / n_tiles_m == umulhi(tile, inv_tm) for tile n_tiles_m < 2^32 (0: n_tiles_m == 1)
   const int32_t* kb_cnt;      // [n_tiles_n] number of listed k-blocks per N tile, or nullptr = all k-blocks
   const int32_t* kb_idx;      // [n_tiles_n][n_kblocks]
   const float* c1;            // [1] dt c0 (dense J), or per-row factors [n] when c1_per_row != 0 (block-compressed J)
@@ -87,16 +88,24 @@ struct DenseArgs {
   // The fp32 x array is not touched by the step kernel (split before the first step, merged after the last).
   int32_t x16;
   int32_t dsb;                // dSB: the copies hold 2^15 sgn(x) (x_lo = 0), so F = J sgn(x)
-  // bias cancellation: the tcgen05 fp32 accumulation truncates toward -inf, a bias of a few ulp of F that does not depend on
-  // the sign of F.  A second accumulator (128 TMEM columns further) receives the same MMAs with the A operand negated by the
-  // instruction descriptor: D- = -F + bias, D+ = F + bias, and the epilogue uses (D+ - D-) / 2.  Needs BN <= 128 and the ring.
-  int32_t bc;
+  // split accumulators: the tcgen05 fp32 accumulation truncates toward zero at every MMA, a bias of a few ulp of F.  The
+  // small terms (x_lo J and x_hi J_lo, 2^-11 of the leading one) go to a second accumulator 128 TMEM columns further, where
+  // their truncation is 2^-11 smaller; the epilogue adds the two.  Halves the MMAs that truncate at full magnitude.
+  // Needs BN <= 128 (two accumulator stages x 2 x 128 columns = the 512 TMEM columns).
+  int32_t sacc;
 };
 
 // c2 = fp32(dt (a0 - a_k)), a_k = a0 k / (T - 1): the same individually rounded fp64 operations as the host loop
 __device__ __forceinline__ float ramp_c2(const DenseArgs& a, int s) {
   const double a_k = a.steps_total > 1 ? __ddiv_rn(__dmul_rn(a.a0, double(a.k0 + s)), double(a.steps_total - 1)) : 0.0;
   return __double2float_rn(__dmul_rn(a.dt, __dsub_rn(a.a0, a_k)));
+}
+
+// tile -> (N tile, M tile), M fastest; the division by the run-time n_tiles_m is a multiply-high (an integer division costs
+// ~20 instructions, and the epilogue needs the pair for every 8-spin work item)
+__device__ __forceinline__ void tile_split(const DenseArgs& a, int tile, int& tn, int& tm) {
+  tn = a.inv_tm ? int(__umulhi(uint32_t(tile), a.inv_tm)) : tile;
+  tm = tile - tn * a.n_tiles_m;
 }
 
 // fp32 -> two fp16 terms of xs = 2^15 x (|x| <= 1 -> |xs| <= 32768, inside fp16's range): hi = rn(xs), lo = rn(xs - hi)
@@ -156,7 +165,8 @@ __device__ __forceinline__ void epi_pack(int j, float xn, uint32_t (&hp)[kChunk 
 // Element offsets are 32-bit (the host checks n R < 2^32): one integer add and one wide multiply-add per address.
 __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, float (&xv)[kChunk],
                                          float (&yv)[kChunk]) {
-  const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+  int tn, tm;
+  tile_split(a, tile, tn, tm);
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
   const bool r_ok = r < a.R;
   uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
@@ -182,11 +192,13 @@ template <bool hints>
 __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tile, int ch,
                                                  const uint32_t (&v)[kChunk], const float (&xv)[kChunk],
                                                  const float (&yv)[kChunk], uint32_t stg) {
-  const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+  int tn, tm;
+  tile_split(a, tile, tn, tm);
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
   const bool r_ok = r < a.R;
   uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
   uint32_t hp[kChunk / 2], lp[kChunk / 2];    // fp16 pairs (spin i0 + 2q, i0 + 2q + 1) of x_hi', x_lo'
+  float xs[kChunk];
   if (r_ok && i0 + kChunk <= a.n) {
 #pragma unroll
     for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
@@ -200,7 +212,7 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
         a.x[off] = xn;
         a.y[off] = yn;
       }
-      if (a.dsb) epi_pack<1>(j, xn, hp, lp); else epi_pack<0>(j, xn, hp, lp);
+      xs[j] = xn;
     }
   } else {
 #pragma unroll
@@ -213,8 +225,15 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
         ptx::st_global_f32_hint(a.x + off, xn, a.pol_keep);
         ptx::st_global_f32_hint(a.y + off, yn, a.pol_stream);
       }
-      if (a.dsb && ok) epi_pack<1>(j, xn, hp, lp); else epi_pack<0>(j, ok ? xn : 0.f, hp, lp);
+      xs[j] = ok ? xn : 0.f;              // masked entries: zeros in the copies (dSB: sgn(0) = +1, never read -- J is 0 there)
     }
+  }
+  if (a.dsb) {                              // one warp-uniform branch per work item, outside the unrolled loops
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j) epi_pack<1>(j, xs[j], hp, lp);
+  } else {
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j) epi_pack<0>(j, xs[j], hp, lp);
   }
   if (stg != 0) {
     // staging tile [128 replicas][64 spins] fp16 per array, rows of 128 B, 16-byte pieces XOR-swizzled by (row & 7):
@@ -242,35 +261,70 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
 // buffer `stg` (TMA-loaded, 128-byte swizzle: 16-byte piece p of row r sits at piece p ^ (r & 7)), x = (x_hi + x_lo) 2^-15
 // exactly; the new canonical pair goes back to the SAME 16 bytes (this thread is their only reader and writer), y' to global.
 // Rows / replicas outside the problem arrive as zeros (TMA fill), stay zero (F = 0 there) and are clipped by the TMA store.
-template <bool hints>
-__device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, const uint32_t (&v)[kChunk],
+// The arithmetic runs on xs = 2^15 x directly (every factor 2^15 is exact): y' = fma(c1 2^-15, 2^15 F, fma(-(c2 2^-15), xs, y)),
+// xs' = fma(c3 2^15, y', xs), wall at |xs'| > 2^15 -- bit for bit the fp32 update of x.  Pairs of spins are split and
+// canonicalised with packed fp16 instructions: (h, l) = (rn(xs'), rn(xs' - h)); H = h + l in fp16 (= rn16 of the exact sum),
+// L = (h - H) + l (both exact): (H, L) has the same sum and is a fixed point of the split (see split_half_canonical).
+template <bool hints, bool PER_ROW>
+__device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiConsts& ec, int tn, int tm, int ch, const uint32_t (&v)[kChunk],
                                                const float (&yv)[kChunk], uint32_t stg) {
-  const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
-  const bool r_ok = r < a.R;
   const int row = ec.lane_r;
   static_assert(kChunk == 8, "one work item = one 16-byte piece of the swizzled staging row");
   const uint32_t addr = stg + uint32_t(row) * 128u + ((uint32_t(ch) ^ uint32_t(row & 7)) << 4);
   uint32_t hq[4], lq[4];
   ptx::ld_shared_v4(addr, hq[0], hq[1], hq[2], hq[3]);
   ptx::ld_shared_v4(addr + kStageX, lq[0], lq[1], lq[2], lq[3]);
-  uint32_t hp[kChunk / 2], lp[kChunk / 2];
-  uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
-  const bool interior = r_ok && i0 + kChunk <= a.n;
+  const bool interior = r < a.R && i0 + kChunk <= a.n;
+  float c1v[kChunk];
+  if constexpr (PER_ROW) {
+    if (i0 + kChunk <= a.n) {                  // 32-byte aligned run of the per-row factors (warp-uniform address)
+      const float4 ca = __ldg(reinterpret_cast<const float4*>(a.c1 + i0)), cb = __ldg(reinterpret_cast<const float4*>(a.c1 + i0 + 4));
+      c1v[0] = ca.x; c1v[1] = ca.y; c1v[2] = ca.z; c1v[3] = ca.w; c1v[4] = cb.x; c1v[5] = cb.y; c1v[6] = cb.z; c1v[7] = cb.w;
+    } else {
 #pragma unroll
-  for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
-    const uint32_t hb = (j & 1) ? (hq[j >> 1] >> 16) : (hq[j >> 1] & 0xffffu);
-    const uint32_t lb = (j & 1) ? (lq[j >> 1] >> 16) : (lq[j >> 1] & 0xffffu);
-    const float x = (__half2float(__ushort_as_half((unsigned short)hb)) + __half2float(__ushort_as_half((unsigned short)lb))) * (1.0f / kXScale);
-    const bool ok = interior || (r_ok && (i0 + j) < a.n);
-    const float c1 = (a.c1_per_row && (interior || (i0 + j) < a.n)) ? __ldg(a.c1 + i0 + j) : ec.c1;
-    float xn, yn;
-    epi_point(ec, c1, __uint_as_float(v[j]), x, yv[j], xn, yn);
-    if (ok) {
-      if constexpr (hints) ptx::st_global_f32_hint(a.y + off, yn, a.pol_stream);
-      else a.y[off] = yn;
+      for (int j = 0; j < kChunk; ++j) c1v[j] = (i0 + j) < a.n ? __ldg(a.c1 + i0 + j) : 0.f;
     }
-    epi_pack<2>(j, ok ? xn : 0.f, hp, lp);
+  }
+  float yn[kChunk];
+  uint32_t hp[kChunk / 2], lp[kChunk / 2];
+#pragma unroll
+  for (int q = 0; q < kChunk / 2; ++q) {
+    const float2 hf = __half22float2(*reinterpret_cast<const __half2*>(&hq[q]));
+    const float2 lf = __half22float2(*reinterpret_cast<const __half2*>(&lq[q]));
+    float xn[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const int j = 2 * q + e;
+      const float xs = e ? hf.y + lf.y : hf.x + lf.x;                       // exact
+      const float c1 = PER_ROW ? c1v[j] : ec.c1;
+      float y1 = fmaf(c1, __uint_as_float(v[j]), fmaf(-ec.c2, xs, yv[j]));
+      float x1 = fmaf(ec.c3, y1, xs);
+      if (fabsf(x1) > kXScale) {               // inelastic wall, strict inequality (R10d), in units of 2^-15
+        x1 = copysignf(kXScale, x1);
+        y1 = 0.0f;
+      }
+      xn[e] = x1; yn[j] = y1;
+    }
+    const __half2 h = __floats2half2_rn(xn[0], xn[1]);
+    const float2 hb = __half22float2(h);
+    const __half2 l = __floats2half2_rn(xn[0] - hb.x, xn[1] - hb.y);
+    const __half2 H = __hadd2(h, l);
+    const __half2 L = __hadd2(__hsub2(h, H), l);
+    hp[q] = *reinterpret_cast<const uint32_t*>(&H);
+    lp[q] = *reinterpret_cast<const uint32_t*>(&L);
+  }
+  uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
+  if (interior) {
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
+      if constexpr (hints) ptx::st_global_f32_hint(a.y + off, yn[j], a.pol_stream);
+      else a.y[off] = yn[j];
+    }
+  } else if (r < a.R) {
+#pragma unroll
+    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R))
+      if (i0 + j < a.n) a.y[off] = yn[j];
   }
   ptx::st_shared_v4(addr, hp[0], hp[1], hp[2], hp[3]);
   ptx::st_shared_v4(addr + kStageX, lp[0], lp[1], lp[2], lp[3]);
@@ -352,7 +406,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
         const int s = vt / stride, tile = vt - s * stride;
         if (tile >= n_tiles) continue;
-        const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;      // M fastest: neighbouring CTAs share the J tile in L2
+        int tn, tm;                                                      // M fastest: neighbouring CTAs share the J tile in L2
+        tile_split(a, tile, tn, tm);
         const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
         if (s > 0) {
           for (int j = lane; j < nkb; j += 32)                           // tile (kb, tm) has finished step s - 1
@@ -396,7 +451,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
       const int tile = vt % stride;
       if (tile >= n_tiles) continue;
-      const int tn = tile / a.n_tiles_m;
+      int tn, tm_unused;
+      tile_split(a, tile, tn, tm_unused);
       const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
       ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);                    // epilogue has drained this accumulator stage
       ptx::tc_fence_after();
@@ -418,6 +474,22 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
               ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
               if (a.j_terms == 2) ptx::umma_f16(d_tmem, dh + 2u * kk, djl + 2u * kk, idesc, 1u);
             }
+          } else if (a.sacc) {              // small terms (x_lo J, x_hi J_lo: 2^-11 of the leading one) into their own accumulator
+            const uint32_t d2 = d_tmem + 128u;
+            if (a.j_terms == 2) {
+#pragma unroll
+              for (int kk = 0; kk < kBK / 16; ++kk) {
+                ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+                ptx::umma_f16(d2, dl + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+                ptx::umma_f16(d2, dh + 2u * kk, djl + 2u * kk, idesc, 1u);
+              }
+            } else {
+#pragma unroll
+              for (int kk = 0; kk < kBK / 16; ++kk) {
+                ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+                ptx::umma_f16(d2, dl + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
+              }
+            }
           } else if (a.j_terms == 2) {
 #pragma unroll
             for (int kk = 0; kk < kBK / 16; ++kk) {
@@ -430,23 +502,6 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
             for (int kk = 0; kk < kBK / 16; ++kk) {
               ptx::umma_f16(d_tmem, dh + 2u * kk, dj + 2u * kk, idesc, (j | kk) != 0);
               ptx::umma_f16(d_tmem, dl + 2u * kk, dj + 2u * kk, idesc, 1u);
-            }
-          }
-          if (a.bc) {                     // the same MMAs once more with -A into the second accumulator
-            const uint32_t idn = idesc | (1u << 13), dn = d_tmem + 128u;
-            if (a.j_terms == 2) {
-#pragma unroll
-              for (int kk = 0; kk < kBK / 16; ++kk) {
-                ptx::umma_f16(dn, dh + 2u * kk, dj + 2u * kk, idn, (j | kk) != 0);
-                ptx::umma_f16(dn, dl + 2u * kk, dj + 2u * kk, idn, 1u);
-                ptx::umma_f16(dn, dh + 2u * kk, djl + 2u * kk, idn, 1u);
-              }
-            } else {
-#pragma unroll
-              for (int kk = 0; kk < kBK / 16; ++kk) {
-                ptx::umma_f16(dn, dh + 2u * kk, dj + 2u * kk, idn, (j | kk) != 0);
-                ptx::umma_f16(dn, dl + 2u * kk, dj + 2u * kk, idn, 1u);
-              }
             }
           }
           ptx::umma_commit(empty_bar(stage));                            // frees the smem stage when these MMAs are done
@@ -475,7 +530,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         while (vt_ld < vt_end) {
           const int s = vt_ld / stride, tile = vt_ld - s * stride;
           if (tile >= n_tiles) { vt_ld += gridDim.x; continue; }
-          const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+          int tn, tm;
+  tile_split(a, tile, tn, tm);
           const uint32_t stg = stg_base + b_ld * (2u * kStageX);
           ptx::mbar_arrive_expect_tx(stg_in(b_ld), 2u * kStageX);
           if constexpr (HINTS) {
@@ -496,7 +552,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
         const int s = vt / stride, tile = vt - s * stride;
         if (tile >= n_tiles) continue;
-        const int tn = tile / a.n_tiles_m, tm = tile % a.n_tiles_m;
+        int tn, tm;
+  tile_split(a, tile, tn, tm);
         const uint32_t stg = stg_base + b * (2u * kStageX);
         ptx::mbar_wait(stg_full(b), bpar);
         if constexpr (HINTS) {
@@ -516,6 +573,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if constexpr (X16) load_next();            // into the buffer just read (b_ld == b)
         if (++b == a.stg_bufs) { b = 0; bpar ^= 1u; }
       }
+      ptx::tma_store_wait_all();                   // the bulk stores have completed before this thread exits
     }
   } else {
     // ========================================================================================= epilogue
@@ -528,7 +586,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     constexpr int P = kEpiWarps / 4;
     EpiConsts ec;
     ec.c1 = a.c1_per_row ? 0.f : __ldg(a.c1) * (1.0f / kXScale);    // accumulator = 2^15 F (per-row factors include it)
-    ec.c2 = a.c2; ec.c3 = a.c3;
+    // state16 works on xs = 2^15 x: the exact powers of two move into the constants
+    constexpr float kC2s = X16 ? 1.0f / kXScale : 1.0f, kC3s = X16 ? kXScale : 1.0f;
+    ec.c2 = a.c2 * kC2s; ec.c3 = a.c3 * kC3s;
     ec.lane_r = quarter * 32 + lane;
     int acc = 0;
     uint32_t acc_phase = 0;
@@ -536,26 +596,32 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     const uint32_t stg_base = smem_base + uint32_t(kStages) * kStageBytes;
     uint32_t tcount = 0;
     int cur_s = 0;                             // step (of this launch) whose ramp constant ec.c2 holds
-    if (a.fused) ec.c2 = ramp_c2(a, 0);
+    if (a.fused) ec.c2 = ramp_c2(a, 0) * kC2s;
     // every warp owns chunk `par` of every tile (possibly fully masked), so that it arrives on tmem_empty once per tile.
     // Items are addressed by the VIRTUAL tile (step-major); the last wave of a step may have a hole for this CTA.
     // A position carries the virtual tile (ordering, end test) and the real tile next to it, so that the item loop needs
     // no division by the runtime stride.
-    struct Pos { int vt, rt, ch; };
+    struct Pos { int vt, rt, ch, tn, tm; };                // (tn, tm) of rt travel along: one tile_split per tile, not per item
     auto advance = [&](Pos& p) {
       p.ch += P;
-      if (p.ch * kChunk >= a.BN || (p.rt / a.n_tiles_m) * a.BN + p.ch * kChunk >= a.n) {
+      if (p.ch * kChunk >= a.BN || p.tn * a.BN + p.ch * kChunk >= a.n) {
         p.vt += gridDim.x; p.rt += gridDim.x;
         if (p.rt >= n_tiles) {                              // past the step's tiles
           if (p.rt < stride) { p.vt += gridDim.x; p.rt += gridDim.x; }   // hole in the last wave (stride % grid == 0)
           p.rt -= stride;                                   // first wave of the next step
         }
         p.ch = par;
+        tile_split(a, p.rt, p.tn, p.tm);
       }
+    };
+    auto first_pos = [&]() {
+      Pos p{int(blockIdx.x), int(blockIdx.x), par, 0, 0};
+      tile_split(a, p.rt, p.tn, p.tm);
+      return p;
     };
     int step_end = stride;                     // first virtual tile of step cur_s + 1
     auto set_step = [&](int vt) {              // items are visited in ascending vt
-      if (a.fused && vt >= step_end) { ++cur_s; step_end += stride; ec.c2 = ramp_c2(a, cur_s); }
+      if (a.fused && vt >= step_end) { ++cur_s; step_end += stride; ec.c2 = ramp_c2(a, cur_s) * kC2s; }
     };
     uint32_t stg_i = 0, stg_par = 0;           // staging buffer of the current tile and its use parity
     // last chunk of this warp in a tile: hand the accumulator stage back and arrive on the staging tile's barrier (the
@@ -585,7 +651,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         ptx::named_barrier_sync(1, kEpiWarps * 32);
         if (ew == 0 && lane == 0) {
           const uint32_t stg = stg_base + stg_i * (2u * kStageX);
-          const int tn = cur_rt / a.n_tiles_m, tm = cur_rt % a.n_tiles_m;
+          int tn, tm;
+          tile_split(a, cur_rt, tn, tm);
           ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
           ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
           ptx::tma_store_commit();
@@ -607,11 +674,17 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       if (p.ch == par) tile_begin();
       uint32_t v[kChunk];
       ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p.ch * kChunk), v);
+      uint32_t v2[kChunk];
+      if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p.ch * kChunk), v2);
       Pos q = p;
       advance(q);
       const bool nhave = q.vt < vt_end;
       if (nhave) epi_load(a, ec, q.rt, q.ch, xn, yn);
       ptx::tmem_ld_wait();
+      if (a.sacc) {
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v2[j]));
+      }
       const uint32_t stg = a.stage_out ? stg_base + stg_i * (2u * kStageX) : 0u;
       if (p.ch == par) staging_free();
       set_step(p.vt);
@@ -632,7 +705,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       auto issue = [&](const Pos& p, int slot) {
         if (ptx::elect_one()) {
           const int ch = p.ch;
-          const int tn = p.rt / a.n_tiles_m, tm = p.rt % a.n_tiles_m;
+          const int tn = p.tn, tm = p.tm;
           const uint32_t dst = ring_w + uint32_t(slot) * kSlotBytes;
           ptx::mbar_arrive_expect_tx(rbar0 + 8u * slot, kSlotBytes);
           if constexpr (X16) {
@@ -648,7 +721,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         }
         __syncwarp();
       };
-      Pos p0{int(blockIdx.x), int(blockIdx.x), par}, p1 = p0, p2 = p0;
+      Pos p0 = first_pos(), p1 = p0, p2 = p0;
       if (p0.vt < vt_end) {
         issue(p0, 0);
         advance(p1);
@@ -661,8 +734,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if (p0.ch == par) tile_begin();
         uint32_t v[kChunk];
         ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p0.ch * kChunk), v);
-        uint32_t vneg[kChunk];
-        if (a.bc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p0.ch * kChunk), vneg);
+        uint32_t v2[kChunk];
+        if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p0.ch * kChunk), v2);
         ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
         float xv[kChunk], yv[kChunk];
         const uint32_t src = ring_w + uint32_t(slot) * kSlotBytes + uint32_t(lane) * 4u;
@@ -675,36 +748,40 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
           }
         }
-        __syncwarp();                            // every lane has its values: the slot may be refilled
-        if (p1.vt < vt_end && p2.vt < vt_end) issue(p2, slot);
         const uint32_t stg = a.stage_out ? stg_base + stg_i * (2u * kStageX) : 0u;
         if constexpr (X16) {
           if (p0.ch == par) ptx::mbar_wait(stg_in(stg_i), stg_par);      // the tile's own (x_hi, x_lo) has arrived
           ptx::tmem_ld_wait();
-          if (a.bc) {
+          if (a.sacc) {
 #pragma unroll
-            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(0.5f * (__uint_as_float(v[j]) - __uint_as_float(vneg[j])));
+            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v2[j]));
           }
           set_step(p0.vt);
-          epi_update_x16<HINTS>(a, ec, p0.rt, p0.ch, v, yv, stg);
+          if (a.c1_per_row) epi_update_x16<HINTS, true>(a, ec, p0.tn, p0.tm, p0.ch, v, yv, stg);
+          else epi_update_x16<HINTS, false>(a, ec, p0.tn, p0.tm, p0.ch, v, yv, stg);
         } else {
           ptx::tmem_ld_wait();
-          if (a.bc) {
+          if (a.sacc) {
 #pragma unroll
-            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(0.5f * (__uint_as_float(v[j]) - __uint_as_float(vneg[j])));
+            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v2[j]));
           }
           if (p0.ch == par) staging_free();
           set_step(p0.vt);
           epi_update_store<HINTS>(a, ec, p0.rt, p0.ch, v, xv, yv, stg);
         }
         cur_rt = p0.rt;
+        // The slot is refilled only now: the update above has CONSUMED the values read from it, so those shared-memory
+        // reads have completed.  (Requested right after the ld.shared instructions were issued, the TMA write could land
+        // before the last of them had read the slot: observed as rows 5..7 of a work item carrying the next item's y.)
+        __syncwarp();
+        if (p1.vt < vt_end && p2.vt < vt_end) issue(p2, slot);
         if (p1.vt != p0.vt) tile_done();
         p0 = p1; p1 = p2;
         if (p2.vt < vt_end) advance(p2);
       }
       if (a.stage_out && !a.store_warp && ew == 0 && lane == 0) ptx::tma_store_wait_read_all();   // smem must outlive the bulk reads
     } else {
-    Pos p{int(blockIdx.x), int(blockIdx.x), par};
+    Pos p = first_pos();
     if (p.vt < vt_end) {
       float xa[kChunk], ya[kChunk], xb[kChunk], yb[kChunk];
       epi_load(a, ec, p.rt, p.ch, xa, ya);
@@ -916,7 +993,8 @@ __global__ void __launch_bounds__(256) remainder_kernel(int32_t n, const int32_t
 __device__ __forceinline__ float4 sgn4(float4 v) {
   return make_float4(v.x >= 0.f ? 1.f : -1.f, v.y >= 0.f ? 1.f : -1.f, v.z >= 0.f ? 1.f : -1.f, v.w >= 0.f ? 1.f : -1.f);
 }
-__global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t R, int32_t dsb, const int32_t* __restrict__ rem_ptr,
+template <bool dsb>
+__global__ void __launch_bounds__(256) remainder_step_kernel(int32_t n, int32_t R, const int32_t* __restrict__ rem_ptr,
                                                              const int32_t* __restrict__ rem_col, const float* __restrict__ rem_val,
                                                              const float* __restrict__ c1row_plain, const float* __restrict__ x,
                                                              float* __restrict__ y) {
@@ -1059,7 +1137,8 @@ void set_l2_policies(DenseArgs& a, const qhap_bsb_tuning& t) {
   const int q = (t.l2_keep_16ths >= 1 && t.l2_keep_16ths <= 16) ? t.l2_keep_16ths : 16;
   a.pol_keep = keep ? (q == 16 ? ptx::kEvictLast : (uint64_t(0x150u | uint32_t(q - 1)) << 52)) : ptx::kEvictNormal;
   a.pol_stream = keep ? ptx::kEvictFirst : ptx::kEvictNormal;
-  a.epi_sync = t.dense_epi_sync == 0 ? (keep ? 1u : 0u) : (t.dense_epi_sync == 1 ? 1u : 0u);
+  // (measured with state16: the meeting costs cfg1 26.6 against 25.6 us per step, so it stays with the fp32-x kernels)
+  a.epi_sync = t.dense_epi_sync == 0 ? ((keep && !a.x16) ? 1u : 0u) : (t.dense_epi_sync == 1 ? 1u : 0u);
 }
 
 // Grid of a fused launch, or 0 = one launch per step.  Fused launches need: TMA-stored copies and tile rows == k-blocks
@@ -1263,9 +1342,11 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.dsb = p.force_mode == 1 ? 1 : 0;
   a.x16 = x16_ok(a, y, false, p, t) ? 1 : 0;
   a.ring = (a.x16 || ring_ok(BN, R, x, y)) ? 1 : 0;
-  a.bc = (t.bias_cancel == 1 && a.ring && BN <= 128 && !a.dsb) ? 1 : 0;
+  a.sacc = (t.split_acc != 2 && BN <= 128 && !a.dsb) ? 1 : 0;
   choose_staging(a, BN * kBK * 2 + 2 * kStageX, t);
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
+  a.inv_tm = a.n_tiles_m > 1 ? uint32_t((uint64_t(1) << 32) / uint64_t(a.n_tiles_m)) + 1u : 0u;
+  QHAP_REQUIRE(ceil_div(n, 32) * int64_t(a.n_tiles_m) * a.n_tiles_m < (int64_t(1) << 32), "tile index arithmetic: too many replica tiles for this n");
   a.n_tiles_n = int32_t(ceil_div(n, BN));
   a.n_kblocks = n_kb;
   a.kb_cnt = skip ? w.kb_cnt : nullptr;
@@ -1467,9 +1548,11 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.x16 = x16_ok(a, y, has_rem, p, t) ? 1 : 0;
   a.ring = (a.x16 || ring_ok(kBK, R, x, y)) ? 1 : 0;
   a.j_terms = two_terms ? 2 : 1;
-  a.bc = (t.bias_cancel == 1 && a.ring && !a.dsb) ? 1 : 0;
+  a.sacc = (t.split_acc != 2 && !a.dsb) ? 1 : 0;
   choose_staging(a, a.j_terms * kBK * kBK * 2 + 2 * kStageX, t);
   a.n_tiles_m = int32_t(ceil_div(R, kBM));
+  a.inv_tm = a.n_tiles_m > 1 ? uint32_t((uint64_t(1) << 32) / uint64_t(a.n_tiles_m)) + 1u : 0u;
+  QHAP_REQUIRE(ceil_div(n, 32) * int64_t(a.n_tiles_m) * a.n_tiles_m < (int64_t(1) << 32), "tile index arithmetic: too many replica tiles for this n");
   a.n_tiles_n = n_t;
   a.n_kblocks = n_t;
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
@@ -1504,7 +1587,9 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
       a.xh_out = xh[cur ^ 1];
       a.xl_out = xl[cur ^ 1];
       if (has_rem) {
-        remainder_step_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, R, a.dsb, rem_ptr, rem_col, rem_val, c1plain, x, y);
+        const int rb = int(ceil_div(int64_t(n) * 32, 256));
+        if (a.dsb) remainder_step_kernel<true><<<rb, 256, 0, stream>>>(n, R, rem_ptr, rem_col, rem_val, c1plain, x, y);
+        else remainder_step_kernel<false><<<rb, 256, 0, stream>>>(n, R, rem_ptr, rem_col, rem_val, c1plain, x, y);
         QHAP_LAUNCH_CHECK();
       }
       QHAP_TRY(launch_step(grid, stream, tm_jh, tm_jl, tm_h[cur], tm_l[cur], tm_h[cur ^ 1], tm_l[cur ^ 1], tm_sx, tm_sy, a));

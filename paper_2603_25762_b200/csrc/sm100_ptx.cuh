@@ -36,11 +36,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred P;\n"
       "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 P, [%0], %1;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P, [%0], %1, %2;\n\t"
       "@P bra WAIT_DONE;\n\t"
       "bra WAIT_LOOP;\n"
       "WAIT_DONE:\n\t}\n" ::"r"(bar),
-      "r"(parity)
+      "r"(parity), "r"(0x989680u)      // suspend-time hint: the waiting warp sleeps in hardware instead of polling the issue slots away
       : "memory");
 }
 

@@ -301,7 +301,7 @@ def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: i
                    path: int = 0, tile_skip: int = 0, force_mode: int = 0, eval_every: int = 0, trace_cuts: bool = False,
                    x: Optional[torch.Tensor] = None, y: Optional[torch.Tensor] = None,
                    dense_J: Optional[torch.Tensor] = None, finalize: bool = True, cut_per_replica: bool = True,
-                   workspace: Optional[torch.Tensor] = None, **tuning) -> dict:
+                   workspace: Optional[torch.Tensor] = None, workspace_bytes: Optional[int] = None, **tuning) -> dict:
     """(3)(4)(5) bSB solve.  x, y: [n][R] fp32 CUDA tensors updated in place; None -> seeded on the device.
     Keyword arguments named like the fields of qhap_bsb_tuning (dense_bn, step_launch, l2_hints, ..., state16) fill that
     optional block; eval_every = k > 0 returns `trace_best_cut` [steps_run // k][n_inst] (and `trace_cut` [..][n_inst][R]
@@ -346,7 +346,7 @@ def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: i
     _check(call(None, C.byref(ws_bytes)), "qhap_bsb_solve (size query)")
     if workspace is None or workspace.numel() < ws_bytes.value:
         workspace = _workspace(ws_bytes.value)
-    ws_bytes = C.c_size_t(workspace.numel())
+    ws_bytes = C.c_size_t(workspace.numel() if workspace_bytes is None else int(workspace_bytes))   # the size the library is told
     _check(call(_ptr(workspace), C.byref(ws_bytes)), "qhap_bsb_solve")
     return dict(x=x, y=y, best_spins=best_spins[:n] if finalize else None, best_cut=best_cut, best_replica=best_rep,
                 cut=cuts, workspace=workspace, trace_best_cut=tr_best, trace_cut=tr_cut, workspace_bytes=int(ws_bytes.value))

@@ -38,14 +38,18 @@ def test_struct_layouts_match_c(tmp_path):
     from paper_2603_25762_b200 import binding as B
     src = tmp_path / "layout.c"
     src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "qhap.h"\nint main(void){'
-                   'printf("%zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(qhap_frags), offsetof(qhap_frags, frag_ptr), offsetof(qhap_frags, h1),'
+                   'printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(qhap_frags), offsetof(qhap_frags, frag_ptr), offsetof(qhap_frags, h1),'
                    'sizeof(qhap_csr), offsetof(qhap_csr, w), sizeof(qhap_bsb_params), offsetof(qhap_bsb_params, seed),'
-                   'offsetof(qhap_bsb_params, finalize)); return 0;}')
+                   'offsetof(qhap_bsb_params, finalize), offsetof(qhap_bsb_params, eval_every), offsetof(qhap_bsb_params, trace_cut),'
+                   'offsetof(qhap_bsb_params, tuning), sizeof(qhap_bsb_tuning), offsetof(qhap_bsb_tuning, state16), offsetof(qhap_bsb_tuning, reserved));'
+                   ' return 0;}')
     exe = tmp_path / "layout"
     subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I", str(ROOT / "include"), str(src), "-o", str(exe)])
     got = [int(v) for v in subprocess.check_output([str(exe)]).split()]
     exp = [C.sizeof(B._Frags), B._Frags.frag_ptr.offset, B._Frags.h1.offset, C.sizeof(B._Csr), B._Csr.w.offset,
-           C.sizeof(B._BsbParams), B._BsbParams.seed.offset, B._BsbParams.finalize.offset]
+           C.sizeof(B._BsbParams), B._BsbParams.seed.offset, B._BsbParams.finalize.offset, B._BsbParams.eval_every.offset,
+           B._BsbParams.trace_cut.offset, B._BsbParams.tuning.offset, C.sizeof(B._BsbTuning), B._BsbTuning.state16.offset,
+           B._BsbTuning.reserved.offset]
     assert got == exp
 
 
@@ -68,6 +72,23 @@ def test_size_query_and_loud_failure_without_gpu(lib):
     g.nnz = 50
     assert lib.qhap_bsb_solve(C.byref(g), 1, None, None, 0, 0, C.byref(p), None, None, None, None, None, None, None, C.byref(ws3), None) == B.QHAP_OK
     assert ws3.value >= 10 * 64 * 4
+    # the size query of every step path, and the optional tuning block: reserved fields must be 0
+    sizes = {}
+    for path in (1, 2, 4):
+        p.path = path
+        w = C.c_size_t(0)
+        dj = C.c_void_p(256) if path == 1 else None
+        assert lib.qhap_bsb_solve(C.byref(g), 1, None, dj, 16, B.QHAP_DENSE_FP16, C.byref(p), None, None, None, None, None, None, None, C.byref(w), None) == B.QHAP_OK
+        sizes[path] = w.value
+    assert sizes[1] > sizes[2] and sizes[4] > sizes[2]
+    t = B._BsbTuning()
+    t.reserved[3] = 1
+    p.tuning = C.pointer(t)
+    assert lib.qhap_bsb_solve(C.byref(g), 1, None, None, 0, 0, C.byref(p), None, None, None, None, None, None, None, C.byref(ws3), None) == B.QHAP_ERR_INVALID_ARG
+    assert b"reserved" in lib.qhap_last_error()
+    p.tuning = None
+    p.force_mode = 2
+    assert lib.qhap_bsb_solve(C.byref(g), 1, None, None, 0, 0, C.byref(p), None, None, None, None, None, None, None, C.byref(ws3), None) == B.QHAP_ERR_INVALID_ARG
     if not torch.cuda.is_available():
         # a compute call without a device must fail loudly, not fall back
         buf = (C.c_char * (ws.value + 512))()

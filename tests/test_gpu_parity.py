@@ -14,9 +14,11 @@ pytestmark = pytest.mark.gpu
 TRAJ_TOL = 1e-3          # north_star
 WALL_BAND = 1e-4         # |x_pre| within this of 1.0: the wall decision may legitimately differ
 RESYNC_TOL = 2e-5        # one step from identical fp32 states (50x tighter than north_star's free-running bar; measured ~1e-6)
-TWIN_TOL = 1e-5          # oracle-vs-perturbed-oracle drift that closes the free-running horizon (R18)
-TWIN_TOL_TC = 1e-6       # the same for the tensor-core paths, whose per-step error is ~10 ulp instead of ~1
-MIN_HORIZON = 5          # every case must stay well conditioned at least this long, else the test would be vacuous
+TWIN_TOL = 1e-5          # oracle-vs-perturbed-oracle drift that closes the free-running horizon (R18); ONE value for
+                         # every step path (round 1 closed the tensor-core paths' window 10x earlier; with the split accumulators
+                         # their per-step error is at the CSR kernel's level and they get no allowance)
+MIN_HORIZON = 8          # every case must stay well conditioned at least this long, else the test would be vacuous
+MAX_TAINTED_FRAC = 0.05  # replicas that may leave the free-running comparison after a marginal wall flip (before the horizon)
 
 
 @pytest.fixture(scope="module")
@@ -329,12 +331,13 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
 
     xo = np.ascontiguousarray(x0[:, cols], np.float64); yo = np.ascontiguousarray(y0[:, cols], np.float64)
     xt = xo * (1.0 + 2.0 ** -23); yt = yo * (1.0 + 2.0 ** -23)        # the oracle's twin, one fp32 ulp away
-    twin_tol = TWIN_TOL_TC if path in (1, 4) else TWIN_TOL
+    twin_tol = TWIN_TOL
     out = dict(case=case, path=path, n=int(n), R=int(R), replicas_compared=int(Rs), steps=int(steps), expect_full=bool(expect_full),
                twin_tol=twin_tol, free_dx=0.0, free_dy=0.0, resync_dx=0.0, resync_dy=0.0, horizon=steps, excluded=0, tail_dx=0.0,
                first_exceed=None, twin_at_first_exceed=None, series_dx=[], series_dy=[], series_twin=[])
     horizon_open = True
     tainted = np.zeros(Rs, bool)
+    twin_tainted = np.zeros(Rs, bool)
     for k in range(steps):
         # (a) resynchronised single step from the oracle's current state rounded to fp32
         xs32, ys32 = np.ascontiguousarray(xo, np.float32), np.ascontiguousarray(yo, np.float32)
@@ -351,9 +354,15 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         assert dx <= RESYNC_TOL and dy <= RESYNC_TOL, f"{case}: resync step {k}: max|dx| {dx:.3e}, max|dy| {dy:.3e}"
         # (b) free-running
         xo, yo, xpre = oracle_step(xo, yo, k)
-        xt, yt, _ = oracle_step(xt, yt, k)
+        xt, yt, xpre_t = oracle_step(xt, yt, k)
         xh, yh = gpu_step(xg, yg, k)
-        twin = float(max(np.abs(xt - xo).max(), np.abs(yt - yo).max()))
+        # the twin measures CONDITIONING, not wall luck: a replica whose twin takes the other wall decision at a marginal
+        # pre-clamp |x| leaves the twin measure (as it would leave the comparison below), and marginal entries' y is masked
+        marg_t = (np.abs(np.abs(xpre) - 1.0) < WALL_BAND) | (np.abs(np.abs(xpre_t) - 1.0) < WALL_BAND)
+        if horizon_open:
+            twin_tainted |= (marg_t & ((yt == 0.0) != (yo == 0.0))).any(axis=0)
+        tk = ~twin_tainted
+        twin = float(max(np.abs(xt - xo)[:, tk].max(), np.abs(np.where(marg_t, 0.0, yt - yo))[:, tk].max())) if tk.any() else 0.0
         if horizon_open and twin > twin_tol and not expect_full:
             out["horizon"], horizon_open = k, False
         # a replica whose GPU run took the OTHER wall decision at a marginal pre-clamp |x| (within WALL_BAND of 1) follows a
@@ -361,7 +370,8 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         # the free-running comparison, and the number of such replicas is bounded below
         marginal = np.abs(np.abs(xpre) - 1.0) < WALL_BAND
         flipped = marginal & ((yh == 0.0) != (yo == 0.0))
-        tainted |= flipped.any(axis=0)
+        if horizon_open:                       # past the horizon nothing is asserted, so nothing needs to be excluded
+            tainted |= flipped.any(axis=0)
         keep = ~tainted
         dx, dy, exc = diff(xh[:, keep], yh[:, keep], xo[:, keep], yo[:, keep], xpre[:, keep]) if keep.any() else (0.0, 0.0, 0)
         out["series_dx"].append(dx); out["series_dy"].append(dy); out["series_twin"].append(twin)
@@ -375,10 +385,12 @@ def compare_trajectory(B, oracle, torch_mod, g, w_int, mode, n, R, T, seed, step
         else:
             out["tail_dx"] = max(out["tail_dx"], dx)
     out["tainted"] = int(tainted.sum())
+    out["twin_dropped"] = int(twin_tainted.sum())
     _record(out)
-    cap = max(2, 0.5 * Rs) if max_tainted is None else max_tainted
+    cap = max(2, MAX_TAINTED_FRAC * Rs) if max_tainted is None else max_tainted
     assert out["tainted"] <= cap, {k: v for k, v in out.items() if not k.startswith("series")}     # the free-running check must not become vacuous
     assert out["excluded"] <= 1e-3 * n * Rs * steps * 2
+    assert out["twin_dropped"] <= max(2, 0.25 * Rs), {k: v for k, v in out.items() if not k.startswith("series")}
     if strict:
         assert out["horizon"] >= min(steps, min_horizon), {k: v for k, v in out.items() if not k.startswith("series")}
     return out
@@ -404,7 +416,8 @@ def test_sparse_trajectory_cfg0(B, oracle, torch_mod, R):
     g = oracle.read_graph(fr)
     for mode in (0, 1):
         w = oracle.read_weights(g, mode)
-        o = compare_trajectory(B, oracle, torch_mod, g, w, mode, fr.n_frag, R, p["T"], p["seed"], expect_full=(mode == 1))
+        o = compare_trajectory(B, oracle, torch_mod, g, w, mode, fr.n_frag, R, p["T"], p["seed"], expect_full=(mode == 1),
+                               case=f"cfg0 sparse mode {mode} R {R}")
         print(f"cfg0 sparse mode {mode} R {R}: {fmt_traj(o)}")
 
 
@@ -415,7 +428,7 @@ def test_sparse_trajectory_snp_graph_batched(B, oracle, torch_mod):
     win = synth.block_windows(fr.n_snp, 500, 450)
     bs = oracle.block_split(g, win)
     o = compare_trajectory(B, oracle, torch_mod, bs, bs["w_fx"], 2, bs["n"], 256, p["T"], p["seed"], steps=50,
-                           inst_ptr=bs["inst_ptr"])
+                           inst_ptr=bs["inst_ptr"], case="cfg3-scaled batched sparse")
     print(f"cfg3-scaled batched: {fmt_traj(o)}")
 
 
@@ -423,7 +436,7 @@ def test_sparse_trajectory_cfg1_scaled(B, oracle, torch_mod):
     fr, p = synth.make_config(1, scale=0.1)
     g = oracle.read_graph(fr)
     w = oracle.read_weights(g, 1)
-    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, 128, p["T"], p["seed"], expect_full=True)
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, 128, p["T"], p["seed"], expect_full=True, case="cfg1-scaled sparse")
     print(f"cfg1-scaled sparse: {fmt_traj(o)}")
 
 
@@ -443,7 +456,8 @@ def test_resident_path_equals_sparse_bitwise(B, oracle, torch_mod, R):
     for k in ("x", "y", "best_spins", "best_cut", "best_replica", "cut"):
         assert torch_mod.equal(outs[2][k], outs[3][k]), k
     w = oracle.read_weights(g, 1)
-    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=20, path=3, expect_full=True)
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=50, path=3, expect_full=True,
+                           case=f"cfg0 resident R {R}")
     print(f"cfg0 resident R {R}: {fmt_traj(o)}")
 
 
@@ -505,8 +519,8 @@ def test_dense_trajectory(B, oracle, torch_mod, name, R, bn, skip):
     B.qhap_bsb_solve(dg, step_begin=17, steps_run=13, x=xg, y=yg, **kw)
     assert torch_mod.equal(xs, xg) and torch_mod.equal(ys, yg)
     print(f"dense {name} R {R} bn {bn} skip {skip}: 10 steps max|dx| {dx:.2e} max|dy| {dy:.2e}")
-    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=20, path=1, dense_J=J,
-                           tile_skip=skip)
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=50, path=1, dense_J=J,
+                           tile_skip=skip, dense_bn=bn, case=f"dense {name} R {R} bn {bn} skip {skip}")
     print(f"dense {name}: {fmt_traj(o)}")
 
 
@@ -644,7 +658,7 @@ def test_block_path_read_graph_equals_dense_tile_skip(B, oracle, torch_mod):
                                dense_J=J if path == 1 else None, finalize=False, tile_skip=1, dense_bn=64)
         outs.append(res)
     assert torch_mod.equal(outs[0]["x"], outs[1]["x"]) and torch_mod.equal(outs[0]["y"], outs[1]["y"])
-    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, 136, p["T"], p["seed"], steps=20, path=4)
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, 136, p["T"], p["seed"], steps=50, path=4, case="block path cfg1-scaled R 136")
     print(f"block path cfg1-scaled: {fmt_traj(o)}")
 
 
@@ -655,8 +669,8 @@ def test_block_path_snp_graph_batched(B, oracle, torch_mod):
     g = oracle.snp_graph(fr, 3, 0.1)
     win = synth.block_windows(fr.n_snp, 500, 450)
     bs = oracle.block_split(g, win)
-    o = compare_trajectory(B, oracle, torch_mod, bs, bs["w_fx"], 2, bs["n"], 256, p["T"], p["seed"], steps=30,
-                           inst_ptr=bs["inst_ptr"], path=4)
+    o = compare_trajectory(B, oracle, torch_mod, bs, bs["w_fx"], 2, bs["n"], 256, p["T"], p["seed"], steps=50,
+                           inst_ptr=bs["inst_ptr"], path=4, case="block path cfg3-scaled batched")
     print(f"block path cfg3-scaled batched: {fmt_traj(o)}")
     dg = B.upload_csr(bs)
     R, T = 64, 400
@@ -680,7 +694,8 @@ def test_block_path_long_range_graph_hybrid(B, oracle, torch_mod):
     g = oracle.snp_graph(fr, 3, 0.1)
     rows = np.repeat(np.arange(g["n"]), np.diff(g["row_ptr"]))
     assert (np.abs(g["col"] - rows) > 256).sum() > 100, "the case must contain long-range edges"
-    o = compare_trajectory(B, oracle, torch_mod, g, g["w_fx"], 2, g["n"], 128, p["T"], p["seed"], steps=30, path=4)
+    o = compare_trajectory(B, oracle, torch_mod, g, g["w_fx"], 2, g["n"], 128, p["T"], p["seed"], steps=50, path=4,
+                           case="block path cfg4-scaled (hybrid)")
     print(f"block path cfg4-scaled (hybrid): {fmt_traj(o)}")
     dg = B.upload_csr(g)
     rb = B.qhap_bsb_solve(dg, replicas=64, steps_total=300, seed=p["seed"], weight_mode=2, path=4)
@@ -689,6 +704,39 @@ def test_block_path_long_range_graph_hybrid(B, oracle, torch_mod):
     assert cb >= cs - 0.005 * abs(cs), (cb, cs)
     ccut, _ = oracle.cut_eval(g["row_ptr"], g["col"], g["w_fx"], rb["best_spins"].cpu().numpy())
     assert ccut[0] == cb
+
+
+# ------------------------------------- north_star's bar at its stated length on the tensor-core paths
+@pytest.mark.parametrize("name,R", [("cfg0", 64), ("cfg1-scaled", 128)])
+def test_tensor_core_paths_hold_1e3_for_50_free_running_steps(B, oracle, torch_mod, name, R):
+    """The two cases on which the fp32 CSR kernel holds max |dx|, |dy| <= 1e-3 against the fp64 oracle over ALL of the first
+    50 free-running steps (the twin run stays conditioned): the tcgen05 paths must hold it too, with no horizon -- the full
+    GEMM (fp32 x), the tile_skip step and the block path (x carried as the fp16 pair), one launch per step; and the FUSED
+    launch run with steps_run = 50 in one call."""
+    fr, p, g, w, J = dense_case(B, oracle, name)
+    for path, skip, kw, tag in ((1, 0, {}, "full GEMM"), (1, 1, {"dense_bn": 64}, "tile_skip state16"), (4, 0, {}, "block state16"),
+                                (1, 1, {"dense_bn": 64, "state16": 2}, "tile_skip fp32 x")):
+        o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=50, path=path,
+                               dense_J=J if path == 1 else None, tile_skip=skip, expect_full=True, max_tainted=2,
+                               case=f"50 free steps {name} R {R} path {path} {tag}", **kw)
+        print(f"{name} path {path} {tag}: {fmt_traj(o)}")
+        assert o["first_exceed"] is None
+    # one call, 50 steps (fused where the tile count allows: cfg1-scaled at R = 256 has 26 tiles on 13 CTAs)
+    Rf = 256 if name != "cfg0" else R
+    x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, Rf)
+    xo, yo, _ = oracle.bsb_run(g["row_ptr"], g["col"], (-w).astype(np.float32), x0.astype(np.float64), y0.astype(np.float64),
+                               steps_total=p["T"], steps_run=50, n_threads=8)
+    dg = B.upload_csr(g)
+    for path in (1, 4):
+        for sl in (0, 1):
+            xg = torch_mod.from_numpy(x0.copy()).cuda(); yg = torch_mod.from_numpy(y0.copy()).cuda()
+            B.qhap_bsb_solve(dg, replicas=Rf, steps_total=p["T"], steps_run=50, weight_mode=1, path=path, dense_J=J if path == 1 else None,
+                             tile_skip=1, dense_bn=64 if path == 1 else 0, x=xg, y=yg, finalize=False, step_launch=sl)
+            dx = float(np.abs(xg.cpu().numpy() - xo).max()); dy = float(np.abs(yg.cpu().numpy() - yo).max())
+            _record(dict(case=f"one call of 50 steps {name} R {Rf} path {path} step_launch {sl}", path=path, n=int(fr.n_frag), R=int(Rf), steps=50,
+                         expect_full=True, free_dx=dx, free_dy=dy, horizon=50, first_exceed=None if max(dx, dy) <= TRAJ_TOL else 50))
+            print(f"{name} path {path} step_launch {sl}: 50 steps in one call max|dx| {dx:.2e} max|dy| {dy:.2e}")
+            assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (name, path, sl, dx, dy)
 
 
 # -------------------------------------------------------------------------------- full solve: quality and phasing
@@ -767,11 +815,27 @@ def test_solve_snp_blocks_quality(B, oracle, torch_mod):
 
 # ----------------------------------------------------------- BASELINE.json configs[1] at FULL size (bench.py's launch config)
 def test_cfg1_full_size_sampled(B, oracle, torch_mod):
-    """cfg1 as bench.py runs it (n = 8,000 fragments, R = 1,024, dense tcgen05 step with tile_skip, device-side seeded
-    start state): graph build bit-exact; the first 10 steps of 8 sampled replicas against the oracle run on exactly those
-    replicas (replicas are independent trajectories); cuts of the sampled replicas and the best cut bit-exact; best cut
-    and switch error against an oracle solve of a 64-replica subset."""
-    fr, p = synth.make_config(1)
+    """cfg1 as bench.py runs it (n = 8,000 fragments, R = 1,024, T = 2,000): see full_size_read_case; plus the CSR step at
+    full size over the first 10 steps of the sampled replicas."""
+    sample = np.array([0, 1, 127, 128, 500, 777, 1000, 1023])
+    fr, p, og, jval = full_size_read_case(B, oracle, torch_mod, 1, sample, "cfg1")
+    assert np.abs(jval).max() <= 256                                       # bf16-exact at this config (SURVEY F3)
+    n, R, T = fr.n_frag, p["R"], p["T"]
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    res = B.qhap_bsb_solve(B.upload_csr(og), replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=1, path=2, finalize=False)
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], jval, np.ascontiguousarray(x0[:, sample], np.float64),
+                               np.ascontiguousarray(y0[:, sample], np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+    dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
+    print(f"cfg1 full size, sparse: 10 steps, 8 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+    assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
+
+
+def full_size_read_case(B, oracle, torch_mod, cfg, sample, name):
+    """A read-based BASELINE config at FULL size, as bench.py launches it (dense tcgen05 step with tile_skip, fused launch,
+    device-side seeded start state): graph + dense J bit-exact, sampled-replica trajectories by the policy of
+    compare_trajectory (the oracle follows exactly those replicas), cuts and best replica bit-exact, and quality against an
+    oracle solve of the SAME replicas for all T steps.  Returns what the caller wants to assert on top."""
+    fr, p = synth.make_config(cfg)
     n, R, T = fr.n_frag, p["R"], p["T"]
     dfr = B.upload_frags(fr)
     og = oracle.read_graph(fr)
@@ -779,23 +843,23 @@ def test_cfg1_full_size_sampled(B, oracle, torch_mod):
     assert_csr_equal(g.to_host(), og, ("d", "c"))
     w = oracle.read_weights(og, 1)
     jval = (-w).astype(np.float32)
-    # dense J is exactly -w scattered (sampled rows)
     Jh = J.cpu().numpy()
-    for a in (0, 1, n // 2, n - 1):
+    for a in (0, 1, n // 3, n // 2, n - 1):          # dense J is exactly -w scattered (sampled rows), zero elsewhere
         row = np.zeros(Jh.shape[1], np.float32)
         sl = slice(og["row_ptr"][a], og["row_ptr"][a + 1])
         row[og["col"][sl]] = jval[sl]
         assert np.array_equal(Jh[a].astype(np.float32), row)
+    o = compare_trajectory(B, oracle, torch_mod, og, w, 1, n, R, T, p["seed"], steps=50, path=1, dense_J=J, tile_skip=1, sample=sample,
+                           case=f"{name} full size, dense tile_skip, {len(sample)} sampled replicas")
+    print(f"{name} full size: {fmt_traj(o)}")
     x0, y0 = synth.bsb_init_state(p["seed"], n, R)
-    sample = np.array([0, 1, 127, 128, 500, 777, 1000, R - 1])
-    for path, skip, name in ((1, 1, "dense tile_skip"), (2, 0, "sparse")):
-        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=1, path=path,
-                               dense_J=J if path == 1 else None, tile_skip=skip, finalize=False)
-        xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], jval, x0[:, sample].astype(np.float64), y0[:, sample].astype(np.float64),
-                                   steps_total=T, step_begin=0, steps_run=10, n_threads=8)
-        dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
-        print(f"cfg1 full size, {name}: 10 steps, 8 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
-        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
+    # one fused call of 10 steps against the oracle on the sampled replicas
+    res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=1, path=1, dense_J=J, tile_skip=1, finalize=False)
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], jval, np.ascontiguousarray(x0[:, sample], np.float64), np.ascontiguousarray(y0[:, sample], np.float64),
+                               steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+    dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
+    print(f"{name} full size, fused launch: 10 steps, {len(sample)} sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+    assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
     res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=p["seed"], weight_mode=1, path=1, dense_J=J, tile_skip=1)
     cuts = res["cut"].cpu().numpy()[0]
     sx = np.where(res["x"].cpu().numpy()[:, sample] >= 0, 1, -1).astype(np.int8)
@@ -805,15 +869,29 @@ def test_cfg1_full_size_sampled(B, oracle, torch_mod):
     gcut = int(res["best_cut"].cpu()[0]); r = int(res["best_replica"].cpu()[0])
     ccut, _ = oracle.cut_eval(og["row_ptr"], og["col"], w, spins)
     assert ccut[0] == gcut == cuts.max() and r == int(np.flatnonzero(cuts == cuts.max())[0])
-    sub = np.arange(64)
-    ores = oracle.solve(og["row_ptr"], og["col"], w, jval, x0[:, sub].copy(), y0[:, sub].copy(), steps_total=T, n_threads=16)
-    assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
+    ores = oracle.solve(og["row_ptr"], og["col"], w, jval, x0, y0, steps_total=T, n_threads=oracle.hardware_threads())
     hap = B.qhap_phase_readout_reads(dfr, res["best_spins"]).cpu().numpy()
     assert np.array_equal(hap, oracle.read_vote(fr, spins))
-    gse, ghe = ser_reads(oracle, fr, spins)
-    ose, ohe = ser_reads(oracle, fr, ores["best_spins"])
-    print(f"cfg1 full size: gpu best cut {gcut} (replica {r}), oracle(64 replicas) {ores['best_cut']}; SE gpu {gse:.5f} oracle {ose:.5f}")
+    gse, _ = ser_reads(oracle, fr, spins)
+    ose, _ = ser_reads(oracle, fr, ores["best_spins"])
+    print(f"{name} full size: gpu best cut {gcut} (replica {r}), oracle ({R} replicas x {T} steps) {ores['best_cut']}; SE gpu {gse:.5f} oracle {ose:.5f}")
+    _record(dict(case=f"{name} full size quality", gpu_best_cut=gcut, oracle_best_cut=int(ores["best_cut"]), replicas=int(R), steps=int(T),
+                 se_gpu=gse, se_oracle=ose, max_abs_J=float(np.abs(jval).max())))
+    assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
     assert gse <= ose + 0.001
+    return fr, p, og, jval
+
+
+# ----------------------------------------------------------- BASELINE.json configs[2] at FULL size (bench.py's launch config)
+def test_cfg2_full_size_sampled(B, oracle, torch_mod):
+    """cfg2 (4,000 ONT-like reads, R = 2,048, T = 3,000): the one config whose |J| exceeds the bf16-exact range at
+    the launch geometry the bench uses (63 N-tiles x 16 M-tiles, fused launch, L2 hints)."""
+    sample = np.array([0, 1, 127, 128, 1023, 1024, 1500, 2047])
+    fr, p, og, jval = full_size_read_case(B, oracle, torch_mod, 2, sample, "cfg2")
+    assert np.abs(jval).max() > 256 and np.abs(jval).max() <= 2048        # fp16-exact, not bf16-exact
+    with pytest.raises(B.QhapError) as ei:
+        B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_BF16)
+    assert ei.value.status == B.QHAP_ERR_RANGE
 
 
 # ------------------------------------------------------------------- (f1) SNP-based iterative refinement, Eq. 15-17
@@ -961,7 +1039,8 @@ def test_read_graph_with_porec_fragments_on_tile_paths(B, oracle, torch_mod):
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
     for k in (2,):
         assert np.abs(outs[k][0] - outs[3][0]).max() <= TRAJ_TOL and np.abs(outs[k][1] - outs[3][1]).max() <= TRAJ_TOL
-    o = compare_trajectory(B, oracle, torch_mod, g, w, 0, g["n"], 96, 500, 3, steps=20, path=4, min_horizon=3)   # stiff: w = D
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 0, g["n"], 96, 500, 3, steps=50, path=4, min_horizon=3,   # stiff: w = D
+                           case="read graph with Pore-C fragments, block path")
     print(f"read graph with Pore-C fragments, block path: {fmt_traj(o)}")
     res = B.qhap_bsb_solve(dg, replicas=64, steps_total=500, seed=3, weight_mode=0, path=4)
     x0, y0 = synth.bsb_init_state(3, g["n"], 64)
@@ -1054,7 +1133,32 @@ def test_cfg3_full_size_sampled(B, oracle, torch_mod):
     covered = np.bincount(fr.snp_idx[fr.allele <= 1], minlength=fr.n_snp) > 0
     m = oracle.switch_hamming(hap[covered], fr.hap_a[covered])
     print(f"cfg3 full size: stitched SE {m['se']:.5f} HE {m['he']:.5f} over {int(covered.sum())} covered SNPs")
-    assert m["se"] <= 0.02
+    # quality as north_star words it, on a stated replica SUBSET matched on both sides: the GPU and the oracle solve replicas
+    # 0..R_sub-1 of every block from the same seeds (replica r's start state does not depend on R) for all T steps
+    R_sub = 32
+    rsub = B.qhap_bsb_solve(bs, replicas=R_sub, steps_total=T, seed=p["seed"], weight_mode=2, path=4)
+    gsp = rsub["best_spins"].cpu().numpy(); gbc = rsub["best_cut"].cpu().numpy()
+    x0s, y0s = synth.bsb_init_state(p["seed"], n, R_sub)
+    osp = np.zeros(n, np.int8)
+    worst = 0.0
+    for b in range(len(win)):
+        lo, hi = int(obs["inst_ptr"][b]), int(obs["inst_ptr"][b + 1])
+        rp = (obs["row_ptr"][lo:hi + 1] - obs["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(obs["row_ptr"][lo]), int(obs["row_ptr"][hi]))
+        cl = (obs["col"][sl] - lo).astype(np.int32)
+        o = oracle.solve(rp, cl, obs["w_fx"][sl], (-obs["w"][sl]).astype(np.float32), x0s[lo:hi], y0s[lo:hi], steps_total=T,
+                         n_threads=oracle.hardware_threads())
+        osp[lo:hi] = o["best_spins"]
+        assert int(gbc[b]) >= o["best_cut"] - 0.005 * abs(o["best_cut"]), (b, int(gbc[b]), o["best_cut"])
+        worst = min(worst, (int(gbc[b]) - o["best_cut"]) / abs(o["best_cut"]))
+    gst = B.qhap_block_stitch(fr.n_snp, win, rsub["best_spins"]).cpu().numpy()
+    ost = oracle.block_stitch(fr.n_snp, win, [osp[int(obs["inst_ptr"][b]):int(obs["inst_ptr"][b + 1])] for b in range(len(win))])
+    gm = oracle.switch_hamming(oracle.snp_readout(fr.h1, gst)[covered], fr.hap_a[covered])
+    om = oracle.switch_hamming(oracle.snp_readout(fr.h1, ost)[covered], fr.hap_a[covered])
+    print(f"cfg3 full size, {R_sub} matched replicas x {T} steps: SE gpu {gm['se']:.5f} oracle {om['se']:.5f}; worst relative best-cut gap {worst:.2e}")
+    _record(dict(case="cfg3 full size quality", replicas=R_sub, steps=int(T), se_gpu=gm["se"], se_oracle=om["se"], worst_rel_cut_gap=worst,
+                 se_gpu_full_R=m["se"]))
+    assert gm["se"] <= om["se"] + 0.001
 
 
 # ------------------------------------------------- BASELINE.json configs[4] at FULL size (hybrid block path, one instance)
@@ -1070,14 +1174,35 @@ def test_cfg4_full_size_sampled(B, oracle, torch_mod):
     assert (np.abs(og["col"] - rows) > 4096).sum() > 500_000
     n, R, T = og["n"], p["R"], p["T"]
     x0, y0 = synth.bsb_init_state(p["seed"], n, R)
-    sample = np.array([0, 63, R - 1])
-    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], (-og["w"]).astype(np.float32), x0[:, sample].astype(np.float64),
-                               y0[:, sample].astype(np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+    sample = np.array([0, 1, 31, 63, 64, 100, 126, R - 1])
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], (-og["w"]).astype(np.float32), np.ascontiguousarray(x0[:, sample], np.float64),
+                               np.ascontiguousarray(y0[:, sample], np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
     for path in (4, 2):
         res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=2, path=path, finalize=False)
         dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
-        print(f"cfg4 full size, path {path}: 10 steps, 3 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+        print(f"cfg4 full size, path {path}: 10 steps, 8 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
         assert dx <= TRAJ_TOL and dy <= TRAJ_TOL
+    o = compare_trajectory(B, oracle, torch_mod, og, og["w_fx"], 2, n, R, T, p["seed"], steps=50, path=4, sample=sample,
+                           case="cfg4 full size, hybrid block path, 8 sampled replicas")
+    print(f"cfg4 full size: {fmt_traj(o)}")
+    # quality on a matched replica subset (same seeds on both sides, all T steps) and switch error against the planted haplotype
+    R_sub = 8
+    rsub = B.qhap_bsb_solve(g, replicas=R_sub, steps_total=T, seed=p["seed"], weight_mode=2, path=4)
+    gcut = int(rsub["best_cut"].cpu()[0])
+    gsp = rsub["best_spins"].cpu().numpy()
+    ccut, _ = oracle.cut_eval(og["row_ptr"], og["col"], og["w_fx"], gsp)
+    assert ccut[0] == gcut
+    x0s, y0s = synth.bsb_init_state(p["seed"], n, R_sub)
+    ores = oracle.solve(og["row_ptr"], og["col"], og["w_fx"], (-og["w"]).astype(np.float32), x0s, y0s, steps_total=T,
+                        n_threads=oracle.hardware_threads())
+    covered = np.bincount(fr.snp_idx[fr.allele <= 1], minlength=fr.n_snp) > 0
+    gm = oracle.switch_hamming(oracle.snp_readout(fr.h1, gsp)[covered], fr.hap_a[covered])
+    om = oracle.switch_hamming(oracle.snp_readout(fr.h1, ores["best_spins"])[covered], fr.hap_a[covered])
+    print(f"cfg4 full size, {R_sub} matched replicas x {T} steps: gpu best cut {gcut} oracle {ores['best_cut']}; SE gpu {gm['se']:.5f} oracle {om['se']:.5f}")
+    _record(dict(case="cfg4 full size quality", replicas=R_sub, steps=int(T), gpu_best_cut=gcut, oracle_best_cut=int(ores["best_cut"]),
+                 se_gpu=gm["se"], se_oracle=om["se"]))
+    assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (gcut, ores["best_cut"])
+    assert gm["se"] <= om["se"] + 0.001
 
 
 # ------------------------------------------------------------------- non-default bSB constants on every step path

@@ -1,0 +1,212 @@
+"""GPU tests added in round 2: the workspace contract (exact sizes, guard bands), the dSB force mode (SURVEY 8(f) f4,
+PAPER.md:L71-L77) and the eval_every trace on every step path, against the CPU oracle."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2603_25762_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+GUARD = 1 << 16          # bytes of canary behind every workspace
+CANARY = 0xA5
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests selected (-m gpu) but no CUDA device is visible"
+    from paper_2603_25762_b200 import binding
+    return binding
+
+
+@pytest.fixture()
+def guarded(B, monkeypatch):
+    """Every workspace the binding allocates gets EXACTLY the size the library asked for, followed by a canary band that
+    must come back untouched (a carve that walks past the size the query reported)."""
+    import torch
+    made = []
+
+    def alloc(nbytes):
+        n = max(int(nbytes), 256)
+        n_al = (n + 255) // 256 * 256
+        buf = torch.full((n_al + GUARD,), CANARY, dtype=torch.uint8, device="cuda")
+        made.append((buf, n_al))
+        return buf[:n]
+    monkeypatch.setattr(B, "_workspace", alloc)
+
+    def check():
+        torch.cuda.synchronize()
+        assert made, "no workspace was allocated"
+        for buf, n in made:
+            tail = buf[n:]
+            assert bool((tail == CANARY).all()), f"workspace of {n} bytes: the guard band behind it was written"
+        return len(made)
+    return check
+
+
+def test_workspace_guard_bands_every_entry_point(B, oracle, guarded):
+    """Graph builds, block split, component split / merge, refinement pieces, read-out, cut evaluation and the bSB solve on
+    paths 1-4 (fused and per-step, with and without a remainder CSR) run inside workspaces of exactly the queried size."""
+    import torch
+    fr, p = synth.make_config(1, scale=0.1)
+    dfr = B.upload_frags(fr)
+    g, J = B.qhap_build_read_graph(dfr, weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    for path, kw in ((1, dict(tile_skip=1)), (1, dict(tile_skip=0)), (1, dict(tile_skip=1, step_launch=1)), (2, {}), (4, {}), (4, dict(step_launch=1)),
+                     (4, dict(state16=2))):
+        res = B.qhap_bsb_solve(g, replicas=256, steps_total=p["T"], steps_run=12, seed=3, weight_mode=1, path=path, dense_J=J if path == 1 else None, **kw)
+        assert int(res["best_cut"].cpu()[0]) > 0
+    fr0, p0 = synth.make_config(0)
+    g0, _ = B.qhap_build_read_graph(B.upload_frags(fr0), weight_mode=1)
+    B.qhap_bsb_solve(g0, replicas=64, steps_total=50, seed=1, weight_mode=1, path=3)
+    hap = B.qhap_phase_readout_reads(B.upload_frags(fr0), torch.ones(fr0.n_frag, dtype=torch.int8, device="cuda"))
+    assert hap.numel() == fr0.n_snp
+    B.qhap_cut_eval(g0, 1, torch.ones((fr0.n_frag, 8), dtype=torch.int8, device="cuda"))
+    B.qhap_component_split(g0, 2)
+    # SNP graph, blocks, hybrid path with a remainder CSR (Pore-C long-range edges)
+    fr3, p3 = synth.make_config(3, scale=0.01)
+    d3 = B.upload_frags(fr3)
+    for tenths in (3, 10):
+        g3 = B.qhap_build_snp_graph(d3, tenths, 0.1)
+    win = synth.block_windows(fr3.n_snp, 500, 450)
+    bs = B.qhap_block_split(g3, win)
+    res = B.qhap_bsb_solve(bs, replicas=64, steps_total=100, seed=5, weight_mode=2, path=4)
+    B.qhap_block_stitch(fr3.n_snp, win, res["best_spins"])
+    B.qhap_bsb_solve(bs, replicas=64, steps_total=100, seed=5, weight_mode=2, path=2)
+    fr4, p4 = synth.make_config(4, scale=0.02)
+    g4 = B.qhap_build_snp_graph(B.upload_frags(fr4), 3, 0.1)
+    B.qhap_bsb_solve(g4, replicas=128, steps_total=60, seed=5, weight_mode=2, path=4)
+    B.qhap_snp_refine(g4, replicas=32, steps_total=60, max_iter=2, seed=5, path=4)
+    B.qhap_flip_count_update(torch.ones(g4.n, dtype=torch.int8, device="cuda"), torch.zeros(g4.n, dtype=torch.int32, device="cuda"))
+    B.qhap_component_split(g4, 2)
+    assert guarded() >= 20
+
+
+def test_workspace_one_byte_short_is_refused(B, oracle):
+    """Every path reports the size it needs and refuses a workspace one byte short with QHAP_ERR_WORKSPACE (no partial run)."""
+    import ctypes as C
+    import torch
+    fr, p = synth.make_config(1, scale=0.1)
+    g, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    for path in (1, 2, 4):
+        res = B.qhap_bsb_solve(g, replicas=128, steps_total=50, steps_run=2, seed=1, weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1)
+        need = res["workspace"].numel()
+        with pytest.raises(B.QhapError) as ei:
+            B.qhap_bsb_solve(g, replicas=128, steps_total=50, steps_run=2, seed=1, weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1,
+                             workspace=res["workspace"], workspace_bytes=need - 1)
+        assert ei.value.status == B.QHAP_ERR_WORKSPACE
+
+
+# ------------------------------------------------------------------------------------------------ dSB (force_mode 1)
+def _dsb_case(B, oracle, name):
+    if name == "cfg0":
+        fr, p = synth.make_config(0)
+        g = oracle.read_graph(fr); w = oracle.read_weights(g, 1); mode = 1
+        dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+        return g, w, (-w).astype(np.float32), mode, dg, J, fr.n_frag, p, None
+    if name == "cfg1-scaled":
+        fr, p = synth.make_config(1, scale=0.1)
+        g = oracle.read_graph(fr); w = oracle.read_weights(g, 1); mode = 1
+        dg, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+        return g, w, (-w).astype(np.float32), mode, dg, J, fr.n_frag, p, None
+    fr, p = synth.make_config(3, scale=0.01)
+    g0 = oracle.snp_graph(fr, 3, 0.1)
+    g = oracle.block_split(g0, synth.block_windows(fr.n_snp, 500, 450))
+    return g, g["w_fx"], (-g["w"]).astype(np.float32), 2, B.upload_csr(g), None, g["n"], p, g["inst_ptr"]
+
+
+@pytest.mark.parametrize("name,R", [("cfg0", 48), ("cfg1-scaled", 136), ("cfg3-scaled", 256)])
+def test_dsb_one_step_from_identical_states_every_path(B, oracle, name, R):
+    """dSB, F = J sgn(x): from the SAME fp32 state the force of every path is an exactly representable integer combination
+    (read graphs: exact on the tensor cores, so the step must agree with the fp64 oracle to fp32 rounding, 1e-6; SNP graphs:
+    fp32 weights, 1e-5 as VERDICT r1 asks), at several points of a trajectory that has walls and sign changes."""
+    import torch
+    g, w_int, jval, mode, dg, J, n, p, inst_ptr = _dsb_case(B, oracle, name)
+    T = p["T"]
+    x0, y0 = synth.bsb_init_state(11, n, R)
+    bounds = [(0, n)] if inst_ptr is None else [(int(inst_ptr[b]), int(inst_ptr[b + 1])) for b in range(len(inst_ptr) - 1)]
+
+    def orc(x, y, k, steps):
+        x, y = x.copy(), y.copy()
+        for lo, hi in bounds:
+            rp = (g["row_ptr"][lo:hi + 1] - g["row_ptr"][lo]).astype(np.int32)
+            e = slice(int(g["row_ptr"][lo]), int(g["row_ptr"][hi]))
+            xs, ys = x[lo:hi].copy(), y[lo:hi].copy()
+            oracle.bsb_run(rp, (g["col"][e] - lo).astype(np.int32), jval[e], xs, ys, steps_total=T, step_begin=k, steps_run=steps, n_threads=8, force_mode=1)
+            x[lo:hi], y[lo:hi] = xs, ys
+        return x, y
+    xo, yo = x0.astype(np.float64), y0.astype(np.float64)
+    tol = 1e-6 if mode == 1 else 1e-5
+    paths = [(2, {}), (4, {}), (4, {"step_launch": 1})] + ([(1, {"tile_skip": 1}), (1, {"tile_skip": 0})] if J is not None else []) + \
+        ([(3, {})] if n * R <= 65536 else [])
+    k = 0
+    for seg in (1, 7, 12, 30):                       # compare ONE step at k = 0, 1, 8, 20, 50 (free-running oracle in between)
+        x32, y32 = xo.astype(np.float32), yo.astype(np.float32)
+        xr, yr = orc(x32.astype(np.float64), y32.astype(np.float64), k, 1)
+        for path, kw in paths:
+            xg, yg = torch.from_numpy(x32.copy()).cuda(), torch.from_numpy(y32.copy()).cuda()
+            B.qhap_bsb_solve(dg, replicas=R, steps_total=T, step_begin=k, steps_run=1, weight_mode=mode, path=path, dense_J=J if path == 1 else None,
+                             force_mode=1, x=xg, y=yg, finalize=False, **kw)
+            dx = np.abs(xg.cpu().numpy() - xr).max(); dy = np.abs(yg.cpu().numpy() - yr).max()
+            assert dx <= tol and dy <= tol, (name, path, kw, k, dx, dy)
+        xo, yo = orc(xo, yo, k, seg)
+        k += seg
+    assert np.any(np.abs(xo) == 1.0)                 # walls were reached
+    # dSB differs from bSB on the same state (the flag reaches the kernels)
+    xg, yg = torch.from_numpy(x32.copy()).cuda(), torch.from_numpy(y32.copy()).cuda()
+    B.qhap_bsb_solve(dg, replicas=R, steps_total=T, step_begin=k - seg, steps_run=1, weight_mode=mode, path=2, force_mode=0, x=xg, y=yg, finalize=False)
+    assert np.abs(yg.cpu().numpy() - yr).max() > 1e-3
+
+
+def test_dsb_multi_step_paths_agree_and_solve_quality(B, oracle):
+    """Integer read graph: the dSB force is exact on every path, so 25 steps in one call give the SAME bits on the CSR,
+    resident, dense (fused and per-step) and block paths; and a full dSB solve reaches the oracle's dSB cut - 0.5 %."""
+    import torch
+    g, w, jval, mode, dg, J, n, p, _ = _dsb_case(B, oracle, "cfg0")
+    R, T = p["R"], p["T"]
+    outs = []
+    for path, kw in ((2, {}), (3, {}), (1, {"tile_skip": 1}), (1, {"tile_skip": 1, "step_launch": 1}), (4, {})):
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, steps_run=25, seed=p["seed"], weight_mode=1, path=path, dense_J=J if path == 1 else None,
+                               force_mode=1, finalize=False, **kw)
+        outs.append((res["x"].cpu().numpy(), res["y"].cpu().numpy()))
+    for o in outs[1:]:
+        # same fp32 operations up to the order of an exact integer sum: identical
+        assert np.array_equal(o[0], outs[0][0]) and np.array_equal(o[1], outs[0][1])
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    ores = oracle.solve(g["row_ptr"], g["col"], w, jval, x0, y0, steps_total=T, n_threads=8, force_mode=1)
+    for path in (2, 1, 4):
+        res = B.qhap_bsb_solve(dg, replicas=R, steps_total=T, seed=p["seed"], weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1, force_mode=1)
+        gcut = int(res["best_cut"].cpu()[0])
+        assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (path, gcut, ores["best_cut"])
+        ccut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, res["best_spins"].cpu().numpy())
+        assert ccut[0] == gcut
+
+
+# ------------------------------------------------------------------------------------------------------- eval_every
+@pytest.mark.parametrize("path", [2, 3, 1, 4])
+def test_eval_every_trace(B, oracle, path):
+    """eval_every = k: row j of the trace is the cut of sgn(x) after (j + 1) k steps -- bit-exact against the oracle's cut
+    evaluation of the GPU state taken at those steps by separate resumed calls, and the run with a trace ends in the same
+    state and cuts as the run without one (Fig. 3: best sample per time step)."""
+    import torch
+    g, w, jval, mode, dg, J, n, p, _ = _dsb_case(B, oracle, "cfg0")
+    R, T, k = 48, 200, 30
+    kw = dict(replicas=R, steps_total=T, weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1)
+    res = B.qhap_bsb_solve(dg, seed=4, steps_run=100, eval_every=k, trace_cuts=True, **kw)
+    ref = B.qhap_bsb_solve(dg, seed=4, steps_run=100, **kw)
+    assert torch.equal(res["x"], ref["x"]) and torch.equal(res["y"], ref["y"]) and torch.equal(res["cut"], ref["cut"])
+    assert res["trace_cut"].shape == (3, 1, R) and res["trace_best_cut"].shape == (3, 1)
+    x0, y0 = synth.bsb_init_state(4, n, R)
+    xg, yg = torch.from_numpy(x0.copy()).cuda(), torch.from_numpy(y0.copy()).cuda()
+    for j in range(3):
+        B.qhap_bsb_solve(dg, step_begin=j * k, steps_run=k, x=xg, y=yg, finalize=False, **kw)
+        s = np.where(xg.cpu().numpy() >= 0, 1, -1).astype(np.int8)
+        ecut, _ = oracle.cut_eval(g["row_ptr"], g["col"], w, s)
+        assert np.array_equal(res["trace_cut"][j, 0].cpu().numpy(), ecut)
+        assert int(res["trace_best_cut"][j, 0].cpu()) == int(ecut.max())
+    # against the oracle's own trace: the best cut per evaluation within 0.5 % (same seeds, same replica count)
+    ores = oracle.solve(g["row_ptr"], g["col"], w, jval, x0, y0, steps_total=T, n_threads=4, eval_every=k)
+    for j in range(3):
+        ob = int(ores["trace"][j].max())
+        assert int(res["trace_best_cut"][j, 0].cpu()) >= ob - 0.005 * abs(ob) - 1

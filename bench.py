@@ -6,8 +6,9 @@ A "step" is one pass of the whole hot path ov
 on BASELINE.json config 1 (read-based MHC-like region: ~8,000 HiFi-like reads, R = 1,024, T = 2,000) by default.
 `value` = n * R * T * n_gpus / seconds per step with the fragments already resident in HBM; `e2e` is the same call
 sequence fed from pinned HOST buffers (H2D of the fragment matrix and D2H of the haplotype + best cut inside the timed
-region).  N > 1 (torchrun): every rank runs its own R replicas of the same region (weak scaling, no per-step exchange),
-then 16 bytes per rank are all-gathered to pick the global best replica (paper_2603_25762_b200/parallel.py).
+region).  N > 1 (torchrun, or `--gpus N` from a plain shell, which re-executes itself under torchrun): every rank runs its
+own R replicas of the same region (weak scaling; `--scaling strong` splits ONE seed's R replicas instead), no per-step
+exchange, then 8 bytes per rank are all-gathered to pick the global best replica (paper_2603_25762_b200/parallel.py).
 
 `--config 3` / `--config 4` (not the default; extra measurements of the sparse CSR step) run the SNP-based path instead:
   qhap_build_snp_graph -> [qhap_block_split] -> qhap_bsb_solve (CSR) -> [qhap_block_stitch] -> qhap_phase_readout_snps.
@@ -53,6 +54,11 @@ def parse_args():
                          "steps), 1 = one launch per step; same bits")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU seconds of the oracle sample")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1 on single-instance configs: weak = every rank runs R replicas from its own seed; strong = ONE seed's R "
+                         "replicas are split into contiguous slices (SURVEY 8(e)); config 3 always shards its blocks (strong)")
+    ap.add_argument("--linkage-tenths", type=int, default=0,
+                    help="SNP configs: linkage depth k/10 of the graph build (0 = the config's own, 3; 10 = the paper's exhaustive setting, PAPER.md:L114)")
     ap.add_argument("--refine-iters", type=int, default=0,
                     help="SNP configs with one instance (config 4): also time qhap_snp_refine (Eq. 15-17) with at most this many solves")
     return ap.parse_args()
@@ -155,10 +161,11 @@ def oracle_sample(fr, p, cores, cpu_seconds, R_o=None):
     return dict(n=n, R_o=R_o, T_o=T_o, t_build=t_build, t_bsb=t_bsb, t_read=t_read, edges=int(g["nnz"]) // 2)
 
 
-def extrapolated(s, p):
-    """spin-updates/s of the whole path at the full R, T from a sample: build + bSB scaled by (R T)/(R_o T_o) + readout."""
-    full = s["t_build"] + s["t_bsb"] * (p["R"] * p["T"]) / (s["R_o"] * s["T_o"]) + s["t_read"] * p["R"] / s["R_o"]
-    return s["n"] * p["R"] * p["T"] / full, full
+def sample_value(s):
+    """spin-updates/s of the bounded sample itself: its n x R_o x T_o spin-updates over its whole wall time (graph build +
+    bSB steps + cut + readout).  No extrapolation: `value` and the time it is divided by describe the same run."""
+    t = s["t_build"] + s["t_bsb"] + s["t_read"]
+    return s["n"] * s["R_o"] * s["T_o"] / t, t
 
 
 def run_reference(args):
@@ -170,7 +177,7 @@ def run_reference(args):
     O.build()
     cores = O.hardware_threads()
     fr, p = synth.make_config(args.config)
-    per_step = max(2.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
+    per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
     times, samples = [], []
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
@@ -178,18 +185,18 @@ def run_reference(args):
         dt = time.perf_counter() - t0
         if it >= args.warmup:
             times.append(dt); samples.append(s)
-    vals = [extrapolated(s, p) for s in samples]
+    vals = [sample_value(s) for s in samples]
     value = float(np.mean([v[0] for v in vals]))
     s = samples[-1]
-    sample = (f"per step: full graph build + {s['R_o']} of {p['R']} replicas x {s['T_o']} of {p['T']} bSB steps + cut + readout; "
-              f"value = n R T / (t_build + t_bsb (R T)/(R_o T_o) + t_readout R/R_o)")
+    sample = (f"per step: full graph build + {s['R_o']} of {p['R']} replicas x {s['T_o']} of {p['T']} bSB steps + cut + readout of that sample; "
+              f"value = n R_o T_o / (t_build + t_bsb + t_readout) of the sample itself (no extrapolation)")
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True, "scaling": "weak",
+           "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([v[1] for v in vals])), "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": workload_name(args.config, fr, p), "sampled": sample},
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-           "region_s_extrapolated": float(np.mean([v[1] for v in vals])), "gpu_launches": 0}
+           "bsb_only_value": float(np.mean([x["n"] * x["R_o"] * x["T_o"] / x["t_bsb"] for x in samples])), "gpu_launches": 0}
     print(json.dumps(out), flush=True)
     return 0
 
@@ -207,9 +214,14 @@ def run_ours(args):
     fr, p = synth.make_config(args.config)
     snp = p["graph"] == "snp"
     mode = B.QHAP_WEIGHT_FX if snp else B.QHAP_WEIGHT_D_MINUS_C     # BASELINE.json: "discordant minus concordant"
-    R, T = p["R"], p["T"]
+    T = p["T"]
     n = fr.n_snp if snp else fr.n_frag
-    seed = parallel.rank_seed(p["seed"], rank)
+    blocks_cfg = "block" in p
+    plan = parallel.plan_rank(p["R"], p["seed"], rank, world, "weak" if blocks_cfg else args.scaling)
+    if blocks_cfg:                       # config 3 shards its independent blocks; every rank runs all R replicas of its blocks
+        plan = dict(replicas=p["R"], replica_begin=0, seed=p["seed"], replicas_total=p["R"])
+    R, seed, r_begin = plan["replicas"], plan["seed"], plan["replica_begin"]
+    tenths = args.linkage_tenths or p.get("linkage_tenths", 10)
     if snp:
         assert args.path in ("auto", "sparse", "block"), "the SNP graphs (configs 3, 4) have no dense J"
         # auto: tcgen05 step on the block-compressed J (config 4: tiles for the banded part + remainder CSR for the long-range edges)
@@ -233,9 +245,9 @@ def run_ours(args):
 
     def one_pass(frags):
         if snp:
-            g0 = B.qhap_build_snp_graph(frags, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
+            g0 = B.qhap_build_snp_graph(frags, tenths, p.get("alpha", 0.1))
             g = B.qhap_block_split(g0, win_mine) if win is not None else g0
-            res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, cut_per_replica=False,
+            res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, replica_begin=r_begin, weight_mode=mode, path=path, cut_per_replica=False,
                                    step_launch=args.step_launch, workspace=state.get("ws"))
             state["ws"] = res["workspace"]
             cut, spins = res["best_cut"], res["best_spins"]
@@ -247,8 +259,8 @@ def run_ours(args):
             state["g"] = g
             return cut, hap
         g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype)
-        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip, step_launch=args.step_launch,
-                               cut_per_replica=False, workspace=state.get("ws"))
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, replica_begin=r_begin, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip,
+                               step_launch=args.step_launch, cut_per_replica=False, workspace=state.get("ws"))
         state["ws"] = res["workspace"]
         cut, spins = res["best_cut"], res["best_spins"]
         if world > 1:
@@ -301,7 +313,7 @@ def run_ours(args):
     # sharded over ranks (strong scaling); every other config runs R replicas of the whole instance per rank (weak scaling)
     blocks = win is not None
     n_solved = int((win[:, 1] - win[:, 0]).sum()) if blocks else n
-    work = n_solved * R * T * (1 if blocks else world)
+    work = n_solved * plan["replicas_total"] * T           # whole job: weak = R per rank x world, strong / blocks = R
     value = work / (ms * 1e-3)
     edges = g.nnz // 2
 
@@ -323,7 +335,7 @@ def run_ours(args):
         hap_host[:hap.numel()].copy_(hap, non_blocking=True)
         cut_host.copy_(cut, non_blocking=True)
 
-    e2e_ms, _ = timed(e2e_pass, max(1, min(args.warmup, 2)), max(2, min(args.steps, 3)))
+    e2e_ms, _ = timed(e2e_pass, args.warmup, args.steps)
     e2e_value = work / (e2e_ms * 1e-3)
 
     # ---- phases of one pass (CUDA events around each C-ABI call; one extra untimed-by-the-headline pass)
@@ -333,7 +345,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         ev[0].record()
         if snp:
-            g0 = B.qhap_build_snp_graph(dfr, p.get("linkage_tenths", 10), p.get("alpha", 0.1))
+            g0 = B.qhap_build_snp_graph(dfr, tenths, p.get("alpha", 0.1))
             gg = B.qhap_block_split(g0, win_mine) if win is not None else g0
             JJ = None
         else:
@@ -374,7 +386,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         return r, e0.elapsed_time(e1)
 
-    g_full = B.qhap_build_snp_graph(dfr, p.get("linkage_tenths", 10), p.get("alpha", 0.1)) if snp else \
+    g_full = B.qhap_build_snp_graph(dfr, tenths, p.get("alpha", 0.1)) if snp else \
         B.qhap_build_read_graph(dfr, weight_mode=mode)[0]
     B.qhap_component_split(g_full, 2)                                      # warm-up
     (cs, _perm), cs_ms = timed_once(lambda: B.qhap_component_split(g_full, 2))
@@ -446,15 +458,20 @@ def run_ours(args):
         nz_blocks = int((cnt >= thr).sum())
         rem = cnt[inv] < thr                          # entries that go through the remainder CSR gather
         rem_rows = int(np.unique(rows[rem]).size)
-        # 16 B fp32 state + 4 B fp16 copies written + 4 B read at least once per spin-update, the kept tiles once, and for
-        # the remainder: (col, val) once, one x row gathered per entry, y read-modify-written for the rows that have one
-        alg_bytes = 24.0 * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms + int(rem.sum()) * (8.0 + 4.0 * R) + rem_rows * 8.0 * R
+        # per spin-update: state16 (the 64-wide tiles' default when R % 4 == 0 and no remainder CSR) carries x as
+        # the fp16 pair -- read the pair 4 B, write it 4 B, read y 4 B, write y 4 B = 16 B; the fp32-x kernel adds x read and
+        # written in fp32 = 24 B.  Plus the kept tiles of J once, and for a remainder: (col, val) once, one x row gathered per
+        # entry, y read-modify-written for the rows that have one
+        state16 = (R % 4 == 0) and int(rem.sum()) == 0
+        state_bytes = 16.0 if state16 else 24.0
+        alg_bytes = state_bytes * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms + int(rem.sum()) * (8.0 + 4.0 * R) + rem_rows * 8.0 * R
+        extra["state_bytes_per_spin_update"] = state_bytes
         extra["remainder_nnz"] = int(rem.sum())
         extra["tile_threshold"] = thr
         if int(rem.sum()) > 0:
             extra["roofline_note"] = ("the remainder gathers (4 B x R per far non-zero, SURVEY 8(d)) are counted as algorithmic HBM bytes, but "
                                       "x (%.0f MB) largely stays in the 126 MB L2, so most of them are L2 hits: frac can exceed 1; "
-                                      "state + tiles alone = %.0f MB per launch" % (4e-6 * g.n * R, (24.0 * g.n * R + nz_blocks * 8192.0 * j_terms) / 1e6))
+                                      "state + tiles alone = %.0f MB per launch" % (4e-6 * g.n * R, (state_bytes * g.n * R + nz_blocks * 8192.0 * j_terms) / 1e6))
         roofline = {"kernel": "dense_step_kernel (tile_skip)" if path == 1 else "dense_step_kernel (block-compressed J)", "bound": "hbm", "achieved": alg_bytes / (step_ms * 1e-3) / 1e9,
                     "peak": peaks["hbm"], "unit": "GB/s", "traffic": None, "bytes_per_launch": alg_bytes, "launch_ms": step_ms,
                     "peak_source": peaks["which"], "nonzero_64x64_blocks_of_J": nz_blocks}
@@ -485,13 +502,14 @@ def run_ours(args):
                         rl["traffic"] = float(f[2]) * rl.get("steps_per_launch", 1)      # the CSV holds bytes per bSB step
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if blocks else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if (blocks or (args.scaling == "strong" and world > 1)) else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": workload_name(args.config, fr, p),
                       "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM)" if tile_skip else " full GEMM"),
                                2: "sparse-csr", 3: "shared-memory resident (one launch for all steps)", 4: "tcgen05 step on the block-compressed J (64 x 64 tiles built from the CSR)"}[path],
                       "weight_mode": "fixed-point Eq. 14" if snp else "D-C", "replicas_per_gpu": R, "spins_solved": n_solved, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
-                      "parallelism": f"blocks x{world} (strong)" if blocks else f"replicas x{world} (weak)"},
-           "region_ms": ms, "edges_replicas_per_s": edges * R * T * (1 if blocks else world) / (ms * 1e-3), "undirected_edges": edges,
+                      "parallelism": f"blocks x{world} (strong)" if blocks else f"replicas x{world} ({args.scaling if world > 1 else 'weak'})",
+                      "linkage_tenths": tenths if snp else None},
+           "region_ms": ms, "edges_replicas_per_s": edges * plan["replicas_total"] * T / (ms * 1e-3), "undirected_edges": edges,
            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
            "gpu_launches": int(launches), "bsb_step_launches_per_solve": int(step_launches),
            "clocks": clocks, "roofline": roofline, "phases": phases, "library": B.qhap_version()}
@@ -501,11 +519,11 @@ def run_ours(args):
         O.build()
         cores = O.hardware_threads()
         s = oracle_sample(fr, p, cores, args.cpu_seconds)
-        v, full = extrapolated(s, p)
+        v, t_sample = sample_value(s)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": (f"full graph build ({s['t_build']:.2f} s) + {s['R_o']} of {R} replicas x {s['T_o']} of {T} bSB steps "
-                                          f"({s['t_bsb']:.2f} s) + cut + readout ({s['t_read']:.2f} s), extrapolated to R x T"),
-                               "bsb_only_value": s["n"] * s["R_o"] * s["T_o"] / s["t_bsb"], "region_s_extrapolated": full}
+                                          f"({s['t_bsb']:.2f} s) + cut + readout ({s['t_read']:.2f} s); value = the sample's own n R_o T_o / its wall time"),
+                               "bsb_only_value": s["n"] * s["R_o"] * s["T_o"] / s["t_bsb"], "sample_s": t_sample}
     if rank == 0:
         print(json.dumps(out), flush=True)
     if world > 1:
@@ -516,6 +534,10 @@ def run_ours(args):
 
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        # started as a plain process: become N ranks, one per GPU (the driver's torchrun launch sets WORLD_SIZE itself)
+        from paper_2603_25762_b200 import parallel
+        parallel.spawn_under_torchrun(args.gpus, str(Path(__file__).resolve()), sys.argv[1:])
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

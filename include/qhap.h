@@ -146,6 +146,8 @@ typedef struct {
   double dt, a0;        /* BASELINE.json: 1.25, 1.0                                                       */
   double c0;            /* <= 0: automatic 0.5 sqrt(N-1) / ||J||_F per instance                           */
   uint64_t seed;        /* used when init_state != 0                                                      */
+  int32_t replica_begin;/* global index of this call's replica 0 in the seeded start state (init_state != 0): devices that */
+                        /*    share one seed run disjoint slices [replica_begin, replica_begin + replicas) of its replicas  */
   int32_t weight_mode;  /* QHAP_WEIGHT_*: which CSR arrays define w (J = -w)                              */
   int32_t path;         /* which bSB step kernel:                                                           */
                         /*  1 tcgen05 GEMM over the dense J (needs dense_J, fp16, one instance);              */

@@ -49,7 +49,7 @@ class _BsbTuning(C.Structure):
 class _BsbParams(C.Structure):
     _fields_ = [("replicas", C.c_int32), ("steps_total", C.c_int32), ("step_begin", C.c_int32), ("steps_run", C.c_int32),
                 ("dt", C.c_double), ("a0", C.c_double), ("c0", C.c_double), ("seed", C.c_uint64),
-                ("weight_mode", C.c_int32), ("path", C.c_int32), ("tile_skip", C.c_int32), ("init_state", C.c_int32),
+                ("replica_begin", C.c_int32), ("weight_mode", C.c_int32), ("path", C.c_int32), ("tile_skip", C.c_int32), ("init_state", C.c_int32),
                 ("finalize", C.c_int32), ("force_mode", C.c_int32), ("eval_every", C.c_int32),
                 ("trace_cut", C.c_void_p), ("trace_best_cut", C.c_void_p), ("tuning", C.POINTER(_BsbTuning))]
 
@@ -298,7 +298,7 @@ def qhap_block_split(graph: Csr, windows: np.ndarray) -> Csr:
 
 def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: int = 0, steps_run: Optional[int] = None,
                    dt: float = 1.25, a0: float = 1.0, c0: float = 0.0, seed: int = 0, weight_mode: int = QHAP_WEIGHT_D,
-                   path: int = 0, tile_skip: int = 0, force_mode: int = 0, eval_every: int = 0, trace_cuts: bool = False,
+                   path: int = 0, tile_skip: int = 0, force_mode: int = 0, eval_every: int = 0, trace_cuts: bool = False, replica_begin: int = 0,
                    x: Optional[torch.Tensor] = None, y: Optional[torch.Tensor] = None,
                    dense_J: Optional[torch.Tensor] = None, finalize: bool = True, cut_per_replica: bool = True,
                    workspace: Optional[torch.Tensor] = None, workspace_bytes: Optional[int] = None, **tuning) -> dict:
@@ -324,7 +324,7 @@ def qhap_bsb_solve(graph: Csr, *, replicas: int, steps_total: int, step_begin: i
     tr_best = torch.empty((n_eval, n_inst), dtype=torch.int64, device=dev) if n_eval else None
     tr_cut = torch.empty((n_eval, n_inst, R), dtype=torch.int64, device=dev) if (n_eval and trace_cuts) else None
     tun = _tuning(tuning)
-    p = _BsbParams(R, steps_total, step_begin, steps_run, dt, a0, c0, seed, weight_mode, path, tile_skip, int(init),
+    p = _BsbParams(R, steps_total, step_begin, steps_run, dt, a0, c0, seed, int(replica_begin), weight_mode, path, tile_skip, int(init),
                    int(finalize), int(force_mode), int(eval_every), tr_cut.data_ptr() if tr_cut is not None else None,
                    tr_best.data_ptr() if tr_best is not None else None, C.pointer(tun) if tun is not None else None)
     gs = graph.c_struct()
@@ -447,7 +447,7 @@ def qhap_snp_refine(graph: Csr, *, replicas: int, steps_total: int, max_iter: in
     x = torch.empty((n, R), dtype=torch.float32, device=dev)
     y = torch.empty((n, R), dtype=torch.float32, device=dev)
     flip = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
-    p = _BsbParams(R, steps_total, 0, steps_total, dt, a0, c0, seed, QHAP_WEIGHT_FX, path, 0, 1, 1, 0, 0, None, None, None)
+    p = _BsbParams(R, steps_total, 0, steps_total, dt, a0, c0, seed, 0, QHAP_WEIGHT_FX, path, 0, 1, 1, 0, 0, None, None, None)
     gs = graph.c_struct()
     iters = C.c_int32(0)
     cuts = (C.c_int64 * max_iter)()

@@ -1121,7 +1121,7 @@ void choose_staging(DenseArgs& a, int stage_bytes, const qhap_bsb_tuning& t) {
     return std::min(kMaxStages, (kSmemBudget - (a.stage_out ? bufs * 2 * kStageX : 0) - ring_bytes) / stage_bytes);
   };
   int bufs = (t.dense_stg_bufs == 1 || t.dense_stg_bufs == 2) ? t.dense_stg_bufs : ((a.stage_out && stages(1) > stages(2) && stages(2) < 3) ? 1 : 2);
-  if (a.x16) bufs = 2;
+  if (a.x16 && t.dense_stg_bufs != 1) bufs = 2;
   a.stg_bufs = uint32_t(bufs);
   a.n_stages = stages(bufs);
   a.store_warp = (bufs == 1 || a.x16) ? 1u : 0u;        // launch_fused sets it too

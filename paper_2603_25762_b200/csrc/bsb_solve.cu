@@ -77,6 +77,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   QHAP_REQUIRE(p->weight_mode >= 0 && p->weight_mode <= 2, "bad weight_mode");
   QHAP_REQUIRE(p->force_mode == 0 || p->force_mode == 1, "force_mode must be 0 (bSB) or 1 (dSB)");
   QHAP_REQUIRE(p->eval_every >= 0, "eval_every must be >= 0");
+  QHAP_REQUIRE(p->replica_begin >= 0, "replica_begin must be >= 0");
   QHAP_REQUIRE(n_inst == 1 || inst_ptr, "inst_ptr (host) is required for n_inst > 1");
   if (p->tuning)
     for (int32_t v : p->tuning->reserved) QHAP_REQUIRE(v == 0, "qhap_bsb_tuning.reserved must be 0");
@@ -115,7 +116,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   }
   QHAP_TRY(materialize_jval(g, p->weight_mode, n_inst, s.inst_ptr, s.jval, s.sumsq, stream));
   QHAP_TRY(compute_c1(n, n_inst, s.inst_ptr, s.sumsq, p->dt, p->c0, s.c1, stream));
-  if (p->init_state && p->step_begin == 0) QHAP_TRY(init_state(n, R, p->seed, x, y, stream));
+  if (p->init_state && p->step_begin == 0) QHAP_TRY(init_state(n, R, p->seed, p->replica_begin, x, y, stream));
 
   // eval_every = k: the steps run in pieces of k, each followed by a cut evaluation of sgn(x) (Fig. 3)
   const bool tracing = p->eval_every > 0 && (p->trace_cut || p->trace_best_cut);

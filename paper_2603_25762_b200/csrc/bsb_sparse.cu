@@ -73,12 +73,12 @@ __device__ __forceinline__ uint64_t splitmix64(uint64_t z) {
 
 // x0, y0 ~ U(-0.1, 0.1): idx = (r n + i) 2 + {0: x, 1: y}; z = splitmix64(seed + GOLDEN (idx + 1)); u = z >> 40;
 // value = fp32( fp64(2u + 1 - 2^24) * fp64(0.1 / 2^24) )   (R11; same formula as synth.bsb_init_state)
-__global__ void __launch_bounds__(256) init_state_kernel(int64_t n, int32_t R, uint64_t seed, float* __restrict__ x,
+__global__ void __launch_bounds__(256) init_state_kernel(int64_t n, int32_t R, uint64_t seed, int32_t r0, float* __restrict__ x,
                                                          float* __restrict__ y) {
   const int64_t total = n * R;
   for (int64_t p = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; p < total; p += int64_t(gridDim.x) * blockDim.x) {
     const int64_t i = p / R, r = p % R;
-    const uint64_t base = (uint64_t(r) * uint64_t(n) + uint64_t(i)) * 2ull;
+    const uint64_t base = (uint64_t(r0 + r) * uint64_t(n) + uint64_t(i)) * 2ull;      // r0 + r: the GLOBAL replica index
 #pragma unroll
     for (int which = 0; which < 2; ++which) {
       const uint64_t z = splitmix64(seed + 0x9E3779B97F4A7C15ull * (base + which + 1ull));
@@ -219,10 +219,10 @@ qhap_status compute_c1(int32_t n, int32_t n_inst, const int32_t* inst_ptr_dev, c
   return QHAP_OK;
 }
 
-qhap_status init_state(int64_t n, int32_t R, uint64_t seed, float* x, float* y, cudaStream_t stream) {
+qhap_status init_state(int64_t n, int32_t R, uint64_t seed, int32_t replica_begin, float* x, float* y, cudaStream_t stream) {
   if (n * R == 0) return QHAP_OK;
   const int blocks = int(std::min<int64_t>(ceil_div(n * R, 256), int64_t(sm_count()) * 16));
-  init_state_kernel<<<blocks, 256, 0, stream>>>(n, R, seed, x, y);
+  init_state_kernel<<<blocks, 256, 0, stream>>>(n, R, seed, replica_begin, x, y);
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;
 }

@@ -54,7 +54,7 @@ qhap_status materialize_jval(const CsrView& g, int mode, int32_t n_inst, const i
 // c1[inst] = (float)(dt * c0_inst), c0_inst = c0 > 0 ? c0 : 0.5 sqrt(N_inst - 1) / sqrt(sumsq[inst])  (1.0 if undefined)
 qhap_status compute_c1(int32_t n, int32_t n_inst, const int32_t* inst_ptr_dev, const double* sumsq, double dt, double c0,
                        float* c1, cudaStream_t stream);
-qhap_status init_state(int64_t n, int32_t R, uint64_t seed, float* x, float* y, cudaStream_t stream);
+qhap_status init_state(int64_t n, int32_t R, uint64_t seed, int32_t replica_begin, float* x, float* y, cudaStream_t stream);
 // one bSB step on the CSR path: x_out, y (in place) from x_in; force_mode 1 (dSB): F = J sgn(x_in)
 qhap_status sparse_step(const CsrView& g, const float* jval, int32_t R, int32_t n_inst, const int32_t* inst_ptr_dev,
                         const float* c1, StepConsts k, int32_t force_mode, const float* x_in, float* x_out, float* y,

@@ -43,6 +43,31 @@ def rank_seed(seed: int, rank: int) -> int:
     return (int(seed) + 0x632BE59BD9B4E019 * int(rank)) & 0xFFFFFFFFFFFFFFFF
 
 
+def plan_rank(replicas: int, seed: int, rank: int, world: int, scaling: str) -> dict:
+    """What one rank runs.  "weak": every rank runs `replicas` replicas of the region from its own seed (per-GPU work
+    fixed).  "strong": ONE seed's `replicas` replicas are split into contiguous slices; rank r starts the
+    device-side seeded state at global replica `replica_begin`, so the union over the ranks is exactly the single-GPU run
+    and the lowest rank that holds the maximal cut also holds the lowest global replica index."""
+    if scaling == "weak" or world == 1:
+        return dict(replicas=int(replicas), replica_begin=0, seed=rank_seed(seed, rank), replicas_total=int(replicas) * int(world))
+    assert scaling == "strong", scaling
+    b, e = replica_shard(replicas, rank, world)
+    return dict(replicas=e - b, replica_begin=b, seed=int(seed), replicas_total=int(replicas))
+
+
+def spawn_under_torchrun(n_gpus: int, script: str, argv: list) -> None:
+    """`bench.py --gpus N` started as a plain process: re-exec it as N ranks (one per GPU) under torch.distributed.run with
+    a loopback rendezvous.  Does not return."""
+    import socket
+    import sys
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={int(n_gpus)}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), script] + list(argv)
+    os.execv(sys.executable, cmd)
+
+
 def select_best_across_ranks(best_cut: torch.Tensor, best_spins: torch.Tensor) -> Tuple[torch.Tensor, torch.Tensor, int]:
     """All ranks return (global best cut [n_inst] int64, its spins [n] int8, winning rank of instance 0).
 

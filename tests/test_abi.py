@@ -67,7 +67,7 @@ def test_size_query_and_loud_failure_without_gpu(lib):
     assert ws2.value > ws.value
     assert lib.qhap_build_snp_graph(C.byref(fr), C.c_int32(11), C.c_double(0.1), None, C.byref(g), None, C.byref(ws2), None) == B.QHAP_ERR_INVALID_ARG
     assert b"linkage_tenths" in lib.qhap_last_error()
-    p = B._BsbParams(64, 100, 0, 100, 1.25, 1.0, 0.0, 1, 0, 2, 0, 1, 1, 0)
+    p = B._BsbParams(64, 100, 0, 100, 1.25, 1.0, 0.0, 1, 0, 0, 2, 0, 1, 1, 0)
     ws3 = C.c_size_t(0)
     g.nnz = 50
     assert lib.qhap_bsb_solve(C.byref(g), 1, None, None, 0, 0, C.byref(p), None, None, None, None, None, None, None, C.byref(ws3), None) == B.QHAP_OK

@@ -47,6 +47,51 @@ def test_select_best_across_two_ranks(tmp_path, cuts, expect):
     assert np.array_equal(got[0][2:], exp_spins)
 
 
+def _rank_logic_worker(rank: int, world: int, port: int, R: int, n: int, scaling: str, out_dir: str):
+    """bench.py's rank logic end to end on CPU tensors: plan_rank -> (stand-in for the solve: a cut per GLOBAL replica id and
+    seed, spins that encode them) -> local best (lowest index on ties) -> select_best_across_ranks."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    r, w, _ = parallel.init_from_env(backend="gloo")
+    plan = parallel.plan_rank(R, 20260001, r, w, scaling)
+    gids = np.arange(plan["replica_begin"], plan["replica_begin"] + plan["replicas"], dtype=np.int64)
+    cuts = _fake_cuts(plan["seed"], gids)
+    lb = int(np.flatnonzero(cuts == cuts.max())[0]) if len(cuts) else 0
+    best = torch.tensor([int(cuts[lb]) if len(cuts) else -(1 << 60)], dtype=torch.int64)
+    spins = torch.from_numpy(_fake_spins(plan["seed"], int(gids[lb]) if len(gids) else -1, n))
+    cut, win_spins, winner = parallel.select_best_across_ranks(best, spins)
+    np.save(os.path.join(out_dir, f"r{rank}.npy"), np.concatenate([[int(cut[0]), winner, plan["replicas"], plan["replica_begin"]],
+                                                                     win_spins.numpy().astype(np.int64)]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def _fake_cuts(seed: int, gids: np.ndarray) -> np.ndarray:
+    return ((gids * 2654435761 + (seed % 1000003)) % 97).astype(np.int64)          # many ties on purpose
+
+
+def _fake_spins(seed: int, gid: int, n: int) -> np.ndarray:
+    return np.where((np.arange(n) + gid + seed % 7) % 3 == 0, 1, -1).astype(np.int8)
+
+
+@pytest.mark.parametrize("scaling", ["strong", "weak"])
+def test_bench_rank_logic_two_ranks(tmp_path, scaling):
+    R, n, world, seed = 37, 24, 2, 20260001
+    mp.spawn(_rank_logic_worker, args=(world, _free_port(), R, n, scaling, str(tmp_path)), nprocs=world, join=True)
+    got = [np.load(tmp_path / f"r{r}.npy") for r in range(world)]
+    assert np.array_equal(got[0][:2], got[1][:2]) and np.array_equal(got[0][4:], got[1][4:])
+    if scaling == "strong":
+        # the union over the ranks is the single-GPU run: same best cut, and the spins of the LOWEST global replica holding it
+        assert got[0][2] + got[1][2] == R and got[0][3] == 0 and got[1][3] == got[0][2]
+        cuts = _fake_cuts(seed, np.arange(R, dtype=np.int64))
+        gbest = int(np.flatnonzero(cuts == cuts.max())[0])
+        assert got[0][0] == cuts.max() and got[0][1] == (0 if gbest < got[0][2] else 1)
+        assert np.array_equal(got[0][4:], _fake_spins(seed, gbest, n))
+    else:
+        assert got[0][2] == got[1][2] == R and got[0][3] == got[1][3] == 0
+        per_rank = [_fake_cuts(parallel.rank_seed(seed, r), np.arange(R, dtype=np.int64)).max() for r in range(world)]
+        assert got[0][0] == max(per_rank) and got[0][1] == int(np.argmax(per_rank))
+
+
 def test_shards_partition_the_work():
     for total, world in [(1024, 8), (10, 3), (2, 4), (0, 2)]:
         spans = [parallel.replica_shard(total, r, world) for r in range(world)]

@@ -18,6 +18,7 @@ struct SolveWs {
   int64_t* wtot;
   int64_t* best_cut;
   int32_t* best_replica;
+  uint32_t* bits;     // packed signs for the cut evaluation
   void* dense;
   size_t dense_bytes;
 };
@@ -33,6 +34,7 @@ SolveWs carve(Workspace& ws, int32_t n, int64_t nnz, int32_t n_inst, int32_t R, 
   s.wtot = ws.take<int64_t>(size_t(n_inst));
   s.best_cut = ws.take<int64_t>(size_t(n_inst));
   s.best_replica = ws.take<int32_t>(size_t(n_inst));
+  s.bits = ws.take<uint32_t>(cut_bits_words(n, R));
   s.dense_bytes = dense ? dense_workspace_bytes(n, ld, R) : (block ? block_workspace_bytes(n, nnz, R) : 0);
   s.dense = (dense || block) ? static_cast<void*>(ws.take<char>(s.dense_bytes)) : nullptr;
   return s;
@@ -130,7 +132,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
     k += pc.steps_run;
     if (tracing && pc.steps_run == p->eval_every) {
       int64_t* cut = p->trace_cut ? p->trace_cut + size_t(row) * n_inst * R : s.cut;
-      QHAP_TRY(cut_from_x(g, p->weight_mode, x, R, n_inst, s.inst_ptr, cut, s.wtot, stream));
+      QHAP_TRY(cut_from_x(g, p->weight_mode, x, R, n_inst, s.inst_ptr, cut, s.wtot, s.bits, stream));
       if (p->trace_best_cut)
         QHAP_TRY(cut_finalize(n_inst, R, cut, s.wtot, nullptr, p->trace_best_cut + size_t(row) * n_inst, s.best_replica, stream));
       ++row;
@@ -139,7 +141,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   if (p->finalize) {
     QHAP_REQUIRE(best_spins && best_cut && best_replica, "best_spins, best_cut, best_replica must not be NULL when finalize != 0");
     int64_t* cut = cut_per_replica ? cut_per_replica : s.cut;
-    QHAP_TRY(cut_from_x(g, p->weight_mode, x, R, n_inst, s.inst_ptr, cut, s.wtot, stream));
+    QHAP_TRY(cut_from_x(g, p->weight_mode, x, R, n_inst, s.inst_ptr, cut, s.wtot, s.bits, stream));
     QHAP_TRY(cut_finalize(n_inst, R, cut, s.wtot, nullptr, best_cut, best_replica, stream));
     QHAP_TRY(gather_best_spins(n, R, x, n_inst, s.inst_ptr, best_replica, best_spins, stream));
   }
@@ -154,6 +156,7 @@ extern "C" qhap_status qhap_cut_eval(const qhap_csr* graph, int32_t weight_mode,
   Workspace ws(workspace);
   int64_t* wtot = ws.take<int64_t>(1);
   int32_t* inst_ptr = ws.take<int32_t>(2);
+  uint32_t* bits = ws.take<uint32_t>(cut_bits_words(graph->n, replicas));
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
@@ -163,7 +166,7 @@ extern "C" qhap_status qhap_cut_eval(const qhap_csr* graph, int32_t weight_mode,
   else QHAP_REQUIRE(graph->nnz == 0 || (graph->d && (weight_mode == 0 || graph->c)), "d (and c) required for weight_mode 0/1");
   cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
   const CsrView g = view_of(*graph);
-  QHAP_TRY(cut_from_spins(g, weight_mode, spins, replicas, 1, inst_ptr, cut, wtot, stream));
+  QHAP_TRY(cut_from_spins(g, weight_mode, spins, replicas, 1, inst_ptr, cut, wtot, bits, stream));
   QHAP_TRY(cut_finalize(1, replicas, cut, wtot, energy, nullptr, nullptr, stream));
   return QHAP_OK;
 }

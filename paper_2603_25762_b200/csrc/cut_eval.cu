@@ -1,9 +1,11 @@
 // (5) Cut / Ising-energy evaluation and best-replica selection.  PAPER.md:L254-L267 [Eq. 4-6].
 //   cut_r = sum_{a<b, s_a != s_b} w_ab,  E_r = W_tot - 2 cut_r,  r* = lowest r with maximal cut.
 // Integer arithmetic only (int32 counts or int64 2^-32 fixed point) -> bit-exact and order independent.
-// Layout: lanes run across replicas (the contiguous dimension of spins[n][R] / x[n][R]); a warp owns a tile of
-// consecutive rows and a chunk of 32*VEC replicas, keeps VEC int64 partial cuts per lane in registers and flushes them
-// with one atomicAdd per (lane, slot) when its tile (or the instance) ends.
+// The signs are first packed to one bit per (spin, replica) (pack_signs_kernel: 4 n R bytes of x read once, n R / 8 bytes
+// written); the accumulation then runs on the packed words: lanes across replicas, a warp owns a tile of consecutive rows and
+// a chunk of 32*VEC replicas, keeps VEC int64 partial cuts per lane in registers and flushes them with one atomicAdd per
+// (lane, slot) when its tile (or the instance) ends.  Per edge a warp reads 4-16 bytes of packed signs instead of the
+// neighbour's 128-512 bytes of fp32 x.
 #include "kernels.cuh"
 
 namespace qhap {
@@ -12,33 +14,50 @@ namespace {
 
 constexpr int kRowsPerWarp = 8;   // a CTA of 8 warps owns 64 consecutive rows and one chunk of replicas
 
+// Packed signs: one bit per (spin, replica), word w of row a holds replicas 32 w .. 32 w + 31, bit set = spin -1.
+// The accumulation kernel reads these words (R / 8 bytes per row) instead of gathering the neighbour's fp32 x row
+// (4 R bytes) for every edge.
+struct PackedBits {};
+
 template <class SpinT, int VEC>
 struct SpinLoad;
 
-// int8 spins, 4 per 32-bit word: returns a mask with bit k set when replica k is -1.
+// load(base, row, R, r) returns a mask with bit k set when replica r + k of `row` is -1.
 template <>
-struct SpinLoad<int8_t, 4> {
-  static __device__ __forceinline__ uint32_t load(const int8_t* p) {
-    uint32_t v = *reinterpret_cast<const uint32_t*>(p);
-    return ((v >> 7) & 1u) | ((v >> 14) & 2u) | ((v >> 21) & 4u) | ((v >> 28) & 8u);
+struct SpinLoad<PackedBits, 4> {
+  static __device__ __forceinline__ uint32_t load(const PackedBits* base, int32_t row, int32_t R, int r) {
+    const uint32_t W = uint32_t(R + 31) >> 5;
+    const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(base) + size_t(row) * W + (uint32_t(r) >> 5));
+    return (w >> (uint32_t(r) & 31u)) & 0xFu;                  // r is a multiple of 4: the four bits do not straddle a word
   }
 };
 template <>
-struct SpinLoad<int8_t, 1> {
-  static __device__ __forceinline__ uint32_t load(const int8_t* p) { return (*p < 0) ? 1u : 0u; }
-};
-// fp32 positions: s = +1 if x >= 0 else -1 (R10e)
-template <>
-struct SpinLoad<float, 4> {
-  static __device__ __forceinline__ uint32_t load(const float* p) {
-    float4 v = *reinterpret_cast<const float4*>(p);
-    return (v.x >= 0.f ? 0u : 1u) | (v.y >= 0.f ? 0u : 2u) | (v.z >= 0.f ? 0u : 4u) | (v.w >= 0.f ? 0u : 8u);
+struct SpinLoad<PackedBits, 1> {
+  static __device__ __forceinline__ uint32_t load(const PackedBits* base, int32_t row, int32_t R, int r) {
+    const uint32_t W = uint32_t(R + 31) >> 5;
+    const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(base) + size_t(row) * W + (uint32_t(r) >> 5));
+    return (w >> (uint32_t(r) & 31u)) & 1u;
   }
 };
-template <>
-struct SpinLoad<float, 1> {
-  static __device__ __forceinline__ uint32_t load(const float* p) { return (*p >= 0.f) ? 0u : 1u; }
-};
+
+// sign sources of the packing kernel: int8 spins or fp32 positions (s = +1 if x >= 0 else -1, R10e)
+__device__ __forceinline__ bool is_minus(int8_t v) { return v < 0; }
+__device__ __forceinline__ bool is_minus(float v) { return !(v >= 0.f); }
+
+// One warp per row: 32 replicas per ballot -> one word.
+template <class SrcT>
+__global__ void __launch_bounds__(256) pack_signs_kernel(int32_t n, int32_t R, const SrcT* __restrict__ src, uint32_t* __restrict__ bits) {
+  const int lane = threadIdx.x & 31;
+  const int32_t W = (R + 31) >> 5;
+  const int64_t n_items = int64_t(n) * W;
+  for (int64_t it = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5; it < n_items; it += (int64_t(gridDim.x) * blockDim.x) >> 5) {
+    const int32_t a = int32_t(it / W), w = int32_t(it % W);
+    const int r = w * 32 + lane;
+    const bool m = r < R && is_minus(src[size_t(a) * R + r]);
+    const uint32_t word = __ballot_sync(0xffffffffu, m);
+    if (lane == 0) bits[it] = word;
+  }
+}
 
 template <class SpinT, int VEC>
 __global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const int32_t* __restrict__ row_ptr,
@@ -106,7 +125,7 @@ __global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const in
         while (a >= inst_ptr[inst + 1]) ++inst;
       }
       const int32_t e0 = row_ptr[a], e1 = row_ptr[a + 1];
-      const uint32_t sa = active ? SpinLoad<SpinT, VEC>::load(spins + size_t(a) * R + r) : 0u;
+      const uint32_t sa = active ? SpinLoad<SpinT, VEC>::load(spins, a, R, r) : 0u;
       for (int32_t eb = e0; eb < e1; eb += 32) {
         // lanes fetch 32 entries, then broadcast them one by one
         const int32_t e = eb + lane;
@@ -118,11 +137,11 @@ __global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const in
         }
         if (chunk == 0 && my_col > a) wsum += my_w;
         const int cnt = min(32, e1 - eb);
-        for (int j = 0; j < cnt; ++j) {
+        for (int j = 0; j < cnt; ++j) {            // every lane takes part in the shuffles; lower-triangle entries are skipped
           const int32_t b = __shfl_sync(0xffffffffu, my_col, j);
           const int64_t w = __shfl_sync(0xffffffffu, my_w, j);
           if (b <= a || !active) continue;
-          const uint32_t diff = sa ^ SpinLoad<SpinT, VEC>::load(spins + size_t(b) * R + r);
+          const uint32_t diff = sa ^ SpinLoad<SpinT, VEC>::load(spins, b, R, r);
 #pragma unroll
           for (int k = 0; k < VEC; ++k) acc[k] += ((diff >> k) & 1u) ? w : 0;
         }
@@ -207,38 +226,44 @@ __global__ void __launch_bounds__(256) gather_best_spins_kernel(int32_t n, int32
   best_spins[a] = (x[size_t(a) * R + best_replica[inst]] >= 0.f) ? int8_t(1) : int8_t(-1);
 }
 
-template <class SpinT>
-qhap_status launch_cut(const CsrView& g, int mode, const SpinT* spins, int32_t R, int32_t n_inst,
-                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream) {
+template <class SrcT>
+qhap_status launch_cut(const CsrView& g, int mode, const SrcT* src, int32_t R, int32_t n_inst,
+                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, uint32_t* bits, cudaStream_t stream) {
   QHAP_CUDA_TRY(cudaMemsetAsync(cut, 0, sizeof(int64_t) * size_t(n_inst) * R, stream));
   QHAP_CUDA_TRY(cudaMemsetAsync(wtot, 0, sizeof(int64_t) * size_t(n_inst), stream));
   if (g.n == 0 || R == 0) return QHAP_OK;
-  const bool vec4 = (R % 4 == 0) && ((reinterpret_cast<uintptr_t>(spins) & (4 * sizeof(SpinT) - 1)) == 0);
+  const int64_t items = int64_t(g.n) * ((R + 31) / 32);
+  pack_signs_kernel<SrcT><<<int(std::min<int64_t>(ceil_div(items, 8), int64_t(sm_count()) * 16)), 256, 0, stream>>>(g.n, R, src, bits);
+  QHAP_LAUNCH_CHECK();
+  const bool vec4 = R % 4 == 0;
   const int chunks = vec4 ? (R + 127) / 128 : (R + 31) / 32;
   const int64_t work = ceil_div(g.n, 8 * kRowsPerWarp) * chunks;
   const int blocks = int(std::max<int64_t>(1, std::min<int64_t>(work, int64_t(sm_count()) * 8)));
   auto* cu = reinterpret_cast<unsigned long long*>(cut);
   auto* wt = reinterpret_cast<unsigned long long*>(wtot);
+  const PackedBits* pb = reinterpret_cast<const PackedBits*>(bits);
   if (vec4)
-    cut_accumulate_kernel<SpinT, 4><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, spins, R,
-                                                                n_inst, inst_ptr_dev, cu, wt);
+    cut_accumulate_kernel<PackedBits, 4><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, pb, R,
+                                                                     n_inst, inst_ptr_dev, cu, wt);
   else
-    cut_accumulate_kernel<SpinT, 1><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, spins, R,
-                                                                n_inst, inst_ptr_dev, cu, wt);
+    cut_accumulate_kernel<PackedBits, 1><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, pb, R,
+                                                                     n_inst, inst_ptr_dev, cu, wt);
   QHAP_LAUNCH_CHECK();
   return QHAP_OK;
 }
 
 }  // namespace
 
+size_t cut_bits_words(int32_t n, int32_t R) { return size_t(n) * size_t((R + 31) / 32); }
+
 qhap_status cut_from_spins(const CsrView& g, int mode, const int8_t* spins, int32_t R, int32_t n_inst,
-                           const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream) {
-  return launch_cut<int8_t>(g, mode, spins, R, n_inst, inst_ptr_dev, cut, wtot, stream);
+                           const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, uint32_t* bits, cudaStream_t stream) {
+  return launch_cut<int8_t>(g, mode, spins, R, n_inst, inst_ptr_dev, cut, wtot, bits, stream);
 }
 
 qhap_status cut_from_x(const CsrView& g, int mode, const float* x, int32_t R, int32_t n_inst,
-                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream) {
-  return launch_cut<float>(g, mode, x, R, n_inst, inst_ptr_dev, cut, wtot, stream);
+                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, uint32_t* bits, cudaStream_t stream) {
+  return launch_cut<float>(g, mode, x, R, n_inst, inst_ptr_dev, cut, wtot, bits, stream);
 }
 
 qhap_status cut_finalize(int32_t n_inst, int32_t R, const int64_t* cut, const int64_t* wtot, int64_t* energy,

@@ -38,10 +38,12 @@ struct StepConsts {
 };
 
 // ---- cut_eval.cu
+// `bits`: scratch of cut_bits_words(n, R) uint32 (the signs packed to one bit per (spin, replica))
+size_t cut_bits_words(int32_t n, int32_t R);
 qhap_status cut_from_spins(const CsrView& g, int mode, const int8_t* spins, int32_t R, int32_t n_inst,
-                           const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream);
+                           const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, uint32_t* bits, cudaStream_t stream);
 qhap_status cut_from_x(const CsrView& g, int mode, const float* x, int32_t R, int32_t n_inst,
-                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, cudaStream_t stream);
+                       const int32_t* inst_ptr_dev, int64_t* cut, int64_t* wtot, uint32_t* bits, cudaStream_t stream);
 qhap_status cut_finalize(int32_t n_inst, int32_t R, const int64_t* cut, const int64_t* wtot, int64_t* energy,
                          int64_t* best_cut, int32_t* best_replica, cudaStream_t stream);
 qhap_status gather_best_spins(int32_t n, int32_t R, const float* x, int32_t n_inst, const int32_t* inst_ptr_dev,

@@ -4,10 +4,13 @@
 // components as ONE block-diagonal CSR + perm (new index -> old vertex) + a host inst_ptr, i.e. exactly the batch
 // format qhap_bsb_solve takes (per-component c0 and best replica).
 // Labels: min-label hooking + pointer jumping (every vertex ends with the smallest vertex of its component as parent;
-// integer atomicMin only -> the result does not depend on the execution order).  The grouping of vertices by label is
-// index arithmetic done on the host (like the block windows of qhap_block_split).
+// integer atomicMin only -> the result does not depend on the execution order).  The grouping of the vertices by label runs
+// on the device too: component sizes (integer atomics), two exclusive scans over the roots (offsets and component
+// numbers, both in ascending root order), one stable radix sort of the vertices by component number (library primitive:
+// cub::DeviceRadixSort) and index arithmetic.  The host only reads back the counts and inst_ptr.
 #include <algorithm>
-#include <vector>
+
+#include <cub/device/device_radix_sort.cuh>
 
 #include "kernels.cuh"
 
@@ -49,6 +52,46 @@ __global__ void __launch_bounds__(256) cc_jump_kernel(int32_t n, int32_t* __rest
     parent[i] = gp;
     *changed = 1;
   }
+}
+
+// size[label] += 1 for every vertex
+__global__ void __launch_bounds__(256) cc_size_kernel(int32_t n, const int32_t* __restrict__ parent, int32_t* __restrict__ size) {
+  const int32_t v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v < n) atomicAdd(size + parent[v], 1);
+}
+
+// per root r (ascending): cnt[r] = size of the component if it is kept, ind[r] = 1 if it is kept
+__global__ void __launch_bounds__(256) cc_keep_kernel(int32_t n, int32_t min_size, const int32_t* __restrict__ parent,
+                                                      const int32_t* __restrict__ size, int32_t* __restrict__ cnt, int32_t* __restrict__ ind) {
+  const int32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n) return;
+  const bool keep = parent[r] == r && size[r] >= min_size;
+  cnt[r] = keep ? size[r] : 0;
+  ind[r] = keep ? 1 : 0;
+}
+
+// sort key of vertex v = number of its component among the kept ones (dropped: INT_MAX); inst[number] = offset of the component
+__global__ void __launch_bounds__(256) cc_key_kernel(int32_t n, int32_t min_size, const int32_t* __restrict__ parent,
+                                                     const int32_t* __restrict__ size, const int32_t* __restrict__ start,
+                                                     const int32_t* __restrict__ cidx, int32_t* __restrict__ key, int32_t* __restrict__ val,
+                                                     int32_t* __restrict__ inst) {
+  const int32_t v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= n) return;
+  const int32_t r = parent[v];
+  const bool keep = size[r] >= min_size;
+  key[v] = keep ? cidx[r] : 0x7fffffff;
+  val[v] = v;
+  if (keep && r == v) inst[cidx[r]] = start[r];
+  if (v == 0) inst[cidx[n]] = start[n];                 // cidx[n] = number of kept components, start[n] = kept vertices
+}
+
+// perm[i] = i-th vertex in (component, vertex) order; inv[v] = its new index, -1 for dropped vertices
+__global__ void __launch_bounds__(256) cc_perm_kernel(int32_t n, const int32_t* __restrict__ m_dev, const int32_t* __restrict__ sorted,
+                                                      int32_t* __restrict__ perm, int32_t* __restrict__ inv) {
+  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t v = sorted[i];
+  if (i < *m_dev) { perm[i] = v; inv[v] = i; } else inv[v] = -1;
 }
 
 __global__ void __launch_bounds__(256) cc_degree_kernel(int32_t m, const int32_t* __restrict__ perm, const int32_t* __restrict__ row_ptr,
@@ -96,8 +139,24 @@ extern "C" qhap_status qhap_component_split(const qhap_csr* graph, int32_t min_s
   int32_t* parent = ws.take<int32_t>(size_t(n) + 1);
   int32_t* inv = ws.take<int32_t>(size_t(n) + 1);
   int32_t* flag = ws.take<int32_t>(4);
-  int64_t* totals = ws.take<int64_t>(2);
+  int64_t* totals = ws.take<int64_t>(4);
   int64_t* scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(graph->n), 4096)) + 1);
+  int32_t* size = ws.take<int32_t>(size_t(n) + 1);
+  int32_t* cnt = ws.take<int32_t>(size_t(n) + 1);       // kept sizes per root, then their exclusive scan (start)
+  int32_t* cidx = ws.take<int32_t>(size_t(n) + 1);      // kept indicator per root, then its exclusive scan (component number)
+  int32_t* key = ws.take<int32_t>(size_t(n) + 1);
+  int32_t* val = ws.take<int32_t>(size_t(n) + 1);
+  int32_t* key2 = ws.take<int32_t>(size_t(n) + 1);
+  int32_t* val2 = ws.take<int32_t>(size_t(n) + 1);
+  int32_t* inst_dev = ws.take<int32_t>(size_t(n) + 2);
+  // scratch of the radix sort: CUB's own query, which launches nothing (a bound is used should the query fail, e.g. without a device)
+  size_t sort_bytes = 0;
+  if (cub::DeviceRadixSort::SortPairs(nullptr, sort_bytes, key, key2, val, val2, std::max(n, 1)) != cudaSuccess) {
+    (void)cudaGetLastError();
+    sort_bytes = size_t(1) << 20;
+  }
+  sort_bytes = std::max(sort_bytes, size_t(1) << 16);
+  char* sort_tmp = ws.take<char>(sort_bytes);
   qhap_status st;
   if (workspace_protocol(ws, workspace, ws_bytes, &st)) return st;
   QHAP_TRY(require_device());
@@ -126,35 +185,34 @@ extern "C" qhap_status qhap_component_split(const qhap_csr* graph, int32_t min_s
     if (!changed) break;
     QHAP_REQUIRE(round < 63, "connected components did not converge");
   }
-  // host: group the vertices by label (= smallest vertex of the component), ascending label, ascending vertex
-  std::vector<int32_t> lab(n), size(n, 0), hperm, hinv(n, -1);
-  QHAP_CUDA_TRY(cudaMemcpyAsync(lab.data(), parent, sizeof(int32_t) * size_t(n), cudaMemcpyDeviceToHost, stream));
+  // group the vertices by label (= smallest vertex of the component): ascending label, ascending vertex inside a component
+  QHAP_CUDA_TRY(cudaMemsetAsync(size, 0, sizeof(int32_t) * (size_t(n) + 1), stream));
+  cc_size_kernel<<<vb, 256, 0, stream>>>(n, parent, size);
+  QHAP_LAUNCH_CHECK();
+  cc_keep_kernel<<<vb, 256, 0, stream>>>(n, min_size, parent, size, cnt, cidx);
+  QHAP_LAUNCH_CHECK();
+  QHAP_TRY(exclusive_scan_i32(cnt, cnt, n, totals, reinterpret_cast<int32_t*>(totals + 3), stream, scan_scratch));       // start[r]; total = kept vertices
+  QHAP_TRY(exclusive_scan_i32(cidx, cidx, n, totals + 1, reinterpret_cast<int32_t*>(totals + 3), stream, scan_scratch));  // number[r]; total = kept components
+  cc_key_kernel<<<vb, 256, 0, stream>>>(n, min_size, parent, size, cnt, cidx, key, val, inst_dev);
+  QHAP_LAUNCH_CHECK();
+  {
+    size_t bytes = sort_bytes;
+    QHAP_CUDA_TRY(cub::DeviceRadixSort::SortPairs(sort_tmp, bytes, key, key2, val, val2, n, 0, 32, stream));   // stable: vertices stay ascending
+    count_launches(3);
+  }
+  cc_perm_kernel<<<vb, 256, 0, stream>>>(n, cnt + n, val2, perm, inv);
+  QHAP_LAUNCH_CHECK();
+  int64_t counts[2] = {0, 0};
+  QHAP_CUDA_TRY(cudaMemcpyAsync(counts, totals, sizeof(counts), cudaMemcpyDeviceToHost, stream));
   QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
-  for (int32_t v = 0; v < n; ++v) size[lab[v]]++;
-  std::vector<int32_t> start(n, -1);
-  int32_t m = 0, nc = 0;
-  for (int32_t r = 0; r < n; ++r) {                      // roots in ascending order
-    if (lab[r] != r || size[r] < min_size) continue;
-    start[r] = m;
-    inst_ptr[nc++] = m;
-    m += size[r];
-  }
-  inst_ptr[nc] = m;
+  const int32_t m = int32_t(counts[0]), nc = int32_t(counts[1]);
+  QHAP_CUDA_TRY(cudaMemcpyAsync(inst_ptr, inst_dev, sizeof(int32_t) * (size_t(nc) + 1), cudaMemcpyDeviceToHost, stream));
   *n_comp = nc;
-  hperm.assign(size_t(m), 0);
-  std::vector<int32_t> fill(start);
-  for (int32_t v = 0; v < n; ++v) {                       // ascending vertex order inside a component
-    const int32_t r = lab[v];
-    if (start[r] < 0) continue;
-    hperm[fill[r]] = v;
-    hinv[v] = fill[r]++;
-  }
   out->n = m;
-  if (m > 0) QHAP_CUDA_TRY(cudaMemcpyAsync(perm, hperm.data(), sizeof(int32_t) * size_t(m), cudaMemcpyHostToDevice, stream));
-  QHAP_CUDA_TRY(cudaMemcpyAsync(inv, hinv.data(), sizeof(int32_t) * size_t(n), cudaMemcpyHostToDevice, stream));
   if (m == 0) {
     QHAP_CUDA_TRY(cudaMemsetAsync(out->row_ptr, 0, sizeof(int32_t), stream));
     QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
+    inst_ptr[0] = 0;
     return QHAP_OK;
   }
   cc_degree_kernel<<<int(ceil_div(m, 256)), 256, 0, stream>>>(m, perm, graph->row_ptr, out->row_ptr);
@@ -166,7 +224,7 @@ extern "C" qhap_status qhap_component_split(const qhap_csr* graph, int32_t min_s
   QHAP_LAUNCH_CHECK();
   int64_t total = 0;
   QHAP_CUDA_TRY(cudaMemcpyAsync(&total, totals, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
-  QHAP_CUDA_TRY(cudaStreamSynchronize(stream));          // also keeps hperm / hinv alive until the copies are done
+  QHAP_CUDA_TRY(cudaStreamSynchronize(stream));          // nnz and inst_ptr are on the host now
   out->nnz = total;
   return QHAP_OK;
 }

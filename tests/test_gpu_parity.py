@@ -721,6 +721,11 @@ def test_tensor_core_paths_hold_1e3_for_50_free_running_steps(B, oracle, torch_m
                                case=f"50 free steps {name} R {R} path {path} {tag}", **kw)
         print(f"{name} path {path} {tag}: {fmt_traj(o)}")
         assert o["first_exceed"] is None
+    # for the record (not asserted): round 1's arithmetic -- one accumulator for all product terms, fp32 x
+    o = compare_trajectory(B, oracle, torch_mod, g, w, 1, fr.n_frag, R, p["T"], p["seed"], steps=50, path=1, dense_J=J, tile_skip=1,
+                           strict=False, max_tainted=R, case=f"(record only) {name} R {R} path 1 one accumulator, fp32 x", dense_bn=64,
+                           state16=2, split_acc=2)
+    print(f"{name} one accumulator (round-1 arithmetic): {fmt_traj(o)}")
     # one call, 50 steps (fused where the tile count allows: cfg1-scaled at R = 256 has 26 tiles on 13 CTAs)
     Rf = 256 if name != "cfg0" else R
     x0, y0 = synth.bsb_init_state(p["seed"], fr.n_frag, Rf)

@@ -131,7 +131,9 @@ typedef struct {
                           /*    second TMEM tile and the epilogue adds the two (the tensor cores' fp32 accumulation truncates at */
                           /*    every MMA; kept apart, the small terms no longer truncate the large sum: measured 2-8x smaller   */
                           /*    trajectory drift); 2 = one accumulator.  Changes result bits (documented in DESIGN.md 4.4)       */
-  int32_t reserved[8];    /* must be 0                                                                                      */
+  int32_t y_ring;         /* state16: how y reaches the epilogue: automatic / 1 = per-warp TMA ring in shared memory, 2 = plain       */
+                          /*    coalesced loads one work item ahead (frees the ring's 32 KB for a fourth operand stage). Same bits     */
+  int32_t reserved[7];    /* must be 0                                                                                      */
 } qhap_bsb_tuning;
 
 /* bSB parameters (PAPER.md:L265 gives the outline; constants from BASELINE.json; readings R10a-f):

@@ -93,6 +93,9 @@ struct DenseArgs {
   // their truncation is 2^-11 smaller; the epilogue adds the two.  Halves the MMAs that truncate at full magnitude.
   // Needs BN <= 128 (two accumulator stages x 2 x 128 columns = the 512 TMEM columns).
   int32_t sacc;
+  // state16: y of the next work item comes by plain coalesced loads into registers instead of the per-warp TMA ring (frees
+  // the ring's 32 KB for a fourth operand stage; every thread re-reads only y values it wrote itself one step earlier)
+  int32_t yldg;
 };
 
 // c2 = fp32(dt (a0 - a_k)), a_k = a0 k / (T - 1): the same individually rounded fp64 operations as the host loop
@@ -722,10 +725,19 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         __syncwarp();
       };
       Pos p0 = first_pos(), p1 = p0, p2 = p0;
+      float yc[kChunk], ynx[kChunk];             // yldg: y of the current / the next item
+      auto ldg_y = [&](const Pos& p, float (&dst)[kChunk]) {
+        const int r = p.tm * kBM + ec.lane_r, i0 = p.tn * a.BN + p.ch * kChunk;
+        uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
+        const bool r_ok = r < a.R;
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) dst[j] = (r_ok && i0 + j < a.n) ? a.y[off] : 0.f;
+      };
+      const bool yldg = X16 && a.yldg;
       if (p0.vt < vt_end) {
-        issue(p0, 0);
+        if (yldg) ldg_y(p0, yc); else issue(p0, 0);
         advance(p1);
-        if (p1.vt < vt_end) issue(p1, 1);
+        if (p1.vt < vt_end && !yldg) issue(p1, 1);
         p2 = p1;
         if (p1.vt < vt_end) advance(p2);
       }
@@ -736,13 +748,19 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p0.ch * kChunk), v);
         uint32_t v2[kChunk];
         if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p0.ch * kChunk), v2);
-        ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
         float xv[kChunk], yv[kChunk];
+        if (yldg) {
+          if (p1.vt < vt_end) ldg_y(p1, ynx);    // in flight while this item is updated
+#pragma unroll
+          for (int j = 0; j < kChunk; ++j) yv[j] = yc[j];
+        } else {
+          ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
+        }
         const uint32_t src = ring_w + uint32_t(slot) * kSlotBytes + uint32_t(lane) * 4u;
 #pragma unroll
         for (int j = 0; j < kChunk; ++j) {
           if constexpr (X16) {
-            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + uint32_t(j) * 128u));
+            if (!yldg) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + uint32_t(j) * 128u));
           } else {
             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(xv[j]) : "r"(src + uint32_t(j) * 128u));
             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
@@ -774,7 +792,12 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         // reads have completed.  (Requested right after the ld.shared instructions were issued, the TMA write could land
         // before the last of them had read the slot: observed as rows 5..7 of a work item carrying the next item's y.)
         __syncwarp();
-        if (p1.vt < vt_end && p2.vt < vt_end) issue(p2, slot);
+        if (yldg) {
+#pragma unroll
+          for (int j = 0; j < kChunk; ++j) yc[j] = ynx[j];
+        } else if (p1.vt < vt_end && p2.vt < vt_end) {
+          issue(p2, slot);
+        }
         if (p1.vt != p0.vt) tile_done();
         p0 = p1; p1 = p2;
         if (p2.vt < vt_end) advance(p2);
@@ -1116,7 +1139,7 @@ qhap_status launch_step(int grid, cudaStream_t stream, const CUtensorMap& tj, co
 // single staging buffer is used whenever that buys another stage (fp32-x kernels; cfg1/cfg2: 2 -> 3 stages).  state16 always
 // has two buffers (tile t + 1's own pair is loaded while tile t is updated) and a ring of half the size.
 void choose_staging(DenseArgs& a, int stage_bytes, const qhap_bsb_tuning& t) {
-  const int ring_bytes = a.x16 ? kRingBytes16 : (a.ring ? kRingBytes : 0);
+  const int ring_bytes = a.x16 ? (a.yldg ? 0 : kRingBytes16) : (a.ring ? kRingBytes : 0);
   auto stages = [&](int bufs) {
     return std::min(kMaxStages, (kSmemBudget - (a.stage_out ? bufs * 2 * kStageX : 0) - ring_bytes) / stage_bytes);
   };
@@ -1130,8 +1153,9 @@ void choose_staging(DenseArgs& a, int stage_bytes, const qhap_bsb_tuning& t) {
 // The arrays that are re-used (x in fp32 and the four fp16 copies: 12 B per (spin, replica); state16: the copies only, 8 B)
 // get the evict_last priority and y evict_first when they fit the L2 with room for the y stream and the J tiles.
 void set_l2_policies(DenseArgs& a, const qhap_bsb_tuning& t) {
-  const double keep_bytes = (a.x16 ? 8.0 : 12.0) * double(a.n) * double(a.R);
-  const bool keep = t.l2_hints == 0 ? keep_bytes <= 104e6 : t.l2_hints == 1;
+  // state16: the copies stay in the L2 without help and the hints cost 1-9 % (cfg1 24.2 against 24.8, cfg2 28.0 against 30.7 us
+  // per step), so automatic = off there
+  const bool keep = t.l2_hints == 0 ? (!a.x16 && 12.0 * double(a.n) * double(a.R) <= 104e6) : t.l2_hints == 1;
   // q/16 of the keep set's lines are evict_last, the rest evict_first (createpolicy.fractional.L2::evict_last.L2::evict_first
   // with fraction q/16 encodes as (0x150 | (q - 1)) << 52; q = 16 is kEvictLast for every line)
   const int q = (t.l2_keep_16ths >= 1 && t.l2_keep_16ths <= 16) ? t.l2_keep_16ths : 16;
@@ -1341,6 +1365,9 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.stage_out = (BN == kBK) ? 1 : 0;
   a.dsb = p.force_mode == 1 ? 1 : 0;
   a.x16 = x16_ok(a, y, false, p, t) ? 1 : 0;
+  // y by plain loads where the ring's 32 KB buy an operand stage that matters: many k-blocks per tile (mean degree >= 70:
+  // cfg2 33.6 -> 28.0 us per step; cfg1, degree 59: 24.2 -> 24.6, so it keeps the ring)
+  a.yldg = (a.x16 && (t.y_ring == 2 || (t.y_ring == 0 && g.nnz >= 70 * int64_t(n)))) ? 1 : 0;
   a.ring = (a.x16 || ring_ok(BN, R, x, y)) ? 1 : 0;
   a.sacc = (t.split_acc != 2 && BN <= 128 && !a.dsb) ? 1 : 0;
   choose_staging(a, BN * kBK * 2 + 2 * kStageX, t);
@@ -1546,6 +1573,9 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.stage_out = 1;
   a.dsb = p.force_mode == 1 ? 1 : 0;
   a.x16 = x16_ok(a, y, has_rem, p, t) ? 1 : 0;
+  // y by plain loads where the ring's 32 KB buy an operand stage that matters: two J terms (48 KB stages: 2 -> 3, cfg3
+  // 221 -> 217.5 us per step) or many k-blocks per tile (mean degree >= 70)
+  a.yldg = (a.x16 && (t.y_ring == 2 || (t.y_ring == 0 && (two_terms || g.nnz >= 70 * int64_t(n))))) ? 1 : 0;
   a.ring = (a.x16 || ring_ok(kBK, R, x, y)) ? 1 : 0;
   a.j_terms = two_terms ? 2 : 1;
   a.sacc = (t.split_acc != 2 && !a.dsb) ? 1 : 0;

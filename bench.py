@@ -59,6 +59,8 @@ def parse_args():
                          "replicas are split into contiguous slices (SURVEY 8(e)); config 3 always shards its blocks (strong)")
     ap.add_argument("--linkage-tenths", type=int, default=0,
                     help="SNP configs: linkage depth k/10 of the graph build (0 = the config's own, 3; 10 = the paper's exhaustive setting, PAPER.md:L114)")
+    ap.add_argument("--porec-edges", type=int, default=0,
+                    help="read configs: add Pore-C multi-contact fragments until this many long-range SNP pairs exist (non-banded read graph, SURVEY 8(f) f3)")
     ap.add_argument("--refine-iters", type=int, default=0,
                     help="SNP configs with one instance (config 4): also time qhap_snp_refine (Eq. 15-17) with at most this many solves")
     return ap.parse_args()
@@ -176,7 +178,7 @@ def run_reference(args):
     from oracle import oracle as O
     O.build()
     cores = O.hardware_threads()
-    fr, p = synth.make_config(args.config)
+    fr, p = synth.make_config(args.config, porec_edges=args.porec_edges)
     per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
     times, samples = [], []
     for it in range(args.warmup + args.steps):
@@ -211,7 +213,7 @@ def run_ours(args):
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    fr, p = synth.make_config(args.config)
+    fr, p = synth.make_config(args.config, porec_edges=args.porec_edges)
     snp = p["graph"] == "snp"
     mode = B.QHAP_WEIGHT_FX if snp else B.QHAP_WEIGHT_D_MINUS_C     # BASELINE.json: "discordant minus concordant"
     T = p["T"]
@@ -258,7 +260,9 @@ def run_ours(args):
             hap = B.qhap_phase_readout_snps(frags.h1, spins) if (win is None or world == 1) else spins
             state["g"] = g
             return cut, hap
-        g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype)
+        # the edge capacity of the previous pass is the hint for this one (one build call instead of count -> allocate -> fill)
+        g, J = B.qhap_build_read_graph(frags, weight_mode=mode, dense_dtype=dense_dtype, capacity_hint=state.get("nnz_hint", 0))
+        state["nnz_hint"] = g.nnz + 1024
         res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, seed=seed, replica_begin=r_begin, weight_mode=mode, path=path, dense_J=J, tile_skip=tile_skip,
                                step_launch=args.step_launch, cut_per_replica=False, workspace=state.get("ws"))
         state["ws"] = res["workspace"]

@@ -159,7 +159,7 @@ typedef struct {
                         /*  4 tcgen05 step on a block-compressed J built from the CSR (64 x 64 tiles; entries */
                         /*    of sparsely filled tiles -- long-range edges -- go through a remainder CSR      */
                         /*    gather; batches allowed; the plan SYNCHRONISES the stream once or a few times); */
-                        /*  0 auto: 3 if it fits, else 1 if dense_J is given, else 4 (2 below 1024 vertices)   */
+                        /*  0 auto: 3 if it fits, else 1 if dense_J is given, else 4 (2 below 1024 or above 2^20 vertices) */
   int32_t tile_skip;    /* path 1: 1 = visit only the 64-column blocks of J that hold a non-zero (bit-identical) */
   int32_t init_state;   /* 1: x, y <- seeded U(-0.1,0.1) counter hash (R11) before the first step */
   int32_t finalize;     /* 1: after the steps compute cut per replica, best replica, best spins           */

@@ -199,9 +199,37 @@ def _two_phase(fn_name, call, alloc):
 
 
 def qhap_build_read_graph(frags: Frags, weight_mode: int = QHAP_WEIGHT_D, dense_dtype: int = QHAP_DENSE_NONE,
-                          dense_ld: Optional[int] = None):
-    """(1) read-graph build -> (Csr with d, c; dense J tensor or None).  PAPER.md:L235-L246."""
+                          dense_ld: Optional[int] = None, capacity_hint: int = 0):
+    """(1) read-graph build -> (Csr with d, c; dense J tensor or None).  PAPER.md:L235-L246.
+    capacity_hint > 0 (e.g. the nnz of a previous region of the same kind): the edge arrays are allocated up front with that
+    capacity and ONE call counts, scans and fills (qhap.h capacity protocol); if the hint is too small the call reports the
+    required nnz and the normal count -> allocate -> fill sequence runs."""
     dev = _dev()
+    if capacity_hint > 0:
+        g = Csr(frags.n_frag, 0, torch.empty(frags.n_frag + 1, dtype=torch.int32, device=dev))
+        g.col, g.d, g.c = (torch.empty(capacity_hint, dtype=torch.int32, device=dev) for _ in range(3))
+        if dense_dtype != QHAP_DENSE_NONE and dense_ld is None:
+            dense_ld = (frags.n_frag + 127) // 128 * 128
+        J = None
+        if dense_dtype != QHAP_DENSE_NONE:
+            J = torch.empty((dense_ld, dense_ld), dtype=torch.float16 if dense_dtype == QHAP_DENSE_FP16 else torch.bfloat16, device=dev)
+        fs, cs = frags.c_struct(), g.c_struct(capacity=capacity_hint)
+
+        def once(ws, ws_bytes):
+            return _lib.qhap_build_read_graph(C.byref(fs), C.c_int32(weight_mode), C.byref(cs), _ptr(J), C.c_int32(dense_ld or 0),
+                                              C.c_int32(dense_dtype), ws, ws_bytes, _stream())
+        nb = C.c_size_t(0)
+        _check(once(None, C.byref(nb)), "qhap_build_read_graph (size query)")
+        ws = _workspace(nb.value)
+        nb = C.c_size_t(ws.numel())
+        st = once(_ptr(ws), C.byref(nb))
+        if st == QHAP_OK:
+            g.nnz = int(cs.nnz)
+            g.col, g.d, g.c = g.col[:g.nnz], g.d[:g.nnz], g.c[:g.nnz]
+            return g, J
+        if st != QHAP_ERR_WORKSPACE:
+            _check(st, "qhap_build_read_graph")
+        # hint too small: fall through to the two-phase protocol
     g = Csr(frags.n_frag, 0, torch.empty(frags.n_frag + 1, dtype=torch.int32, device=dev))
     fs = frags.c_struct()
     state = {"cs": g.c_struct(), "J": None}

@@ -87,7 +87,7 @@ extern "C" qhap_status qhap_bsb_solve(const qhap_csr* graph, int32_t n_inst, con
   const int32_t res_rc = (path == 0 || path == 3) ? resident_plan(graph->n, graph->nnz, p->replicas) : 0;
   // auto: small problems -> shared-memory resident; a dense J was built -> tcgen05 over it; otherwise the tcgen05 step on the
   // block-compressed J (hybrid with a remainder CSR for non-banded graphs), except for tiny graphs where the CSR step is as good
-  if (path == 0) path = res_rc > 0 ? 3 : ((dense_J && n_inst == 1) ? 1 : (graph->n >= 1024 ? 4 : 2));
+  if (path == 0) path = res_rc > 0 ? 3 : ((dense_J && n_inst == 1) ? 1 : ((graph->n >= 1024 && graph->n <= (1 << 20)) ? 4 : 2));   // path 4's tile-occupancy table is (n / 64)^2 ints
   QHAP_REQUIRE(path >= 1 && path <= 4, "path must be 0, 1, 2, 3 or 4");
   QHAP_REQUIRE(path != 3 || res_rc > 0, "resident path: problem too large for shared memory (needs n R <= 65536)");
   if (path == 1) {

@@ -247,8 +247,12 @@ def merge_fragments(a: Fragments, b: Fragments) -> Fragments:
                    np.concatenate([a.frag_hap, b.frag_hap]), a.snp_pos, meta)
 
 
-def make_config(cfg: int, scale: float = 1.0, seed: int | None = None) -> tuple[Fragments, dict]:
-    """Fragments + solver parameters of BASELINE.json config ``cfg`` (optionally shrunk by ``scale``)."""
+def make_config(cfg: int, scale: float = 1.0, seed: int | None = None, porec_edges: int = 0) -> tuple[Fragments, dict]:
+    """Fragments + solver parameters of BASELINE.json config ``cfg`` (optionally shrunk by ``scale``).
+
+    ``porec_edges`` > 0 on a read-based config adds Pore-C multi-contact fragments (contact distances 10 kb .. L) until that
+    many long-range SNP pairs exist: the reads of such a region no longer form a banded read graph (SURVEY.md
+    8(f) f3)."""
     p = dict(CONFIGS[cfg])
     seed = _seed_for(cfg) if seed is None else seed
     if scale != 1.0:
@@ -264,6 +268,11 @@ def make_config(cfg: int, scale: float = 1.0, seed: int | None = None) -> tuple[
         pc = make_porec_fragments(seed=seed + 7919, base=fr, L=p["L"], flip=p["flip"], qual=p["qual"],
                                   target_edges=p["porec_edges"])
         fr = merge_fragments(fr, pc)
+    if porec_edges > 0 and cfg != 4:
+        pc = make_porec_fragments(seed=seed + 7919, base=fr, L=p["L"], flip=p["flip"], qual=p["qual"],
+                                  target_edges=int(porec_edges), batch=256, d_min=1e4, d_max=float(p["L"]))
+        fr = merge_fragments(fr, pc)
+        p["name"] += f"+porec{int(porec_edges)}"
     p["dt"], p["a0"], p["seed"] = BSB_DT, BSB_A0, seed
     return fr, p
 

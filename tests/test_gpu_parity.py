@@ -1234,3 +1234,48 @@ def test_bsb_constants_every_path(B, oracle, torch_mod, dt, a0, c0, begin):
                          x=xg, y=yg, dense_J=J if path == 1 else None, tile_skip=1, finalize=False)
         dx = np.abs(xg.cpu().numpy() - xo).max(); dy = np.abs(yg.cpu().numpy() - yo).max()
         assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (path, dx, dy)
+
+
+# ------------------------------- (f3) at FULL size: cfg1's reads + Pore-C fragments, a read graph that is no longer banded
+def test_cfg1_with_porec_fragments_full_size(B, oracle, torch_mod):
+    """cfg1's 8,000 HiFi-like reads plus 768 Pore-C multi-contact fragments (they enter the read graph
+    unweighted): about 99k of the 654k entries lie more than 256 reads away from the diagonal and a 64-row tile lists ~40
+    k-blocks instead of ~5.  Graph and dense J bit-exact; the dense tile_skip step (lists from the actual occupancy) and the
+    hybrid block path (tiles + remainder CSR) over the first 10 steps on sampled replicas; cuts exact; best cut and switch
+    error against an oracle solve of the SAME 64 seeded replicas for all T steps."""
+    fr, p = synth.make_config(1, porec_edges=20000)
+    n, R, T = fr.n_frag, p["R"], p["T"]
+    og = oracle.read_graph(fr)
+    rows = np.repeat(np.arange(og["n"]), np.diff(og["row_ptr"]))
+    assert (np.abs(og["col"] - rows) > 256).sum() > 50_000
+    dfr = B.upload_frags(fr)
+    g, J = B.qhap_build_read_graph(dfr, weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    assert_csr_equal(g.to_host(), og, ("d", "c"))
+    w = oracle.read_weights(og, 1)
+    jval = (-w).astype(np.float32)
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    sample = np.array([0, 127, 128, 600, 1023])
+    xo, yo, _ = oracle.bsb_run(og["row_ptr"], og["col"], jval, np.ascontiguousarray(x0[:, sample], np.float64),
+                               np.ascontiguousarray(y0[:, sample], np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+    for path in (1, 4):
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=1, path=path,
+                               dense_J=J if path == 1 else None, tile_skip=1, finalize=False)
+        dx = np.abs(res["x"].cpu().numpy()[:, sample] - xo).max(); dy = np.abs(res["y"].cpu().numpy()[:, sample] - yo).max()
+        print(f"cfg1 + Pore-C full size, path {path}: 10 steps, 5 sampled replicas: max|dx| {dx:.2e} max|dy| {dy:.2e}")
+        assert dx <= TRAJ_TOL and dy <= TRAJ_TOL, (path, dx, dy)
+    R_sub = 64
+    ores = oracle.solve(og["row_ptr"], og["col"], w, jval, x0[:, :R_sub].copy(), y0[:, :R_sub].copy(), steps_total=T,
+                        n_threads=oracle.hardware_threads())
+    ose, _ = ser_reads(oracle, fr, ores["best_spins"])
+    for path in (1, 4):
+        res = B.qhap_bsb_solve(g, replicas=R_sub, steps_total=T, seed=p["seed"], weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1)
+        spins = res["best_spins"].cpu().numpy()
+        gcut = int(res["best_cut"].cpu()[0])
+        ccut, _ = oracle.cut_eval(og["row_ptr"], og["col"], w, spins)
+        assert ccut[0] == gcut
+        gse, _ = ser_reads(oracle, fr, spins)
+        print(f"cfg1 + Pore-C full size, path {path}: gpu best cut {gcut} oracle {ores['best_cut']} ({R_sub} matched replicas x {T} steps); SE gpu {gse:.5f} oracle {ose:.5f}")
+        _record(dict(case=f"cfg1 + Pore-C full size quality path {path}", gpu_best_cut=gcut, oracle_best_cut=int(ores["best_cut"]), replicas=R_sub,
+                     steps=int(T), se_gpu=gse, se_oracle=ose))
+        assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (path, gcut, ores["best_cut"])
+        assert gse <= ose + 0.001

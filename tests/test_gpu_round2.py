@@ -210,3 +210,20 @@ def test_eval_every_trace(B, oracle, path):
     for j in range(3):
         ob = int(ores["trace"][j].max())
         assert int(res["trace_best_cut"][j, 0].cpu()) >= ob - 0.005 * abs(ob) - 1
+
+
+def test_read_graph_single_call_with_capacity_hint(B, oracle):
+    """qhap.h capacity protocol: with edge arrays of sufficient capacity ONE call counts, scans and fills; a hint that is too
+    small falls back to count -> allocate -> fill.  Same graph and dense J, bit for bit."""
+    import torch
+    fr, _ = synth.make_config(1, scale=0.1)
+    dfr = B.upload_frags(fr)
+    exp = oracle.read_graph(fr)
+    ref, Jref = B.qhap_build_read_graph(dfr, weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    for hint in (exp["nnz"] + 1000, exp["nnz"], 17):
+        g, J = B.qhap_build_read_graph(dfr, weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16, capacity_hint=hint)
+        h = g.to_host()
+        assert h["nnz"] == exp["nnz"]
+        for k in ("row_ptr", "col", "d", "c"):
+            assert np.array_equal(h[k], exp[k]), (hint, k)
+        assert torch.equal(J, Jref)

@@ -1279,3 +1279,39 @@ def test_cfg1_with_porec_fragments_full_size(B, oracle, torch_mod):
                      steps=int(T), se_gpu=gse, se_oracle=ose))
         assert gcut >= ores["best_cut"] - 0.005 * abs(ores["best_cut"]), (path, gcut, ores["best_cut"])
         assert gse <= ose + 0.001
+
+
+# ----------------------------------- cfg3 at the paper's exhaustive linkage depth 10/10, FULL size
+def test_cfg3_depth10_full_size(B, oracle, torch_mod):
+    """cfg3's 250k reads at linkage depth 10/10 -- the setting of all of the paper's results (L114; SURVEY 8(d) asks for it as
+    a second row): 15.9 M directed entries, 76 neighbours per SNP.  SNP graph and 47-block split bit-exact; the block path
+    over the first 10 steps on sampled replicas of the first and the last block; per-block cuts of a short solve exact."""
+    fr, p = synth.make_config(3)
+    dfr = B.upload_frags(fr)
+    og = oracle.snp_graph(fr, 10, 0.1)
+    assert og["nnz"] > 15_000_000
+    g = B.qhap_build_snp_graph(dfr, 10, 0.1)
+    assert_csr_equal(g.to_host(), og, ("w_fx", "w"))
+    win = synth.block_windows(fr.n_snp, p["block"], p["stride"])
+    obs = oracle.block_split(og, win)
+    bs = B.qhap_block_split(g, win)
+    assert_csr_equal(bs.to_host(), obs, ("w_fx", "w"))
+    n, R, T = obs["n"], p["R"], p["T"]
+    x0, y0 = synth.bsb_init_state(p["seed"], n, R)
+    sample = np.array([0, 100, R - 1])
+    res = B.qhap_bsb_solve(bs, replicas=R, steps_total=T, steps_run=10, seed=p["seed"], weight_mode=2, path=4, finalize=False)
+    xg = res["x"].cpu().numpy()
+    res = B.qhap_bsb_solve(bs, replicas=R, steps_total=T, step_begin=10, steps_run=190, weight_mode=2, path=4, x=res["x"], y=res["y"])
+    spins = res["best_spins"].cpu().numpy()
+    for b in (0, len(win) - 1):
+        lo, hi = int(obs["inst_ptr"][b]), int(obs["inst_ptr"][b + 1])
+        rp = (obs["row_ptr"][lo:hi + 1] - obs["row_ptr"][lo]).astype(np.int32)
+        sl = slice(int(obs["row_ptr"][lo]), int(obs["row_ptr"][hi]))
+        cl = (obs["col"][sl] - lo).astype(np.int32)
+        xo, yo, _ = oracle.bsb_run(rp, cl, (-obs["w"][sl]).astype(np.float32), np.ascontiguousarray(x0[lo:hi][:, sample], np.float64),
+                                   np.ascontiguousarray(y0[lo:hi][:, sample], np.float64), steps_total=T, step_begin=0, steps_run=10, n_threads=8)
+        dx = np.abs(xg[lo:hi][:, sample] - xo).max()
+        print(f"cfg3 depth 10/10 full size, block {b}: 10 steps, 3 sampled replicas: max|dx| {dx:.2e}")
+        assert dx <= TRAJ_TOL
+        ccut, _ = oracle.cut_eval(rp, cl, obs["w_fx"][sl], spins[lo:hi])
+        assert ccut[0] == int(res["best_cut"].cpu()[b])

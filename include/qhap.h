@@ -19,7 +19,7 @@
  *    one count back).  qhap_bsb_solve on paths 1-3, qhap_cut_eval, the readouts, qhap_block_stitch, qhap_gauge_transform,
  *    qhap_flip_count_update, qhap_refine_readout and qhap_component_merge are asynchronous: results are valid after the
  *    caller synchronises.
- *  - no global state, no hidden RNG, no CPU fallback: without an sm_100 device every call returns QHAP_ERR_CUDA.
+ *  - no global state (one exception: the static scratch array of qhap_cut_eval_static, documented there), no hidden RNG, no CPU fallback: without an sm_100 device every call returns QHAP_ERR_CUDA.
  *  - qhap_last_error() returns a thread-local text for the last non-OK status.
  */
 #ifndef QHAP_H_
@@ -188,6 +188,19 @@ QHAP_API qhap_status qhap_bsb_solve(const qhap_csr *graph, int32_t n_inst, const
  * in the graph's integer units (counts, or 2^-32 fixed point).  spins: [n][R] int8 (+1/-1).  energy may be NULL. */
 QHAP_API qhap_status qhap_cut_eval(const qhap_csr *graph, int32_t weight_mode, const int8_t *spins, int32_t replicas,
                           int64_t *cut, int64_t *energy, void *workspace, size_t *ws_bytes, void *stream);
+
+/* (5') qhap_cut_eval WITHOUT a workspace, for callers that cannot allocate device memory (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc).  Same arguments, same results bit for bit, asynchronous on `stream`.
+ * The scratch (512 bytes + one bit per (spin, replica), rows padded to 32 replicas) lives in a static device array of
+ * QHAP_CUT_STATIC_BYTES inside the library: every GPU that loads the library holds that much until the process exits.
+ * Limit: 512 + 4 n ceil(replicas / 32) <= QHAP_CUT_STATIC_BYTES (e.g. 8,000 spins x 4,096 replicas), else
+ * QHAP_ERR_WORKSPACE with a message naming both sizes and nothing is launched.  The call allocates and frees nothing.
+ * All calls on a device SHARE the array: calls that overlap on the GPU (different streams, no ordering between them) race;
+ * calls ordered on one stream, or by events, are safe.  The array keeps the last call's contents; every call clears or
+ * overwrites what it reads. */
+#define QHAP_CUT_STATIC_BYTES (4u << 20)
+QHAP_API qhap_status qhap_cut_eval_static(const qhap_csr *graph, int32_t weight_mode, const int8_t *spins, int32_t replicas,
+                                 int64_t *cut, int64_t *energy, void *stream);
 
 /* (6) Phase readout.  Read-based vote, PAPER.md:L271-L281 [Eq. 7-8]: v_j = sum_i s_i M_ij;
  * hap1[j] = H1 allele if v_j > 0, the other allele if v_j < 0, -1 (unphased) if v_j == 0.

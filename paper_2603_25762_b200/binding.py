@@ -23,7 +23,7 @@ QHAP_OK, QHAP_ERR_INVALID_ARG, QHAP_ERR_RANGE, QHAP_ERR_WORKSPACE, QHAP_ERR_CUDA
 QHAP_WEIGHT_D, QHAP_WEIGHT_D_MINUS_C, QHAP_WEIGHT_FX = 0, 1, 2
 QHAP_DENSE_NONE, QHAP_DENSE_FP16, QHAP_DENSE_BF16 = 0, 1, 2
 
-EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_build_snp_graph_fill", "qhap_bsb_solve", "qhap_cut_eval",
+EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_build_snp_graph_fill", "qhap_bsb_solve", "qhap_cut_eval", "qhap_cut_eval_static",
            "qhap_phase_readout_reads", "qhap_phase_readout_snps", "qhap_block_split", "qhap_block_stitch",
            "qhap_gauge_transform", "qhap_flip_count_update", "qhap_refine_readout", "qhap_snp_refine",
            "qhap_component_split", "qhap_component_merge",
@@ -67,7 +67,7 @@ def _tuning(kw: dict):
     return t
 
 
-for _name in EXPORTS[:15]:
+for _name in EXPORTS[:-3]:           # every entry point but the last three returns a qhap_status
     getattr(_lib, _name).restype = C.c_int
 _lib.qhap_last_error.restype = C.c_char_p
 _lib.qhap_version.restype = C.c_char_p
@@ -399,6 +399,30 @@ def qhap_cut_eval(graph: Csr, weight_mode: int, spins: torch.Tensor, want_energy
     ws = _workspace(ws_bytes.value)
     ws_bytes = C.c_size_t(ws.numel())
     _check(call(_ptr(ws), C.byref(ws_bytes)), "qhap_cut_eval")
+    return cut, energy
+
+
+QHAP_CUT_STATIC_BYTES = 4 << 20
+
+
+def qhap_cut_eval_static(graph: Csr, weight_mode: int, spins: torch.Tensor, cut: Optional[torch.Tensor] = None,
+                         energy: Optional[torch.Tensor] = None, want_energy: bool = True):
+    """(5') qhap_cut_eval without a workspace: the scratch is a static device array inside the library
+    (QHAP_CUT_STATIC_BYTES; larger problems are rejected).  `cut` / `energy` may be passed in (int64 [R], device), in which
+    case this call allocates nothing at all.  Calls that overlap on the GPU share the scratch and race."""
+    dev = _dev()
+    if spins.dim() == 1:
+        spins = spins[:, None].contiguous()
+    n, R = spins.shape
+    assert n == graph.n and spins.dtype == torch.int8
+    if cut is None:
+        cut = torch.empty(R, dtype=torch.int64, device=dev)
+    if energy is None and want_energy:
+        energy = torch.empty(R, dtype=torch.int64, device=dev)
+    assert cut.dtype == torch.int64 and cut.numel() == R and (energy is None or (energy.dtype == torch.int64 and energy.numel() == R))
+    gs = graph.c_struct()
+    _check(_lib.qhap_cut_eval_static(C.byref(gs), C.c_int32(weight_mode), _ptr(spins), C.c_int32(R), _ptr(cut), _ptr(energy), _stream()),
+           "qhap_cut_eval_static")
     return cut, energy
 
 

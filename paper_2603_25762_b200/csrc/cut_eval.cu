@@ -6,6 +6,8 @@
 // a chunk of 32*VEC replicas, keeps VEC int64 partial cuts per lane in registers and flushes them with one atomicAdd per
 // (lane, slot) when its tile (or the instance) ends.  Per edge a warp reads 4-16 bytes of packed signs instead of the
 // neighbour's 128-512 bytes of fp32 x.
+#include <atomic>
+
 #include "kernels.cuh"
 
 namespace qhap {
@@ -287,3 +289,65 @@ qhap_status gather_best_spins(int32_t n, int32_t R, const float* x, int32_t n_in
 }
 
 }  // namespace qhap
+
+// ------------------------------------------------------------------ qhap_cut_eval_static: the cut evaluation with NO workspace
+// For callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the scratch of the
+// cut evaluation -- W_tot and the packed sign bits -- lives in a file-scope device array of QHAP_CUT_STATIC_BYTES.  Every GPU
+// that loads the library holds the array until the process exits.  In host code the array's NAME is a host-side stand-in, not
+// a device address: the address comes from cudaGetSymbolAddress, once per device, with that device current.
+// All calls on a device share the array: calls that overlap on the GPU (different streams) race.  It keeps the last call's
+// contents; W_tot is cleared by launch_cut and every packed word a call reads is written by its own pack_signs_kernel.
+namespace qhap {
+namespace {
+static __device__ __align__(256) unsigned char g_cut_static_scratch[QHAP_CUT_STATIC_BYTES];
+
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t kStaticBitsOffset = 512;                 // [0, 8): W_tot; [256, 264): instance pointer (unused: one instance)
+std::atomic<unsigned char*> g_cut_static_ptr[kStaticMaxDevices];
+
+qhap_status cut_static_scratch(unsigned char** out) {
+  int dev = -1;
+  QHAP_CUDA_TRY(cudaGetDevice(&dev));
+  QHAP_REQUIRE(dev >= 0 && dev < kStaticMaxDevices, "qhap_cut_eval_static: device ordinal %d not supported (max %d)", dev, kStaticMaxDevices - 1);
+  unsigned char* p = g_cut_static_ptr[dev].load(std::memory_order_acquire);
+  if (p == nullptr) {                                     // racing first calls resolve the same address twice: harmless
+    void* sym = nullptr;
+    QHAP_CUDA_TRY(cudaGetSymbolAddress(&sym, g_cut_static_scratch));
+    QHAP_REQUIRE(sym != nullptr, "qhap_cut_eval_static: cudaGetSymbolAddress returned NULL");
+    p = static_cast<unsigned char*>(sym);
+    g_cut_static_ptr[dev].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return QHAP_OK;
+}
+}  // namespace
+}  // namespace qhap
+
+extern "C" qhap_status qhap_cut_eval_static(const qhap_csr* graph, int32_t weight_mode, const int8_t* spins, int32_t replicas,
+                                            int64_t* cut, int64_t* energy, void* stream_v) {
+  using namespace qhap;
+  QHAP_REQUIRE(graph, "graph must not be NULL");
+  QHAP_REQUIRE(graph->n >= 0 && graph->nnz >= 0 && replicas >= 1, "bad sizes");
+  QHAP_REQUIRE(weight_mode >= 0 && weight_mode <= 2, "bad weight_mode");
+  const size_t need = kStaticBitsOffset + sizeof(uint32_t) * cut_bits_words(graph->n, replicas);
+  if (need > size_t(QHAP_CUT_STATIC_BYTES)) {
+    set_error("qhap_cut_eval_static: n = %d spins x %d replicas need %zu bytes of scratch, the static array holds %zu "
+              "(QHAP_CUT_STATIC_BYTES); use qhap_cut_eval with a caller workspace", graph->n, replicas, need, size_t(QHAP_CUT_STATIC_BYTES));
+    return QHAP_ERR_WORKSPACE;
+  }
+  QHAP_TRY(require_device());
+  QHAP_REQUIRE(spins && cut, "spins and cut must not be NULL");
+  QHAP_REQUIRE(graph->n == 0 || (graph->row_ptr && (graph->nnz == 0 || graph->col)), "graph arrays must not be NULL");
+  if (weight_mode == QHAP_WEIGHT_FX) QHAP_REQUIRE(graph->nnz == 0 || graph->w_fx, "w_fx required for weight_mode 2");
+  else QHAP_REQUIRE(graph->nnz == 0 || (graph->d && (weight_mode == 0 || graph->c)), "d (and c) required for weight_mode 0/1");
+  unsigned char* base = nullptr;
+  QHAP_TRY(cut_static_scratch(&base));
+  int64_t* wtot = reinterpret_cast<int64_t*>(base);
+  const int32_t* inst_ptr = reinterpret_cast<const int32_t*>(base + 256);
+  uint32_t* bits = reinterpret_cast<uint32_t*>(base + kStaticBitsOffset);
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+  const CsrView g = view_of(*graph);
+  QHAP_TRY(launch_cut<int8_t>(g, weight_mode, spins, replicas, 1, inst_ptr, cut, wtot, bits, stream));
+  QHAP_TRY(cut_finalize(1, replicas, cut, wtot, energy, nullptr, nullptr, stream));
+  return QHAP_OK;
+}

@@ -15,6 +15,8 @@ namespace qhap {
 namespace {
 
 constexpr int kRowsPerWarp = 8;   // a CTA of 8 warps owns 64 consecutive rows and one chunk of replicas
+constexpr int kBitplaneMinR = 256; // above this many replicas the integer weight modes use the bit-plane kernel (below, its
+                                   // 32-replica lanes are mostly empty and the per-replica kernel is cheaper)
 
 // Packed signs: one bit per (spin, replica), word w of row a holds replicas 32 w .. 32 w + 31, bit set = spin -1.
 // The accumulation kernel reads these words (R / 8 bytes per row) instead of gathering the neighbour's fp32 x row
@@ -173,6 +175,163 @@ __global__ void __launch_bounds__(256) cut_accumulate_kernel(int32_t n, const in
   }
 }
 
+// ------------------------------------------------------------------------------------ bit-plane accumulation
+// Integer weight modes (read graphs), one instance, many replicas.  Lanes run across the packed WORDS (lane = 32 replicas), an
+// edge costs one XOR per lane, and the per-replica sums are kept BIT-SLICED: plane p of an accumulator is a word whose bit k
+// is bit p of replica k's sum.  Adding the warp-uniform magnitude |w| to the replicas selected by diff = bits[a] ^ bits[b] is
+// a ripple-carry adder of bitwise instructions -- about 2 LOP3 per plane for 32 replicas at once, instead of ~6 instructions
+// per replica.  Two levels:
+//   level 1: two unsigned accumulators of kP1 planes (edges with w > 0 / w < 0; unsigned, so that carries die out a plane or
+//            two above the weight's top bit and the adder stops there), flushed every kL1Edges edges (16 (2^15 - 1) < 2^19);
+//   level 2: one signed two's-complement accumulator of 32 planes (+= level-1 positive, -= level-1 negative), flushed at the
+//            end of the warp's rows or after kItemEdges edges (|sum| < 2^15 2^15).
+// A level-2 flush transposes the planes through shared memory, rebuilds one int32 per replica and adds it to cut[] with one
+// coalesced 64-bit atomic per 32 replicas.  Weights with |w| >= 2^15 (not expected from read depths) take a per-replica atomic
+// path.  All integer: any order of the additions gives the same bits as the oracle's sum.
+constexpr int kP1 = 19, kL1Edges = 16, kItemEdges = 1 << 15;
+constexpr int kBpWarps = 4;       // warps per CTA, each with its own items and its own 4 KB transposition tile
+
+// acc += mag (warp-uniform, < 2^15) on the replicas whose bit is set in diff
+__device__ __forceinline__ void bp_add(uint32_t (&acc)[kP1], uint32_t mag, uint32_t diff) {
+  uint32_t carry = 0;
+#pragma unroll
+  for (int q = 0; q < (kP1 + 3) / 4; ++q) {
+    const uint32_t rest = mag >> (4 * q);           // weight bits at and above this group of four planes
+    if (rest == 0) {
+      if (!__any_sync(0xffffffffu, carry != 0)) return;
+#pragma unroll
+      for (int p = 4 * q; p < 4 * q + 4 && p < kP1; ++p) {
+        const uint32_t t = acc[p];
+        acc[p] = t ^ carry;
+        carry &= t;
+      }
+    } else {
+#pragma unroll
+      for (int p = 4 * q; p < 4 * q + 4 && p < kP1; ++p) {
+        const uint32_t add = ((mag >> p) & 1u) ? diff : 0u;
+        const uint32_t t = acc[p];
+        acc[p] = t ^ add ^ carry;
+        carry = (t & add) | (t & carry) | (add & carry);
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(32 * kBpWarps) cut_bitplane_kernel(int32_t n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
+                                                                    const int32_t* __restrict__ d, const int32_t* __restrict__ c, int mode,
+                                                                    const uint32_t* __restrict__ bits, int32_t R, int32_t rows_per_item,
+                                                                    unsigned long long* __restrict__ cut, unsigned long long* __restrict__ wtot) {
+  __shared__ uint32_t s_t[kBpWarps][32][33];
+  const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
+  const int32_t W = (R + 31) >> 5;
+  const int chunks = (W + 31) >> 5;
+  const int64_t n_items = int64_t((n + rows_per_item - 1) / rows_per_item) * chunks;
+  uint32_t (*tile)[33] = s_t[wic];
+  for (int64_t item = int64_t(blockIdx.x) * kBpWarps + wic; item < n_items; item += int64_t(gridDim.x) * kBpWarps) {
+    const int chunk = int(item % chunks);
+    const int32_t a0 = int32_t(item / chunks) * rows_per_item, a1 = min(n, a0 + rows_per_item);
+    const int32_t wj = chunk * 32 + lane;
+    const bool active = wj < W;
+    uint32_t l1p[kP1], l1n[kP1], l2[32];
+#pragma unroll
+    for (int p = 0; p < kP1; ++p) { l1p[p] = 0; l1n[p] = 0; }
+#pragma unroll
+    for (int p = 0; p < 32; ++p) l2[p] = 0;
+    int n1 = 0, n2 = 0;
+    int64_t wsum = 0;
+    auto flush1 = [&]() {                       // l2 += l1p (zero-extended); l2 -= l1n; both cleared
+      uint32_t carry = 0, borrow = 0;
+#pragma unroll
+      for (int p = 0; p < 32; ++p) {
+        const uint32_t add = p < kP1 ? l1p[p] : 0u, sub = p < kP1 ? l1n[p] : 0u;
+        uint32_t t = l2[p];
+        const uint32_t s1 = t ^ add ^ carry;
+        carry = (t & add) | (t & carry) | (add & carry);
+        t = s1;
+        l2[p] = t ^ sub ^ borrow;
+        borrow = (~t & sub) | (~t & borrow) | (sub & borrow);
+      }
+#pragma unroll
+      for (int p = 0; p < kP1; ++p) { l1p[p] = 0; l1n[p] = 0; }
+      n2 += n1;
+      n1 = 0;
+    };
+    auto flush2 = [&]() {
+      if (n1) flush1();
+#pragma unroll
+      for (int p = 0; p < 32; ++p) tile[p][lane] = l2[p];
+      __syncwarp();
+      const int words = min(32, W - chunk * 32);
+      for (int j = 0; j < words; ++j) {         // word j of the chunk: lane k rebuilds replica 32 (32 chunk + j) + k
+        uint32_t v = 0;
+#pragma unroll
+        for (int p = 0; p < 32; ++p) v = __funnelshift_r(v, tile[p][j] >> lane, 1);
+        const int32_t r = (chunk * 32 + j) * 32 + lane;
+        if (r < R && v != 0) atomicAdd(&cut[r], (unsigned long long)(long long)(int32_t)v);
+      }
+      __syncwarp();
+#pragma unroll
+      for (int p = 0; p < 32; ++p) l2[p] = 0;
+      n2 = 0;
+    };
+    for (int32_t a = a0; a < a1; ++a) {
+      const int32_t e0 = row_ptr[a], e1 = row_ptr[a + 1];
+      const uint32_t sa = active ? __ldg(bits + size_t(a) * W + wj) : 0u;
+      for (int32_t eb = e0; eb < e1; eb += 32) {
+        const int32_t e = eb + lane;
+        int32_t my_col = -1, my_w = 0;
+        if (e < e1) {
+          my_col = col[e];
+          if (my_col > a) {                      // each undirected edge once
+            const int64_t w = edge_weight(mode, d, c, nullptr, e);
+            if (chunk == 0) wsum += w;
+            const bool big = w >= (1 << 15) || w <= -(1 << 15);
+            my_w = big ? 0 : int32_t(w);
+            if (big) {                           // per-replica path, this lane walks the words of the chunk itself
+              for (int j = 0; j < min(32, W - chunk * 32); ++j) {
+                const int32_t wq = chunk * 32 + j;
+                uint32_t df = __ldg(bits + size_t(a) * W + wq) ^ __ldg(bits + size_t(my_col) * W + wq);
+                while (df) {
+                  const int k = __ffs(df) - 1;
+                  df &= df - 1;
+                  if (wq * 32 + k < R) atomicAdd(&cut[wq * 32 + k], (unsigned long long)w);
+                }
+              }
+            }
+          }
+        }
+        uint32_t m = __ballot_sync(0xffffffffu, my_w != 0);
+        // the neighbour's word of the NEXT listed edge is requested before the current one is added.  Every lane takes part
+        // in every shuffle (the inactive ones too): the shuffles stay outside the `active` branches.
+        uint32_t nxt = 0;
+        int jn = m ? __ffs(m) - 1 : 0;
+        const int32_t b0 = __shfl_sync(0xffffffffu, my_col, jn);
+        if (m && active) nxt = __ldg(bits + size_t(b0) * W + wj);
+        while (m) {
+          const int j = jn;
+          const uint32_t sb = nxt;
+          m &= m - 1;
+          jn = m ? __ffs(m) - 1 : 0;
+          const int32_t bn = __shfl_sync(0xffffffffu, my_col, jn);
+          if (m && active) nxt = __ldg(bits + size_t(bn) * W + wj);
+          const int32_t w = __shfl_sync(0xffffffffu, my_w, j);
+          const uint32_t diff = active ? (sa ^ sb) : 0u;
+          if (w > 0) bp_add(l1p, uint32_t(w), diff); else bp_add(l1n, uint32_t(-w), diff);
+          if (++n1 == kL1Edges) {
+            flush1();
+            if (n2 >= kItemEdges) flush2();
+          }
+        }
+      }
+    }
+    flush2();
+    if (chunk == 0) {
+      const int64_t t = warp_sum(wsum);
+      if (lane == 0 && t != 0) atomicAdd(&wtot[0], (unsigned long long)t);
+    }
+  }
+}
+
 // One CTA per instance: energy = W_tot - 2 cut, best replica = lowest index with maximal cut.
 __global__ void __launch_bounds__(256) cut_finalize_kernel(int32_t R, const long long* __restrict__ cut,
                                                            const long long* __restrict__ wtot,
@@ -237,12 +396,21 @@ qhap_status launch_cut(const CsrView& g, int mode, const SrcT* src, int32_t R, i
   const int64_t items = int64_t(g.n) * ((R + 31) / 32);
   pack_signs_kernel<SrcT><<<int(std::min<int64_t>(ceil_div(items, 8), int64_t(sm_count()) * 16)), 256, 0, stream>>>(g.n, R, src, bits);
   QHAP_LAUNCH_CHECK();
+  auto* cu = reinterpret_cast<unsigned long long*>(cut);
+  auto* wt = reinterpret_cast<unsigned long long*>(wtot);
+  if (mode != QHAP_WEIGHT_FX && n_inst == 1 && R > kBitplaneMinR) {
+    // rows per warp item: enough items for ~16 warps per SM, at least 2 and at most 16 rows (a level-2 flush per item)
+    const int64_t chunks_w = ceil_div(ceil_div(R, 32), 32);
+    const int32_t rows = int32_t(std::min<int64_t>(16, std::max<int64_t>(2, int64_t(g.n) * chunks_w / (int64_t(sm_count()) * 16))));
+    const int64_t items = ceil_div(g.n, rows) * chunks_w;
+    cut_bitplane_kernel<<<int(ceil_div(items, kBpWarps)), 32 * kBpWarps, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, mode, bits, R, rows, cu, wt);
+    QHAP_LAUNCH_CHECK();
+    return QHAP_OK;
+  }
   const bool vec4 = R % 4 == 0;
   const int chunks = vec4 ? (R + 127) / 128 : (R + 31) / 32;
   const int64_t work = ceil_div(g.n, 8 * kRowsPerWarp) * chunks;
   const int blocks = int(std::max<int64_t>(1, std::min<int64_t>(work, int64_t(sm_count()) * 8)));
-  auto* cu = reinterpret_cast<unsigned long long*>(cut);
-  auto* wt = reinterpret_cast<unsigned long long*>(wtot);
   const PackedBits* pb = reinterpret_cast<const PackedBits*>(bits);
   if (vec4)
     cut_accumulate_kernel<PackedBits, 4><<<blocks, 256, 0, stream>>>(g.n, g.row_ptr, g.col, g.d, g.c, g.w_fx, mode, pb, R,

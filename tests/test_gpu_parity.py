@@ -223,7 +223,7 @@ def test_block_split_and_stitch_bit_exact(B, oracle, torch_mod):
 
 
 # ------------------------------------------------------------------------------------------ (5) cut / energy
-@pytest.mark.parametrize("R", [1, 5, 64, 200])
+@pytest.mark.parametrize("R", [1, 5, 64, 200, 300, 1024, 1100])       # above 256 replicas: the bit-plane kernel (integer modes)
 def test_cut_eval_bit_exact(B, oracle, torch_mod, R):
     fr, _ = synth.make_config(0)
     rg = oracle.read_graph(fr)
@@ -236,6 +236,33 @@ def test_cut_eval_bit_exact(B, oracle, torch_mod, R):
             ecut, een = oracle.cut_eval(g["row_ptr"], g["col"], w, s)
             cut, en = B.qhap_cut_eval(dg, mode, torch_mod.from_numpy(s).cuda())
             assert np.array_equal(cut.cpu().numpy(), ecut) and np.array_equal(en.cpu().numpy(), een)
+
+
+@pytest.mark.parametrize("R", [40, 700])
+def test_cut_eval_large_and_mixed_weights(B, oracle, torch_mod, R):
+    """Integer weights of both signs and of every size, |w| >= 2^15 included (the bit-plane kernel's per-replica path), on a
+    random graph with rows of 0 .. 150 entries (several 32-entry batches, level-1 flushes inside a row): cuts and energies exact."""
+    rng = np.random.default_rng(R)
+    n = 257
+    dense = np.triu(rng.random((n, n)) < 0.2, 1)
+    dense[5, :] = False; dense[:, 5] = False                       # an isolated vertex
+    dense[7, 8:160] = True                                         # a long row
+    iu = np.argwhere(dense)
+    wu = rng.integers(-60, 61, len(iu)).astype(np.int64)
+    bigs = rng.random(len(iu)) < 0.02
+    wu[bigs] = rng.integers(-(1 << 20), 1 << 20, int(bigs.sum()))
+    wu[:4] = [32767, -32767, 32768, -32768]
+    rows = np.concatenate([iu[:, 0], iu[:, 1]]); cols = np.concatenate([iu[:, 1], iu[:, 0]]); w2 = np.concatenate([wu, wu])
+    order = np.lexsort((cols, rows))
+    rows, cols, w2 = rows[order], cols[order], w2[order]
+    row_ptr = np.zeros(n + 1, np.int32); np.add.at(row_ptr, rows + 1, 1); row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    dpos = np.where(w2 > 0, w2, 0).astype(np.int32); cneg = np.where(w2 < 0, -w2, 0).astype(np.int32)
+    g = B.Csr(n, len(w2), torch_mod.from_numpy(row_ptr).cuda(), torch_mod.from_numpy(cols.astype(np.int32)).cuda(),
+              torch_mod.from_numpy(dpos).cuda(), torch_mod.from_numpy(cneg).cuda())
+    s = synth.random_spins(3, n, R)
+    ecut, een = oracle.cut_eval(row_ptr, cols.astype(np.int32), w2, s)
+    cut, en = B.qhap_cut_eval(g, 1, torch_mod.from_numpy(s).cuda())                      # w = D - C
+    assert np.array_equal(cut.cpu().numpy(), ecut) and np.array_equal(en.cpu().numpy(), een)
 
 
 def test_cut_eval_empty_graph(B, torch_mod):

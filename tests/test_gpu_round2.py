@@ -227,3 +227,57 @@ def test_read_graph_single_call_with_capacity_hint(B, oracle):
         for k in ("row_ptr", "col", "d", "c"):
             assert np.array_equal(h[k], exp[k]), (hint, k)
         assert torch.equal(J, Jref)
+
+
+# ---------------------------------------------------------- block path with exactly as many tiles as the tile arrays hold
+@pytest.mark.parametrize("extra_tile", [0, 1])
+def test_block_path_at_exact_tile_capacity(B, oracle, guarded, extra_tile):
+    """The block path's tile arrays hold 16 nnz / 4096 + ceil(n / 64) + 1 tiles of 64 x 64.  A graph whose non-empty tiles number
+    EXACTLY that capacity (extra_tile = 0) keeps every tile; one tile more (extra_tile = 1) no longer fits, the threshold rises
+    and every entry goes to the remainder CSR.  Both run inside a guarded workspace of exactly the queried size and follow the
+    fp64 oracle over 10 steps; cuts of the final signs are exact."""
+    import torch
+    T_rows, n = 6, 6 * 64
+    edges = []
+
+    def inside(tr, tc, k):                       # k edges from tile row tr into tile column tc (distinct rows and columns)
+        for i in range(k):
+            a, b = tr * 64 + 3 + 5 * i, tc * 64 + 40 + 4 * i
+            edges.append((min(a, b), max(a, b)))
+    for t in range(4):
+        inside(t, t, 3)                          # four diagonal tiles
+    inside(4, 5, 3)                              # tiles (4, 5) and (5, 4)
+    inside(4, 4, 2)                              # seventh tile
+    if extra_tile:
+        inside(5, 5, 2)                          # eighth tile: one more than the capacity
+    edges = sorted(set(edges))
+    rng = np.random.default_rng(5)
+    wd = rng.integers(1, 9, len(edges)); wc = rng.integers(0, 5, len(edges))
+    rows = np.array([e[0] for e in edges] + [e[1] for e in edges]); cols = np.array([e[1] for e in edges] + [e[0] for e in edges])
+    d2 = np.concatenate([wd, wd]).astype(np.int32); c2 = np.concatenate([wc, wc]).astype(np.int32)
+    order = np.lexsort((cols, rows))
+    rows, cols, d2, c2 = rows[order], cols[order].astype(np.int32), d2[order], c2[order]
+    row_ptr = np.zeros(n + 1, np.int64); np.add.at(row_ptr, rows + 1, 1); row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    nnz = len(cols)
+    tiles = {(int(a) // 64, int(b) // 64) for a, b in zip(rows, cols)}
+    n_tiles = len(tiles) + sum(1 for t in range(T_rows) if not any(tt[0] == t for tt in tiles))      # + a forced tile per empty tile row
+    cap = 16 * nnz // 4096 + T_rows + 1
+    assert n_tiles == cap + extra_tile, (n_tiles, cap)
+    g = B.Csr(n, nnz, torch.from_numpy(row_ptr).cuda(), torch.from_numpy(cols).cuda(), torch.from_numpy(d2).cuda(), torch.from_numpy(c2).cuda())
+    w = (d2 - c2).astype(np.int64)
+    R, T = 64, 200
+    x0, y0 = synth.bsb_init_state(9, n, R)
+    outs = {}
+    for path in (4, 2):
+        xg, yg = torch.from_numpy(x0.copy()).cuda(), torch.from_numpy(y0.copy()).cuda()
+        res = B.qhap_bsb_solve(g, replicas=R, steps_total=T, steps_run=10, weight_mode=1, path=path, x=xg, y=yg)
+        outs[path] = (xg.cpu().numpy(), yg.cpu().numpy(), res)
+    xo, yo = x0.astype(np.float64), y0.astype(np.float64)
+    oracle.bsb_run(row_ptr, cols, (-w).astype(np.float32), xo, yo, steps_total=T, step_begin=0, steps_run=10, n_threads=4)
+    for path in (4, 2):
+        dx = np.abs(outs[path][0] - xo).max(); dy = np.abs(outs[path][1] - yo).max()
+        assert dx <= 1e-3 and dy <= 1e-3, (path, extra_tile, dx, dy)
+        res = outs[path][2]
+        ccut, _ = oracle.cut_eval(row_ptr, cols, w, res["best_spins"].cpu().numpy())
+        assert int(ccut[0]) == int(res["best_cut"].cpu()[0])
+    assert guarded() >= 2

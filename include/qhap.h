@@ -133,7 +133,10 @@ typedef struct {
                           /*    trajectory drift); 2 = one accumulator.  Changes result bits (documented in DESIGN.md 4.4)       */
   int32_t y_ring;         /* state16: how y reaches the epilogue: automatic / 1 = per-warp TMA ring in shared memory, 2 = plain       */
                           /*    coalesced loads one work item ahead (frees the ring's 32 KB for a fourth operand stage). Same bits     */
-  int32_t reserved[7];    /* must be 0                                                                                      */
+  int32_t pair_tiles;     /* state16 on the dense tile_skip path: automatic / 1 = two neighbouring 64-spin boxes of a replica tile */
+                          /*    share one N = 128 accumulator where that does not unbalance the CTAs (each staged x k-block feeds  */
+                          /*    128 output spins; y by plain loads unless y_ring = 1), 2 = every box on its own.  Same bits          */
+  int32_t reserved[6];    /* must be 0                                                                                      */
 } qhap_bsb_tuning;
 
 /* bSB parameters (PAPER.md:L265 gives the outline; constants from BASELINE.json; readings R10a-f):

@@ -43,7 +43,7 @@ class _Csr(C.Structure):
 
 class _BsbTuning(C.Structure):
     _fields_ = [("dense_bn", C.c_int32), ("step_launch", C.c_int32), ("l2_hints", C.c_int32), ("dense_stg_bufs", C.c_int32),
-                ("dense_epi_sync", C.c_int32), ("l2_keep_16ths", C.c_int32), ("state16", C.c_int32), ("split_acc", C.c_int32), ("y_ring", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("dense_epi_sync", C.c_int32), ("l2_keep_16ths", C.c_int32), ("state16", C.c_int32), ("split_acc", C.c_int32), ("y_ring", C.c_int32), ("pair_tiles", C.c_int32), ("reserved", C.c_int32 * 6)]
 
 
 class _BsbParams(C.Structure):
@@ -54,7 +54,7 @@ class _BsbParams(C.Structure):
                 ("trace_cut", C.c_void_p), ("trace_best_cut", C.c_void_p), ("tuning", C.POINTER(_BsbTuning))]
 
 
-TUNING_KEYS = ("dense_bn", "step_launch", "l2_hints", "dense_stg_bufs", "dense_epi_sync", "l2_keep_16ths", "state16", "split_acc", "y_ring")
+TUNING_KEYS = ("dense_bn", "step_launch", "l2_hints", "dense_stg_bufs", "dense_epi_sync", "l2_keep_16ths", "state16", "split_acc", "y_ring", "pair_tiles")
 
 
 def _tuning(kw: dict):

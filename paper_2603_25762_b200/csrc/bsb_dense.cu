@@ -96,7 +96,17 @@ struct DenseArgs {
   // state16: y of the next work item comes by plain coalesced loads into registers instead of the per-warp TMA ring (frees
   // the ring's 32 KB for a fourth operand stage; every thread re-reads only y values it wrote itself one step earlier)
   int32_t yldg;
+  // Paired tiles (state16, tile_skip lists, dense J): the unit of CTA work is a SLOT = one 64-spin box, or a PAIR of boxes
+  // (2q, 2q + 1) of the same replica tile that share one N = 128 accumulator: every staged x k-block then feeds 128 output
+  // spins instead of 64 (the operand feed -- bytes in flight per SM against the L2 latency -- is what bounds the 64-wide
+  // step).  Slots of a step: first the pairs (q-major, replica tile fastest), then the remaining boxes as singles; the state
+  // side (staging buffers, TMA stores, done[]) stays per box.  pair_lines = pairs per replica tile (0: every slot is a box).
+  int32_t pair_lines, n_slots;
+  const int32_t* pk_cnt;      // [pair_lines] union of the two boxes' k-block lists
+  const int32_t* pk_idx;      // [pair_lines][n_kblocks]
 };
+
+struct Slot { int tn0, tm, width, q; };
 
 // c2 = fp32(dt (a0 - a_k)), a_k = a0 k / (T - 1): the same individually rounded fp64 operations as the host loop
 __device__ __forceinline__ float ramp_c2(const DenseArgs& a, int s) {
@@ -109,6 +119,24 @@ __device__ __forceinline__ float ramp_c2(const DenseArgs& a, int s) {
 __device__ __forceinline__ void tile_split(const DenseArgs& a, int tile, int& tn, int& tm) {
   tn = a.inv_tm ? int(__umulhi(uint32_t(tile), a.inv_tm)) : tile;
   tm = tile - tn * a.n_tiles_m;
+}
+
+// slot -> (first box, replica tile, width); slots [0, pair_lines n_tiles_m) are pairs, the rest single boxes
+template <bool PAIR>
+__device__ __forceinline__ Slot slot_of(const DenseArgs& a, int slot) {
+  Slot s;
+  tile_split(a, slot, s.q, s.tm);
+  if (PAIR && s.q < a.pair_lines) { s.tn0 = 2 * s.q; s.width = 2; }
+  else { s.tn0 = PAIR ? s.q + a.pair_lines : s.q; s.width = 1; }
+  return s;
+}
+// k-block list of a slot (nullptr: all k-blocks)
+template <bool PAIR>
+__device__ __forceinline__ const int32_t* slot_list(const DenseArgs& a, const Slot& sl, int& nkb) {
+  if (a.kb_cnt == nullptr) { nkb = a.n_kblocks; return nullptr; }
+  if (PAIR && sl.width == 2) { nkb = a.pk_cnt[sl.q]; return a.pk_idx + size_t(sl.q) * a.n_kblocks; }
+  nkb = a.kb_cnt[sl.tn0];
+  return a.kb_idx + size_t(sl.tn0) * a.n_kblocks;
 }
 
 // fp32 -> two fp16 terms of xs = 2^15 x (|x| <= 1 -> |xs| <= 32768, inside fp16's range): hi = rn(xs), lo = rn(xs - hi)
@@ -166,10 +194,8 @@ __device__ __forceinline__ void epi_pack(int j, float xn, uint32_t (&hp)[kChunk 
 
 // fp32 state of one work item (kChunk spins x this thread's replica) -> registers; masked entries read as 0.
 // Element offsets are 32-bit (the host checks n R < 2^32): one integer add and one wide multiply-add per address.
-__device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec, int tile, int ch, float (&xv)[kChunk],
+__device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec, int tn, int tm, int ch, float (&xv)[kChunk],
                                          float (&yv)[kChunk]) {
-  int tn, tm;
-  tile_split(a, tile, tn, tm);
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
   const bool r_ok = r < a.R;
   uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
@@ -192,11 +218,9 @@ __device__ __forceinline__ void epi_load(const DenseArgs& a, const EpiConsts& ec
 // Fused update of one work item: y' = y + dt(-(a0 - a_k) x + c0 F), x' = x + dt a0 y', inelastic wall; stores x', y'
 // (fp32, coalesced across the warp's 32 replicas) and the fp16 split of x' (16 contiguous bytes per thread and array: into the staging tiles, or directly).
 template <bool hints>
-__device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tile, int ch,
+__device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiConsts& ec, int tn, int tm, int ch,
                                                  const uint32_t (&v)[kChunk], const float (&xv)[kChunk],
                                                  const float (&yv)[kChunk], uint32_t stg) {
-  int tn, tm;
-  tile_split(a, tile, tn, tm);
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
   const bool r_ok = r < a.R;
   uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
@@ -336,7 +360,7 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
 // RING: the fp32 state arrives through the per-warp TMA ring; HINTS: L2 eviction priorities on every state access.
 // Compile-time variants keep each instantiation's hot loops small (the single run-time kernel had grown from 63 to 88 KB
 // of SASS and cost cfg3 3 %).
-template <bool RING, bool HINTS, bool X16>
+template <bool RING, bool HINTS, bool X16, bool PAIR>
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
                   const __grid_constant__ CUtensorMap tm_xh,
@@ -347,7 +371,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;       // 128B swizzle needs 1024-byte alignment
   const int kStages = a.n_stages;
   const uint32_t kTileJ = uint32_t(a.BN) * kBK * 2;                    // one J tile; a second one (J_lo) follows if j_terms == 2
-  const uint32_t kStageJ = kTileJ * uint32_t(a.j_terms), kStageBytes = kStageJ + 2 * kStageX;
+  // paired tiles: room for the J tiles of both boxes (rows 0..63 | 64..127 of one N = 128 operand)
+  const uint32_t kStageJ = kTileJ * uint32_t(a.j_terms) * (PAIR ? 2u : 1u), kStageBytes = kStageJ + 2 * kStageX;
   const uint32_t bar_base = smem_base + kSmemBudget;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
@@ -395,9 +420,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
-  const int n_tiles = a.n_tiles_m * a.n_tiles_n;
-  const int stride = a.tile_stride, vt_end = a.n_steps * a.tile_stride;   // virtual tiles: step-major, holes in [n_tiles, stride)
-  const uint32_t stage_tx = kStageJ + 2u * kStageX;
+  const int n_tiles = a.n_slots;                                          // slots of a step (boxes, or pairs of boxes)
+  const int stride = a.tile_stride, vt_end = a.n_steps * a.tile_stride;   // virtual slots: step-major, holes in [n_slots, stride)
 
   if (warp == 0) {
     // ===================================================================================== TMA producer
@@ -407,22 +431,24 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       int stage = 0;
       uint32_t phase = 0;
       for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
-        const int s = vt / stride, tile = vt - s * stride;
-        if (tile >= n_tiles) continue;
-        int tn, tm;                                                      // M fastest: neighbouring CTAs share the J tile in L2
-        tile_split(a, tile, tn, tm);
-        const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
+        const int s = vt / stride, slot = vt - s * stride;
+        if (slot >= n_tiles) continue;
+        const Slot sl = slot_of<PAIR>(a, slot);                                // replica tile fastest: neighbouring CTAs share the J tile in L2
+        const int tn = sl.tn0, tm = sl.tm;
+        int nkb;
+        const int32_t* list = slot_list<PAIR>(a, sl, nkb);
         if (s > 0) {
-          for (int j = lane; j < nkb; j += 32)                           // tile (kb, tm) has finished step s - 1
-            ptx::wait_at_least_acquire(a.done + a.kb_idx[size_t(tn) * a.n_kblocks + j] * a.n_tiles_m + tm, uint32_t(s));
+          for (int j = lane; j < nkb; j += 32)                           // box (kb, tm) has finished step s - 1
+            ptx::wait_at_least_acquire(a.done + list[j] * a.n_tiles_m + tm, uint32_t(s));
           __syncwarp();
           ptx::fence_proxy_async_global();
         }
         if (lane != 0) continue;
         const CUtensorMap* mh = (s & 1) ? &tm_oh : &tm_xh;               // odd steps of a fused launch read what even steps wrote
         const CUtensorMap* ml = (s & 1) ? &tm_ol : &tm_xl;
+        const uint32_t stage_tx = kTileJ * uint32_t(a.j_terms) * uint32_t(sl.width) + 2u * kStageX;
         for (int j = 0; j < nkb; ++j) {
-          const int kb = a.kb_cnt ? a.kb_idx[size_t(tn) * a.n_kblocks + j] : j;
+          const int kb = list ? list[j] : j;
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t sj = smem_base + stage * kStageBytes;
           ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx);
@@ -432,6 +458,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
             if (a.j_terms == 2) ptx::tma_load_2d(sj + kTileJ, &tm_jl, full_bar(stage), 0, brow);
           } else {
             ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
+            if (PAIR && sl.width == 2) ptx::tma_load_2d(sj + kTileJ, &tm_j, full_bar(stage), kb * kBK, (tn + 1) * a.BN);   // rows 64..127
           }
           if constexpr (HINTS) {
             ptx::tma_load_2d_hint(sj + kStageJ, mh, full_bar(stage), kb * kBK, tm * kBM, a.pol_keep);
@@ -446,17 +473,18 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     }
   } else if (warp == 1) {
     // ======================================================================================= MMA issuer
-    const uint32_t idesc = ptx::umma_idesc_f16_f32(kBM, uint32_t(a.BN));
+    const uint32_t idesc1 = ptx::umma_idesc_f16_f32(kBM, uint32_t(a.BN)), idesc2 = ptx::umma_idesc_f16_f32(kBM, 2u * uint32_t(a.BN));
     int stage = 0;
     uint32_t phase = 0;
     int acc = 0;
     uint32_t acc_phase = 0;
     for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
-      const int tile = vt % stride;
-      if (tile >= n_tiles) continue;
-      int tn, tm_unused;
-      tile_split(a, tile, tn, tm_unused);
-      const int nkb = a.kb_cnt ? a.kb_cnt[tn] : a.n_kblocks;
+      const int slot = vt % stride;
+      if (slot >= n_tiles) continue;
+      const Slot sl = slot_of<PAIR>(a, slot);
+      int nkb;
+      (void)slot_list<PAIR>(a, sl, nkb);
+      const uint32_t idesc = (PAIR && sl.width == 2) ? idesc2 : idesc1;
       ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1);                    // epilogue has drained this accumulator stage
       ptx::tc_fence_after();
       const uint32_t d_tmem = tmem_base + uint32_t(acc) * kMaxBN;
@@ -527,14 +555,14 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       // epilogue updates the buffer in place and the store below writes it to the other copy.  A buffer is reloaded right
       // after its store has read it.  Fused steps: the tile's own pair of step s - 1 was stored (and waited for with
       // wait_group 0) by this same thread at least stg_bufs tiles earlier -- every CTA has >= 2 tiles per step.
-      int vt_ld = blockIdx.x;
+      int vt_ld = blockIdx.x, bx_ld = 0;             // next box to load: slot vt_ld, box bx_ld of it
       uint32_t b_ld = 0;
       auto load_next = [&]() {
         while (vt_ld < vt_end) {
-          const int s = vt_ld / stride, tile = vt_ld - s * stride;
-          if (tile >= n_tiles) { vt_ld += gridDim.x; continue; }
-          int tn, tm;
-  tile_split(a, tile, tn, tm);
+          const int s = vt_ld / stride, slot = vt_ld - s * stride;
+          if (slot >= n_tiles) { vt_ld += gridDim.x; continue; }
+          const Slot sl = slot_of<PAIR>(a, slot);
+          const int tn = sl.tn0 + bx_ld, tm = sl.tm;
           const uint32_t stg = stg_base + b_ld * (2u * kStageX);
           ptx::mbar_arrive_expect_tx(stg_in(b_ld), 2u * kStageX);
           if constexpr (HINTS) {
@@ -544,7 +572,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
             ptx::tma_load_2d(stg, (s & 1) ? &tm_oh : &tm_xh, stg_in(b_ld), tn * a.BN, tm * kBM);
             ptx::tma_load_2d(stg + kStageX, (s & 1) ? &tm_ol : &tm_xl, stg_in(b_ld), tn * a.BN, tm * kBM);
           }
-          vt_ld += gridDim.x;
+          if (!PAIR || ++bx_ld == sl.width) { bx_ld = 0; vt_ld += gridDim.x; }
           if (++b_ld == a.stg_bufs) b_ld = 0;
           return;
         }
@@ -553,10 +581,11 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         for (uint32_t q = 0; q < a.stg_bufs; ++q) load_next();
       }
       for (int vt = blockIdx.x; vt < vt_end; vt += gridDim.x) {
-        const int s = vt / stride, tile = vt - s * stride;
-        if (tile >= n_tiles) continue;
-        int tn, tm;
-  tile_split(a, tile, tn, tm);
+        const int s = vt / stride, slot = vt - s * stride;
+        if (slot >= n_tiles) continue;
+        const Slot sl = slot_of<PAIR>(a, slot);
+        for (int bx = 0; bx < (PAIR ? sl.width : 1); ++bx) {
+        const int tn = sl.tn0 + bx, tm = sl.tm;
         const uint32_t stg = stg_base + b * (2u * kStageX);
         ptx::mbar_wait(stg_full(b), bpar);
         if constexpr (HINTS) {
@@ -571,10 +600,11 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         if constexpr (!X16) ptx::mbar_arrive(stg_empty(b));
         if (a.fused) {
           ptx::tma_store_wait_all();
-          ptx::signal_add_release(a.done + tile, 1u);
+          ptx::signal_add_release(a.done + (tn * a.n_tiles_m + tm), 1u);
         }
         if constexpr (X16) load_next();            // into the buffer just read (b_ld == b)
         if (++b == a.stg_bufs) { b = 0; bpar ^= 1u; }
+        }
       }
       ptx::tma_store_wait_all();                   // the bulk stores have completed before this thread exits
     }
@@ -604,24 +634,33 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     // Items are addressed by the VIRTUAL tile (step-major); the last wave of a step may have a hole for this CTA.
     // A position carries the virtual tile (ordering, end test) and the real tile next to it, so that the item loop needs
     // no division by the runtime stride.
-    struct Pos { int vt, rt, ch, tn, tm; };                // (tn, tm) of rt travel along: one tile_split per tile, not per item
+    // vt / rt: virtual and real slot; bx: box of the slot (0, or 1 in a pair); (tn, tm) of the BOX travel along
+    struct Pos { int vt, rt, ch, tn, tm, bx, width; };
     auto advance = [&](Pos& p) {
       p.ch += P;
       if (p.ch * kChunk >= a.BN || p.tn * a.BN + p.ch * kChunk >= a.n) {
+        p.ch = par;
+        if constexpr (PAIR) {
+          if (p.bx + 1 < p.width) {                         // second box of a pair: same accumulator, columns BN .. 2 BN - 1
+            ++p.bx; ++p.tn;
+            return;
+          }
+        }
         p.vt += gridDim.x; p.rt += gridDim.x;
-        if (p.rt >= n_tiles) {                              // past the step's tiles
+        if (p.rt >= n_tiles) {                              // past the step's slots
           if (p.rt < stride) { p.vt += gridDim.x; p.rt += gridDim.x; }   // hole in the last wave (stride % grid == 0)
           p.rt -= stride;                                   // first wave of the next step
         }
-        p.ch = par;
-        tile_split(a, p.rt, p.tn, p.tm);
+        const Slot sl = slot_of<PAIR>(a, p.rt);
+        p.tn = sl.tn0; p.tm = sl.tm; p.bx = 0; p.width = sl.width;
       }
     };
     auto first_pos = [&]() {
-      Pos p{int(blockIdx.x), int(blockIdx.x), par, 0, 0};
-      tile_split(a, p.rt, p.tn, p.tm);
-      return p;
+      const Slot sl = slot_of<PAIR>(a, int(blockIdx.x));
+      return Pos{int(blockIdx.x), int(blockIdx.x), par, sl.tn0, sl.tm, 0, sl.width};
     };
+    auto same_box = [](const Pos& p, const Pos& q) { return p.vt == q.vt && (!PAIR || p.bx == q.bx); };
+    auto box_of = [](const Pos& p) { return PAIR ? p.bx : 0; };
     int step_end = stride;                     // first virtual tile of step cur_s + 1
     auto set_step = [&](int vt) {              // items are visited in ascending vt
       if (a.fused && vt >= step_end) { ++cur_s; step_end += stride; ec.c2 = ramp_c2(a, cur_s) * kC2s; }
@@ -633,12 +672,14 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     // order), so every lane crosses to the async proxy in between: after every fence_every-th tile, with
     // fence_every <= (fewest tiles a CTA has per step) - 1, the fence that follows a tile's stores comes at most
     // fence_every - 1 tiles later, the request at least (tiles per step) - 1 tiles later.
-    int cur_rt = 0;                            // real tile of the item being finished (for the store above)
-    auto tile_done = [&]() {
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+    int cur_tn = 0, cur_tm = 0;                // box of the item being finished (for the store below)
+    auto tile_done = [&](bool slot_end) {      // last chunk of this warp in a box; slot_end: ... and in the slot's accumulator
+      if (slot_end) {
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      }
       if (a.stage_out && a.store_warp) {
         ptx::fence_proxy_async();
         if (RING && a.fused && ++tcount == a.fence_every) { tcount = 0; ptx::fence_proxy_async_global(); }
@@ -654,10 +695,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         ptx::named_barrier_sync(1, kEpiWarps * 32);
         if (ew == 0 && lane == 0) {
           const uint32_t stg = stg_base + stg_i * (2u * kStageX);
-          int tn, tm;
-          tile_split(a, cur_rt, tn, tm);
-          ptx::tma_store_2d(&tm_oh, stg, tn * a.BN, tm * kBM);
-          ptx::tma_store_2d(&tm_ol, stg + kStageX, tn * a.BN, tm * kBM);
+          ptx::tma_store_2d(&tm_oh, stg, cur_tn * a.BN, cur_tm * kBM);
+          ptx::tma_store_2d(&tm_ol, stg + kStageX, cur_tn * a.BN, cur_tm * kBM);
           ptx::tma_store_commit();
         }
         stg_i ^= 1u;
@@ -674,15 +713,15 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     };
     auto step = [&](Pos& p, const float (&xc)[kChunk], const float (&yc)[kChunk], float (&xn)[kChunk],
                     float (&yn)[kChunk]) -> bool {
-      if (p.ch == par) tile_begin();
+      if (p.ch == par && box_of(p) == 0) tile_begin();
       uint32_t v[kChunk];
-      ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p.ch * kChunk), v);
+      ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + box_of(p) * a.BN + p.ch * kChunk), v);
       uint32_t v2[kChunk];
-      if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p.ch * kChunk), v2);
+      if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + box_of(p) * a.BN + p.ch * kChunk), v2);
       Pos q = p;
       advance(q);
       const bool nhave = q.vt < vt_end;
-      if (nhave) epi_load(a, ec, q.rt, q.ch, xn, yn);
+      if (nhave) epi_load(a, ec, q.tn, q.tm, q.ch, xn, yn);
       ptx::tmem_ld_wait();
       if (a.sacc) {
 #pragma unroll
@@ -691,9 +730,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       const uint32_t stg = a.stage_out ? stg_base + stg_i * (2u * kStageX) : 0u;
       if (p.ch == par) staging_free();
       set_step(p.vt);
-      epi_update_store<HINTS>(a, ec, p.rt, p.ch, v, xc, yc, stg);
-      cur_rt = p.rt;
-      if (q.vt != p.vt) tile_done();
+      epi_update_store<HINTS>(a, ec, p.tn, p.tm, p.ch, v, xc, yc, stg);
+      cur_tn = p.tn; cur_tm = p.tm;
+      if (!same_box(p, q)) tile_done(q.vt != p.vt);
       p = q;
       return nhave;
     };
@@ -743,14 +782,18 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       }
       for (uint32_t k = 0; p0.vt < vt_end; ++k) {
         const int slot = int(k & 1u);
-        if (p0.ch == par) tile_begin();
+        if (p0.ch == par && box_of(p0) == 0) tile_begin();
         uint32_t v[kChunk];
-        ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + p0.ch * kChunk), v);
+        ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + box_of(p0) * a.BN + p0.ch * kChunk), v);
         uint32_t v2[kChunk];
-        if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + p0.ch * kChunk), v2);
+        if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + box_of(p0) * a.BN + p0.ch * kChunk), v2);
         float xv[kChunk], yv[kChunk];
         if (yldg) {
           if (p1.vt < vt_end) ldg_y(p1, ynx);    // in flight while this item is updated
+          if (PAIR && p2.vt < vt_end && lane < kChunk) {   // ... and the item after it on its way from DRAM to the L2
+            const int r = p2.tm * kBM + quarter * 32, i = p2.tn * a.BN + p2.ch * kChunk + lane;
+            if (r < a.R && i < a.n) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.y + size_t(i) * a.R + r));
+          }
 #pragma unroll
           for (int j = 0; j < kChunk; ++j) yv[j] = yc[j];
         } else {
@@ -785,9 +828,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           }
           if (p0.ch == par) staging_free();
           set_step(p0.vt);
-          epi_update_store<HINTS>(a, ec, p0.rt, p0.ch, v, xv, yv, stg);
+          epi_update_store<HINTS>(a, ec, p0.tn, p0.tm, p0.ch, v, xv, yv, stg);
         }
-        cur_rt = p0.rt;
+        cur_tn = p0.tn; cur_tm = p0.tm;
         // The slot is refilled only now: the update above has CONSUMED the values read from it, so those shared-memory
         // reads have completed.  (Requested right after the ld.shared instructions were issued, the TMA write could land
         // before the last of them had read the slot: observed as rows 5..7 of a work item carrying the next item's y.)
@@ -798,7 +841,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         } else if (p1.vt < vt_end && p2.vt < vt_end) {
           issue(p2, slot);
         }
-        if (p1.vt != p0.vt) tile_done();
+        if (!same_box(p0, p1)) tile_done(p1.vt != p0.vt);
         p0 = p1; p1 = p2;
         if (p2.vt < vt_end) advance(p2);
       }
@@ -807,7 +850,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     Pos p = first_pos();
     if (p.vt < vt_end) {
       float xa[kChunk], ya[kChunk], xb[kChunk], yb[kChunk];
-      epi_load(a, ec, p.rt, p.ch, xa, ya);
+      epi_load(a, ec, p.tn, p.tm, p.ch, xa, ya);
       while (true) {
         if (!step(p, xa, ya, xb, yb)) break;
         if (!step(p, xb, yb, xa, ya)) break;
@@ -901,6 +944,28 @@ __global__ void __launch_bounds__(32) kb_list_kernel(int32_t n_kblocks, int32_t 
     // lists symmetric (fused steps: "tn lists kb <=> kb lists tn") and is ordered against itself by the owning CTA
     if (cnt == 0) { out[0] = min(n_kblocks - 1, int32_t((int64_t(tn) * BN) / kBK)); cnt = 1; }
     kb_cnt[tn] = cnt;
+  }
+}
+
+// Paired tiles: ascending union of the k-block flags of boxes 2q and 2q + 1 (one CTA per pair; never empty: an empty union
+// lists the left box's own k-block, like kb_list_kernel).
+__global__ void __launch_bounds__(32) pair_list_kernel(int32_t n_kblocks, const int32_t* __restrict__ flag, int32_t* __restrict__ pk_cnt,
+                                                       int32_t* __restrict__ pk_idx) {
+  const int q = blockIdx.x, lane = threadIdx.x;
+  const int32_t* f0 = flag + size_t(2 * q) * n_kblocks;
+  const int32_t* f1 = f0 + n_kblocks;
+  int32_t* out = pk_idx + size_t(q) * n_kblocks;
+  int32_t cnt = 0;
+  for (int32_t base = 0; base < n_kblocks; base += 32) {
+    const int32_t kb = base + lane;
+    const bool on = kb < n_kblocks && (f0[kb] | f1[kb]) != 0;
+    const uint32_t m = __ballot_sync(0xffffffffu, on);
+    if (on) out[cnt + __popc(m & ((1u << lane) - 1u))] = kb;
+    cnt += __popc(m);
+  }
+  if (lane == 0) {
+    if (cnt == 0) { out[0] = min(n_kblocks - 1, 2 * q); cnt = 1; }
+    pk_cnt[q] = cnt;
   }
 }
 
@@ -1100,9 +1165,10 @@ typedef void (*StepKernel)(const CUtensorMap, const CUtensorMap, const CUtensorM
                            const CUtensorMap, const CUtensorMap, const CUtensorMap, const DenseArgs);
 StepKernel step_kernel_of(const DenseArgs& a) {
   const bool hints = a.pol_keep != ptx::kEvictNormal;
-  if (a.x16) return hints ? dense_step_kernel<true, true, true> : dense_step_kernel<true, false, true>;
-  if (a.ring) return hints ? dense_step_kernel<true, true, false> : dense_step_kernel<true, false, false>;
-  return hints ? dense_step_kernel<false, true, false> : dense_step_kernel<false, false, false>;
+  if (a.x16 && a.pair_lines) return hints ? dense_step_kernel<true, true, true, true> : dense_step_kernel<true, false, true, true>;
+  if (a.x16) return hints ? dense_step_kernel<true, true, true, false> : dense_step_kernel<true, false, true, false>;
+  if (a.ring) return hints ? dense_step_kernel<true, true, false, false> : dense_step_kernel<true, false, false, false>;
+  return hints ? dense_step_kernel<false, true, false, false> : dense_step_kernel<false, false, false, false>;
 }
 
 // One launch of the step kernel.  Per-step launches carry the programmatic-stream-serialization attribute (see the
@@ -1171,7 +1237,7 @@ void set_l2_policies(DenseArgs& a, const qhap_bsb_tuning& t) {
 // Worth it while a CTA has few tiles per step (launch gap, pipeline fill and drain per step); with ~50 tiles per CTA and
 // step (cfg3) the boundary is amortised and lock-step launches keep the L2 reuse between neighbouring CTAs.
 int fused_grid(const DenseArgs& a, const qhap_bsb_params& p, const qhap_bsb_tuning& t) {
-  const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;
+  const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;          // boxes
   if (t.step_launch != 0 || !a.stage_out || a.BN != kBK || a.kb_cnt == nullptr || p.steps_run < 2) return 0;
   int per_sm = 0, coop = 0, dev = 0;
   StepKernel kernel = step_kernel_of(a);
@@ -1191,11 +1257,11 @@ int fused_grid(const DenseArgs& a, const qhap_bsb_params& p, const qhap_bsb_tuni
 qhap_status launch_fused(int grid, cudaStream_t stream, const CUtensorMap& tj, const CUtensorMap& tjl, const CUtensorMap (&tm_h)[2],
                          const CUtensorMap (&tm_l)[2], const CUtensorMap& tsx, const CUtensorMap& tsy, DenseArgs a,
                          const qhap_bsb_params& p, uint32_t* done, int& cur) {
-  const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;
+  const int64_t n_tiles = int64_t(a.n_tiles_m) * a.n_tiles_n;          // boxes (done[] has one counter per box)
   a.fused = 1;
   a.store_warp = 1;
-  a.tile_stride = int32_t(ceil_div(n_tiles, grid) * grid);
-  a.fence_every = uint32_t(std::max<int64_t>(1, n_tiles / grid - 1));
+  a.tile_stride = int32_t(ceil_div(int64_t(a.n_slots), grid) * grid);
+  a.fence_every = uint32_t(std::max<int64_t>(1, int64_t(a.n_slots) / grid - 1));
   a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0;
   a.c3 = float(p.dt * p.a0);
   a.c2 = 0.f;
@@ -1308,6 +1374,8 @@ struct DenseWs {
   __half* xl[2];
   int32_t* kb_cnt;
   int32_t* kb_idx;
+  int32_t* pk_cnt;
+  int32_t* pk_idx;
   int32_t* flags;
   uint32_t* done;
 };
@@ -1319,9 +1387,33 @@ DenseWs carve_dense(Workspace& ws, int32_t n, int32_t R) {
   const size_t n_kb = size_t(ceil_div(n, kBK)), n_tn_max = size_t(ceil_div(n, 32));
   w.kb_cnt = ws.take<int32_t>(n_tn_max);
   w.kb_idx = ws.take<int32_t>(n_tn_max * n_kb);
+  w.pk_cnt = ws.take<int32_t>(n_kb / 2 + 1);                 // paired tiles (64-wide boxes only)
+  w.pk_idx = ws.take<int32_t>((n_kb / 2 + 1) * n_kb);
   w.flags = ws.take<int32_t>(n_tn_max * n_kb);
   w.done = ws.take<uint32_t>(n_tn_max * size_t(ceil_div(R, kBM)));   // fused steps
   return w;
+}
+
+// Paired tiles: pairs per replica tile.  Slots go to CTAs round robin (slot % grid), pairs first; the step lasts as long as
+// the most loaded CTA (in boxes), so: the largest number of pairs that does not raise that maximum above what single boxes
+// give, ceil(boxes / grid) -- or, when min_boxes > 0 (fused launches: state prefetch distance), leaves a CTA with fewer
+// than min_boxes boxes per step.
+int32_t choose_pair_lines(int32_t n_tiles_n, int32_t n_tiles_m, int grid, int min_boxes) {
+  const int64_t boxes = int64_t(n_tiles_n) * n_tiles_m;
+  const int64_t target = ceil_div(boxes, grid);
+  for (int32_t P = n_tiles_n / 2; P > 0; --P) {
+    const int64_t np = int64_t(P) * n_tiles_m, ns = int64_t(n_tiles_n - 2 * P) * n_tiles_m;
+    int64_t mx = 0, mn = INT64_MAX;
+    for (int c = 0; c < grid; ++c) {
+      const int64_t pc = np / grid + (c < np % grid ? 1 : 0);
+      const int64_t c0 = ((c - np) % grid + grid) % grid;            // first single i with (np + i) % grid == c
+      const int64_t sc = c0 < ns ? (ns - c0 + grid - 1) / grid : 0;
+      mx = std::max(mx, 2 * pc + sc);
+      mn = std::min(mn, 2 * pc + sc);
+    }
+    if (mx <= target && mn >= min_boxes) return P;
+  }
+  return 0;
 }
 
 // state16 is usable when the tile is one swizzle box wide with TMA-stored copies, the y ring's boxes are legal (row pitch a
@@ -1380,6 +1472,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.kb_idx = skip ? w.kb_idx : nullptr;
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
+  a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = w.pk_cnt; a.pk_idx = w.pk_idx;
   set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
@@ -1402,10 +1495,29 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
     QHAP_LAUNCH_CHECK();
   }
 
-  const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
-  a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
+  // Paired tiles (DenseArgs::pair_lines): state16 with two staging buffers on the tile_skip lists.  y then comes by plain
+  // loads (the ring's 32 KB go to the third 48 KB operand stage) unless the caller insists on the ring.
+  const int gf = fused_grid(a, p, t);
+  if (a.x16 && skip && BN == kBK && a.stg_bufs == 2 && t.pair_tiles != 2) {
+    const int g0 = gf ? gf : int(std::min<int64_t>(a.n_slots, sm_count()));
+    const int32_t P = choose_pair_lines(a.n_tiles_n, a.n_tiles_m, g0, gf ? 2 : 0);
+    if (P > 0) {
+      DenseArgs b = a;
+      b.pair_lines = P;
+      b.n_slots = P * a.n_tiles_m + (a.n_tiles_n - 2 * P) * a.n_tiles_m;
+      if (t.y_ring != 1) b.yldg = 1;
+      choose_staging(b, 2 * BN * kBK * 2 + 2 * kStageX, t);
+      if (b.n_stages >= 2 && b.stg_bufs == 2) {
+        a = b;
+        pair_list_kernel<<<P, 32, 0, stream>>>(n_kb, w.flags, w.pk_cnt, w.pk_idx);
+        QHAP_LAUNCH_CHECK();
+      }
+    }
+  }
+  const int grid = int(std::min<int64_t>(a.n_slots, sm_count()));
+  a.tile_stride = int32_t(ceil_div(int64_t(a.n_slots), grid) * grid);
   int cur = 0;
-  if (const int gf = fused_grid(a, p, t)) {
+  if (gf) {
     QHAP_TRY(launch_fused(gf, stream, tm_j, tm_j, tm_h, tm_l, tm_sx, tm_sy, a, p, w.done, cur));
   } else {
     for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {
@@ -1586,6 +1698,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.n_tiles_n = n_t;
   a.n_kblocks = n_t;
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
+  a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = nullptr; a.pk_idx = nullptr;
   a.c1 = c1row; a.c1_per_row = 1;
   a.x = x; a.y = y;
   set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;

@@ -667,6 +667,11 @@ def test_l2_hints_and_staging_variants_are_bit_identical(B, oracle, torch_mod, s
             f, l = run(path, y_ring=yr)
             assert np.array_equal(f[0], ref_first[0]) and np.array_equal(f[1], ref_first[1]) and np.array_equal(l[0], ref_last[0]) \
                 and np.array_equal(l[1], ref_last[1]), (path, "y_ring", yr)
+        for pt in (1, 2):                                    # paired tiles (N = 128 accumulators for two boxes) or single boxes
+            for yr in (0, 1, 2):
+                f, l = run(path, pair_tiles=pt, y_ring=yr)
+                assert np.array_equal(f[0], ref_first[0]) and np.array_equal(f[1], ref_first[1]) and np.array_equal(l[0], ref_last[0]) \
+                    and np.array_equal(l[1], ref_last[1]), (path, "pair_tiles", pt, yr)
         for q in (1, 8, 11):
             f, l = run(path, l2_hints=1, l2_keep_16ths=q)
             assert np.array_equal(f[0], ref_first[0]) and np.array_equal(l[1], ref_last[1]) and np.array_equal(l[0], ref_last[0]), (path, q)

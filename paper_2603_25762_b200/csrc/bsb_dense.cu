@@ -360,7 +360,8 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
 // RING: the fp32 state arrives through the per-warp TMA ring; HINTS: L2 eviction priorities on every state access.
 // Compile-time variants keep each instantiation's hot loops small (the single run-time kernel had grown from 63 to 88 KB
 // of SASS and cost cfg3 3 %).
-template <bool RING, bool HINTS, bool X16, bool PAIR>
+// YLDG (state16 only): y by plain loads instead of the ring.
+template <bool RING, bool HINTS, bool X16, bool PAIR, bool YLDG>
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
                   const __grid_constant__ CUtensorMap tm_xh,
@@ -636,24 +637,25 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
     // no division by the runtime stride.
     // vt / rt: virtual and real slot; bx: box of the slot (0, or 1 in a pair); (tn, tm) of the BOX travel along
     struct Pos { int vt, rt, ch, tn, tm, bx, width; };
+    auto next_box = [&](Pos& p) {                           // first item of this warp in the box after p's
+      p.ch = par;
+      if constexpr (PAIR) {
+        if (p.bx + 1 < p.width) {                           // second box of a pair: same accumulator, columns BN .. 2 BN - 1
+          ++p.bx; ++p.tn;
+          return;
+        }
+      }
+      p.vt += gridDim.x; p.rt += gridDim.x;
+      if (p.rt >= n_tiles) {                                // past the step's slots
+        if (p.rt < stride) { p.vt += gridDim.x; p.rt += gridDim.x; }   // hole in the last wave (stride % grid == 0)
+        p.rt -= stride;                                     // first wave of the next step
+      }
+      const Slot sl = slot_of<PAIR>(a, p.rt);
+      p.tn = sl.tn0; p.tm = sl.tm; p.bx = 0; p.width = sl.width;
+    };
     auto advance = [&](Pos& p) {
       p.ch += P;
-      if (p.ch * kChunk >= a.BN || p.tn * a.BN + p.ch * kChunk >= a.n) {
-        p.ch = par;
-        if constexpr (PAIR) {
-          if (p.bx + 1 < p.width) {                         // second box of a pair: same accumulator, columns BN .. 2 BN - 1
-            ++p.bx; ++p.tn;
-            return;
-          }
-        }
-        p.vt += gridDim.x; p.rt += gridDim.x;
-        if (p.rt >= n_tiles) {                              // past the step's slots
-          if (p.rt < stride) { p.vt += gridDim.x; p.rt += gridDim.x; }   // hole in the last wave (stride % grid == 0)
-          p.rt -= stride;                                   // first wave of the next step
-        }
-        const Slot sl = slot_of<PAIR>(a, p.rt);
-        p.tn = sl.tn0; p.tm = sl.tm; p.bx = 0; p.width = sl.width;
-      }
+      if (p.ch * kChunk >= a.BN || p.tn * a.BN + p.ch * kChunk >= a.n) next_box(p);
     };
     auto first_pos = [&]() {
       const Slot sl = slot_of<PAIR>(a, int(blockIdx.x));
@@ -736,7 +738,65 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       p = q;
       return nhave;
     };
-    if constexpr (RING) {
+    if constexpr (X16 && YLDG) {
+      {
+        // state16 with y by plain loads: the loop is unrolled twice over two register buffers (current / next item's y and
+        // position change roles), so that nothing is copied at the back edge; y of the NEXT box is on its way from DRAM to the
+        // L2 while this box is updated (lanes 0 .. 15 touch the 16 lines this warp will read there).
+        auto ldg_y = [&](const Pos& p, float (&dst)[kChunk]) {
+          const int r = p.tm * kBM + ec.lane_r, i0 = p.tn * a.BN + p.ch * kChunk;
+          uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
+          if (r < a.R && i0 + kChunk <= a.n) {
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) dst[j] = a.y[off];
+          } else {
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) dst[j] = (r < a.R && i0 + j < a.n) ? a.y[off] : 0.f;
+          }
+        };
+        auto item = [&](const Pos& p, const float (&yc)[kChunk], Pos& q, float (&yn)[kChunk]) -> bool {
+          const bool first = p.ch == par;                    // this warp's first item of the box
+          if (first && box_of(p) == 0) tile_begin();
+          uint32_t v[kChunk], v2[kChunk];
+          ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + box_of(p) * a.BN + p.ch * kChunk), v);
+          if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + box_of(p) * a.BN + p.ch * kChunk), v2);
+          q = p;
+          advance(q);
+          const bool nhave = q.vt < vt_end;
+          if (nhave) ldg_y(q, yn);
+          if (first) {
+            Pos nb = p;
+            next_box(nb);
+            if (nb.vt < vt_end && lane < 2 * kChunk) {
+              const int r = nb.tm * kBM + quarter * 32, i = nb.tn * a.BN + (par + (lane >> 3) * P) * kChunk + (lane & 7);
+              if (r < a.R && i < min(a.n, (nb.tn + 1) * a.BN)) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.y + size_t(i) * a.R + r));
+            }
+            ptx::mbar_wait(stg_in(stg_i), stg_par);          // the box's own (x_hi, x_lo) has arrived
+          }
+          const uint32_t stg = stg_base + stg_i * (2u * kStageX);
+          ptx::tmem_ld_wait();
+          if (a.sacc) {
+#pragma unroll
+            for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v2[j]));
+          }
+          set_step(p.vt);
+          if (a.c1_per_row) epi_update_x16<HINTS, true>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+          else epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+          if (!same_box(p, q)) tile_done(q.vt != p.vt);
+          return nhave;
+        };
+        Pos pa = first_pos(), pb = pa;
+        if (pa.vt < vt_end) {
+          float ya[kChunk], yb[kChunk];
+          ldg_y(pa, ya);
+          while (true) {
+            if (!item(pa, ya, pb, yb)) break;
+            if (!item(pb, yb, pa, ya)) break;
+          }
+        }
+      }
+    }
+    else if constexpr (RING) {
       // State through TMA: every warp owns two 2 KB slots (x and y of one work item: a box of 8 spins x 32 replicas
       // each).  The item two ahead is requested as soon as the current item's values are in registers, so the loads
       // need no registers, no address arithmetic and no LSU slots; out-of-range rows / replicas arrive as zeros.
@@ -764,19 +824,10 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         __syncwarp();
       };
       Pos p0 = first_pos(), p1 = p0, p2 = p0;
-      float yc[kChunk], ynx[kChunk];             // yldg: y of the current / the next item
-      auto ldg_y = [&](const Pos& p, float (&dst)[kChunk]) {
-        const int r = p.tm * kBM + ec.lane_r, i0 = p.tn * a.BN + p.ch * kChunk;
-        uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
-        const bool r_ok = r < a.R;
-#pragma unroll
-        for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) dst[j] = (r_ok && i0 + j < a.n) ? a.y[off] : 0.f;
-      };
-      const bool yldg = X16 && a.yldg;
       if (p0.vt < vt_end) {
-        if (yldg) ldg_y(p0, yc); else issue(p0, 0);
+        issue(p0, 0);
         advance(p1);
-        if (p1.vt < vt_end && !yldg) issue(p1, 1);
+        if (p1.vt < vt_end) issue(p1, 1);
         p2 = p1;
         if (p1.vt < vt_end) advance(p2);
       }
@@ -788,22 +839,12 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         uint32_t v2[kChunk];
         if (a.sacc) ptx::tmem_ld_32x32b_x8(tmem_base + (uint32_t(quarter * 32) << 16) + uint32_t(acc * kMaxBN + 128 + box_of(p0) * a.BN + p0.ch * kChunk), v2);
         float xv[kChunk], yv[kChunk];
-        if (yldg) {
-          if (p1.vt < vt_end) ldg_y(p1, ynx);    // in flight while this item is updated
-          if (PAIR && p2.vt < vt_end && lane < kChunk) {   // ... and the item after it on its way from DRAM to the L2
-            const int r = p2.tm * kBM + quarter * 32, i = p2.tn * a.BN + p2.ch * kChunk + lane;
-            if (r < a.R && i < a.n) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.y + size_t(i) * a.R + r));
-          }
-#pragma unroll
-          for (int j = 0; j < kChunk; ++j) yv[j] = yc[j];
-        } else {
-          ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
-        }
+        ptx::mbar_wait(rbar0 + 8u * slot, (k >> 1) & 1u);
         const uint32_t src = ring_w + uint32_t(slot) * kSlotBytes + uint32_t(lane) * 4u;
 #pragma unroll
         for (int j = 0; j < kChunk; ++j) {
           if constexpr (X16) {
-            if (!yldg) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + uint32_t(j) * 128u));
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + uint32_t(j) * 128u));
           } else {
             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(xv[j]) : "r"(src + uint32_t(j) * 128u));
             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(yv[j]) : "r"(src + kRingSlot + uint32_t(j) * 128u));
@@ -835,12 +876,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         // reads have completed.  (Requested right after the ld.shared instructions were issued, the TMA write could land
         // before the last of them had read the slot: observed as rows 5..7 of a work item carrying the next item's y.)
         __syncwarp();
-        if (yldg) {
-#pragma unroll
-          for (int j = 0; j < kChunk; ++j) yc[j] = ynx[j];
-        } else if (p1.vt < vt_end && p2.vt < vt_end) {
-          issue(p2, slot);
-        }
+        if (p1.vt < vt_end && p2.vt < vt_end) issue(p2, slot);
         if (!same_box(p0, p1)) tile_done(p1.vt != p0.vt);
         p0 = p1; p1 = p2;
         if (p2.vt < vt_end) advance(p2);
@@ -1165,10 +1201,16 @@ typedef void (*StepKernel)(const CUtensorMap, const CUtensorMap, const CUtensorM
                            const CUtensorMap, const CUtensorMap, const CUtensorMap, const DenseArgs);
 StepKernel step_kernel_of(const DenseArgs& a) {
   const bool hints = a.pol_keep != ptx::kEvictNormal;
-  if (a.x16 && a.pair_lines) return hints ? dense_step_kernel<true, true, true, true> : dense_step_kernel<true, false, true, true>;
-  if (a.x16) return hints ? dense_step_kernel<true, true, true, false> : dense_step_kernel<true, false, true, false>;
-  if (a.ring) return hints ? dense_step_kernel<true, true, false, false> : dense_step_kernel<true, false, false, false>;
-  return hints ? dense_step_kernel<false, true, false, false> : dense_step_kernel<false, false, false, false>;
+  if (a.x16) {
+    if (a.pair_lines) {
+      if (a.yldg) return hints ? dense_step_kernel<true, true, true, true, true> : dense_step_kernel<true, false, true, true, true>;
+      return hints ? dense_step_kernel<true, true, true, true, false> : dense_step_kernel<true, false, true, true, false>;
+    }
+    if (a.yldg) return hints ? dense_step_kernel<true, true, true, false, true> : dense_step_kernel<true, false, true, false, true>;
+    return hints ? dense_step_kernel<true, true, true, false, false> : dense_step_kernel<true, false, true, false, false>;
+  }
+  if (a.ring) return hints ? dense_step_kernel<true, true, false, false, false> : dense_step_kernel<true, false, false, false, false>;
+  return hints ? dense_step_kernel<false, true, false, false, false> : dense_step_kernel<false, false, false, false, false>;
 }
 
 // One launch of the step kernel.  Per-step launches carry the programmatic-stream-serialization attribute (see the

@@ -1499,9 +1499,9 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.stage_out = (BN == kBK) ? 1 : 0;
   a.dsb = p.force_mode == 1 ? 1 : 0;
   a.x16 = x16_ok(a, y, false, p, t) ? 1 : 0;
-  // y by plain loads where the ring's 32 KB buy an operand stage that matters: many k-blocks per tile (mean degree >= 70:
-  // cfg2 33.6 -> 28.0 us per step; cfg1, degree 59: 24.2 -> 24.6, so it keeps the ring)
-  a.yldg = (a.x16 && (t.y_ring == 2 || (t.y_ring == 0 && g.nnz >= 70 * int64_t(n)))) ? 1 : 0;
+  // y by plain loads (its own twice-unrolled epilogue loop, and the ring's 32 KB become an operand stage) unless the caller
+  // asks for the ring: measured faster on every config (cfg1 24.2 -> 22.7 us per step with single boxes)
+  a.yldg = (a.x16 && t.y_ring != 1) ? 1 : 0;
   a.ring = (a.x16 || ring_ok(BN, R, x, y)) ? 1 : 0;
   a.sacc = (t.split_acc != 2 && BN <= 128 && !a.dsb) ? 1 : 0;
   choose_staging(a, BN * kBK * 2 + 2 * kStageX, t);
@@ -1727,9 +1727,8 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.stage_out = 1;
   a.dsb = p.force_mode == 1 ? 1 : 0;
   a.x16 = x16_ok(a, y, has_rem, p, t) ? 1 : 0;
-  // y by plain loads where the ring's 32 KB buy an operand stage that matters: two J terms (48 KB stages: 2 -> 3, cfg3
-  // 221 -> 217.5 us per step) or many k-blocks per tile (mean degree >= 70)
-  a.yldg = (a.x16 && (t.y_ring == 2 || (t.y_ring == 0 && (two_terms || g.nnz >= 70 * int64_t(n))))) ? 1 : 0;
+  // y by plain loads unless the caller asks for the ring (see dense_solve_steps; read graphs here: cfg1 25.1 -> 23.6 us)
+  a.yldg = (a.x16 && t.y_ring != 1) ? 1 : 0;
   a.ring = (a.x16 || ring_ok(kBK, R, x, y)) ? 1 : 0;
   a.j_terms = two_terms ? 2 : 1;
   a.sacc = (t.split_acc != 2 && !a.dsb) ? 1 : 0;

@@ -779,9 +779,13 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
 #pragma unroll
             for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v2[j]));
           }
-          set_step(p.vt);
-          if (a.c1_per_row) epi_update_x16<HINTS, true>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
-          else epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+          if (first) set_step(p.vt);                         // the ramp constant changes between boxes only
+          if constexpr (PAIR) {                              // pairs exist on the dense path only: one c1 for all rows
+            epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+          } else {
+            if (a.c1_per_row) epi_update_x16<HINTS, true>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+            else epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+          }
           if (!same_box(p, q)) tile_done(q.vt != p.vt);
           return nhave;
         };

@@ -281,3 +281,50 @@ def test_block_path_at_exact_tile_capacity(B, oracle, guarded, extra_tile):
         ccut, _ = oracle.cut_eval(row_ptr, cols, w, res["best_spins"].cpu().numpy())
         assert int(ccut[0]) == int(res["best_cut"].cpu()[0])
     assert guarded() >= 2
+
+
+# ------------------------------------------------------------------------------ paired tiles: same bits
+@pytest.mark.parametrize("shape", ["all-pairs-ragged", "pairs-and-singles"])
+def test_paired_tiles_are_bit_identical_to_single_boxes(B, oracle, shape):
+    """pair_tiles = 1 (two neighbouring 64-spin boxes share one N = 128 accumulator where that keeps the CTAs balanced) against
+    pair_tiles = 2 (every box on its own): a k-block that only one box of a pair lists contributes exact zeros to the other, so
+    every bit must agree -- fused launch and one launch per step, y through the ring and by plain loads, odd step counts, resume.
+    Shapes (148 CTAs): 36 boxes x 16 replica tiles -> every box is in a pair and the ragged last box (10 spins) is the RIGHT
+    half of one; 38 boxes x 8 replica tiles -> 18 pairs + 2 single boxes per replica tile.  Against the CSR path within 1e-3."""
+    import torch
+    scale, R = (0.28125, 2048) if shape == "all-pairs-ragged" else (0.3, 1024)
+    fr, pp = synth.make_config(1, scale=scale)
+    g, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    n, T = g.n, pp["T"]
+    boxes = (n + 63) // 64
+    assert (boxes, n % 64 != 0) == ((36, True) if shape == "all-pairs-ragged" else (38, True)), (n, boxes)
+    x0, y0 = synth.bsb_init_state(17, n, R)
+
+    def run(path=1, **knobs):
+        xg, yg = torch.from_numpy(x0.copy()).cuda(), torch.from_numpy(y0.copy()).cuda()
+        kw = dict(replicas=R, steps_total=T, weight_mode=1, path=path, dense_J=J if path == 1 else None, tile_skip=1 if path == 1 else 0,
+                  finalize=False, x=xg, y=yg, **knobs)
+        B.qhap_bsb_solve(g, step_begin=0, steps_run=9, **kw)
+        first = (xg.cpu().numpy(), yg.cpu().numpy())
+        B.qhap_bsb_solve(g, step_begin=9, steps_run=6, **kw)
+        return first, (xg.cpu().numpy(), yg.cpu().numpy())
+
+    ref = run(pair_tiles=2, step_launch=1)
+    for knobs in (dict(pair_tiles=1), dict(pair_tiles=1, step_launch=1), dict(pair_tiles=1, y_ring=1), dict(pair_tiles=1, y_ring=1, step_launch=1),
+                  dict(pair_tiles=2), dict()):
+        got = run(**knobs)
+        for a, b in zip(ref, got):
+            assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]), (shape, knobs)
+    # against the CSR path after the first 9 steps (all replicas), against the fp64 oracle after all 15 on sampled replicas (walls
+    # are hit from step 3 on here, so single marginal wall decisions separate fp32 trajectories of different kernels later on)
+    csr = run(path=2)
+    dx = np.abs(ref[0][0] - csr[0][0]).max(); dy = np.abs(ref[0][1] - csr[0][1]).max()
+    og = oracle.read_graph(fr)
+    sample = np.array([0, 5, R // 3, R - 1])
+    xo, yo = np.ascontiguousarray(x0[:, sample], np.float64), np.ascontiguousarray(y0[:, sample], np.float64)
+    oracle.bsb_run(og["row_ptr"].astype(np.int32), og["col"].astype(np.int32), (-oracle.read_weights(og, 1)).astype(np.float32), xo, yo,
+                   steps_total=T, step_begin=0, steps_run=15, n_threads=8)
+    ox = np.abs(ref[1][0][:, sample] - xo).max(); oy = np.abs(ref[1][1][:, sample] - yo).max()
+    print(f"paired tiles {shape}: n {n} R {R}: 9 steps against the CSR path max|dx| {dx:.2e} max|dy| {dy:.2e}; 15 steps against the oracle "
+          f"(4 replicas) {ox:.2e} {oy:.2e}")
+    assert dx <= 1e-3 and dy <= 1e-3 and ox <= 1e-3 and oy <= 1e-3

@@ -462,12 +462,13 @@ def run_ours(args):
         nz_blocks = int((cnt >= thr).sum())
         rem = cnt[inv] < thr                          # entries that go through the remainder CSR gather
         rem_rows = int(np.unique(rows[rem]).size)
-        # per spin-update: state16 (the 64-wide tiles' default when R % 4 == 0 and no remainder CSR) carries x as
+        # per spin-update: state16 (the 64-wide tiles' default when R % 4 == 0) carries x as
         # the fp16 pair -- read the pair 4 B, write it 4 B, read y 4 B, write y 4 B = 16 B; the fp32-x kernel adds x read and
         # written in fp32 = 24 B.  Plus the kept tiles of J once, and for a remainder: (col, val) once, one x row gathered per
         # entry, y read-modify-written for the rows that have one
-        state16 = (R % 4 == 0) and int(rem.sum()) == 0
-        state_bytes = 16.0 if state16 else 24.0
+        # next to a remainder CSR state16 also writes the fp32 x for the gather (write only): 20 B
+        state16 = (R % 4 == 0)
+        state_bytes = (20.0 if int(rem.sum()) > 0 else 16.0) if state16 else 24.0
         alg_bytes = state_bytes * g.n * R + nz_blocks * 64 * 64 * 2.0 * j_terms + int(rem.sum()) * (8.0 + 4.0 * R) + rem_rows * 8.0 * R
         extra["state_bytes_per_spin_update"] = state_bytes
         extra["remainder_nnz"] = int(rem.sum())

@@ -101,6 +101,9 @@ struct DenseArgs {
   // spins instead of 64 (the operand feed -- bytes in flight per SM against the L2 latency -- is what bounds the 64-wide
   // step).  Slots of a step: first the pairs (q-major, replica tile fastest), then the remaining boxes as singles; the state
   // side (staging buffers, TMA stores, done[]) stays per box.  pair_lines = pairs per replica tile (0: every slot is a box).
+  // state16 next to a remainder CSR (hybrid block path): the remainder gather reads fp32 x rows of the whole graph between two
+  // tile steps, so the epilogue also writes x' = (x_hi' + x_lo') 2^-15 to the fp32 array (write only: 20 B per spin-update)
+  int32_t xw32;
   int32_t pair_lines, n_slots;
   const int32_t* pk_cnt;      // [pair_lines] union of the two boxes' k-block lists
   const int32_t* pk_idx;      // [pair_lines][n_kblocks]
@@ -292,7 +295,7 @@ __device__ __forceinline__ void epi_update_store(const DenseArgs& a, const EpiCo
 // xs' = fma(c3 2^15, y', xs), wall at |xs'| > 2^15 -- bit for bit the fp32 update of x.  Pairs of spins are split and
 // canonicalised with packed fp16 instructions: (h, l) = (rn(xs'), rn(xs' - h)); H = h + l in fp16 (= rn16 of the exact sum),
 // L = (h - H) + l (both exact): (H, L) has the same sum and is a fixed point of the split (see split_half_canonical).
-template <bool hints, bool PER_ROW>
+template <bool hints, bool PER_ROW, bool XW = false>
 __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiConsts& ec, int tn, int tm, int ch, const uint32_t (&v)[kChunk],
                                                const float (&yv)[kChunk], uint32_t stg) {
   const int r = tm * kBM + ec.lane_r, i0 = tn * a.BN + ch * kChunk;
@@ -314,6 +317,7 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
     }
   }
   float yn[kChunk];
+  float xf[XW ? kChunk : 1];
   uint32_t hp[kChunk / 2], lp[kChunk / 2];
 #pragma unroll
   for (int q = 0; q < kChunk / 2; ++q) {
@@ -340,6 +344,11 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
     const __half2 L = __hadd2(__hsub2(h, H), l);
     hp[q] = *reinterpret_cast<const uint32_t*>(&H);
     lp[q] = *reinterpret_cast<const uint32_t*>(&L);
+    if constexpr (XW) {                          // the fp32 value of the pair, as merge_x_kernel forms it
+      const float2 Hf = __half22float2(H), Lf = __half22float2(L);
+      xf[2 * q] = (Hf.x + Lf.x) * (1.0f / kXScale);
+      xf[2 * q + 1] = (Hf.y + Lf.y) * (1.0f / kXScale);
+    }
   }
   uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
   if (interior) {
@@ -347,11 +356,15 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
     for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
       if constexpr (hints) ptx::st_global_f32_hint(a.y + off, yn[j], a.pol_stream);
       else a.y[off] = yn[j];
+      if constexpr (XW) a.x[off] = xf[j];
     }
   } else if (r < a.R) {
 #pragma unroll
     for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R))
-      if (i0 + j < a.n) a.y[off] = yn[j];
+      if (i0 + j < a.n) {
+        a.y[off] = yn[j];
+        if constexpr (XW) a.x[off] = xf[j];
+      }
   }
   ptx::st_shared_v4(addr, hp[0], hp[1], hp[2], hp[3]);
   ptx::st_shared_v4(addr + kStageX, lp[0], lp[1], lp[2], lp[3]);
@@ -360,8 +373,9 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
 // RING: the fp32 state arrives through the per-warp TMA ring; HINTS: L2 eviction priorities on every state access.
 // Compile-time variants keep each instantiation's hot loops small (the single run-time kernel had grown from 63 to 88 KB
 // of SASS and cost cfg3 3 %).
-// YLDG (state16 only): y by plain loads instead of the ring.
-template <bool RING, bool HINTS, bool X16, bool PAIR, bool YLDG>
+// YLDG (state16 only): y by plain loads instead of the ring.  XW (YLDG kernels without pairs): the epilogue also writes the fp32
+// x (DenseArgs::xw32; its own instantiation: as a run-time branch it cost cfg3 3.6 % through the size of the item loop).
+template <bool RING, bool HINTS, bool X16, bool PAIR, bool YLDG, bool XW>
 __global__ void __launch_bounds__(kThreads, 1)
 dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constant__ CUtensorMap tm_jl,
                   const __grid_constant__ CUtensorMap tm_xh,
@@ -782,6 +796,8 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           if (first) set_step(p.vt);                         // the ramp constant changes between boxes only
           if constexpr (PAIR) {                              // pairs exist on the dense path only: one c1 for all rows
             epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
+          } else if constexpr (XW) {                         // hybrid block path: per-row c1, fp32 x written next to the pair
+            epi_update_x16<HINTS, true, true>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
           } else {
             if (a.c1_per_row) epi_update_x16<HINTS, true>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
             else epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
@@ -1207,14 +1223,15 @@ StepKernel step_kernel_of(const DenseArgs& a) {
   const bool hints = a.pol_keep != ptx::kEvictNormal;
   if (a.x16) {
     if (a.pair_lines) {
-      if (a.yldg) return hints ? dense_step_kernel<true, true, true, true, true> : dense_step_kernel<true, false, true, true, true>;
-      return hints ? dense_step_kernel<true, true, true, true, false> : dense_step_kernel<true, false, true, true, false>;
+      if (a.yldg) return hints ? dense_step_kernel<true, true, true, true, true, false> : dense_step_kernel<true, false, true, true, true, false>;
+      return hints ? dense_step_kernel<true, true, true, true, false, false> : dense_step_kernel<true, false, true, true, false, false>;
     }
-    if (a.yldg) return hints ? dense_step_kernel<true, true, true, false, true> : dense_step_kernel<true, false, true, false, true>;
-    return hints ? dense_step_kernel<true, true, true, false, false> : dense_step_kernel<true, false, true, false, false>;
+    if (a.yldg && a.xw32) return hints ? dense_step_kernel<true, true, true, false, true, true> : dense_step_kernel<true, false, true, false, true, true>;
+    if (a.yldg) return hints ? dense_step_kernel<true, true, true, false, true, false> : dense_step_kernel<true, false, true, false, true, false>;
+    return hints ? dense_step_kernel<true, true, true, false, false, false> : dense_step_kernel<true, false, true, false, false, false>;
   }
-  if (a.ring) return hints ? dense_step_kernel<true, true, false, false, false> : dense_step_kernel<true, false, false, false, false>;
-  return hints ? dense_step_kernel<false, true, false, false, false> : dense_step_kernel<false, false, false, false, false>;
+  if (a.ring) return hints ? dense_step_kernel<true, true, false, false, false, false> : dense_step_kernel<true, false, false, false, false, false>;
+  return hints ? dense_step_kernel<false, true, false, false, false, false> : dense_step_kernel<false, false, false, false, false, false>;
 }
 
 // One launch of the step kernel.  Per-step launches carry the programmatic-stream-serialization attribute (see the
@@ -1466,7 +1483,8 @@ int32_t choose_pair_lines(int32_t n_tiles_n, int32_t n_tiles_m, int grid, int mi
 // multiple of 16 bytes, aligned base) and nothing outside the step kernel needs the fp32 x between steps (no remainder
 // gather, no dSB sign copies).
 bool x16_ok(const DenseArgs& a, const float* y, bool has_rem, const qhap_bsb_params& p, const qhap_bsb_tuning& t) {
-  return t.state16 != 2 && a.stage_out && a.BN == kBK && a.R % 4 == 0 && (reinterpret_cast<uintptr_t>(y) & 15) == 0 && !has_rem &&
+  return t.state16 != 2 && a.stage_out && a.BN == kBK && a.R % 4 == 0 && (reinterpret_cast<uintptr_t>(y) & 15) == 0 &&
+         (!has_rem || t.y_ring != 1) &&      // with a remainder CSR: the plain-y loop, which also writes the fp32 x (DenseArgs::xw32)
          p.force_mode == 0;
 }
 }  // namespace
@@ -1518,7 +1536,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.kb_idx = skip ? w.kb_idx : nullptr;
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
-  a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = w.pk_cnt; a.pk_idx = w.pk_idx;
+  a.xw32 = 0; a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = w.pk_cnt; a.pk_idx = w.pk_idx;
   set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
@@ -1743,6 +1761,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.n_tiles_n = n_t;
   a.n_kblocks = n_t;
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
+  a.xw32 = (a.x16 && has_rem) ? 1 : 0;
   a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = nullptr; a.pk_idx = nullptr;
   a.c1 = c1row; a.c1_per_row = 1;
   a.x = x; a.y = y;
@@ -1761,6 +1780,10 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   const dim3 tgrid(unsigned(ceil_div(n_k, 32)), unsigned(ceil_div(R, 32)));
   split_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, a.x16 ? 2 : a.dsb, x, xh[0], xl[0]);
   QHAP_LAUNCH_CHECK();
+  if (a.xw32) {                       // the remainder gather of the first step must see the pair's value, not the caller's fp32 x
+    merge_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, xh[0], xl[0], x);
+    QHAP_LAUNCH_CHECK();
+  }
   const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
   a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
   int cur = 0;

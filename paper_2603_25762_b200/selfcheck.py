@@ -37,6 +37,13 @@ def main(steps: int = 6) -> int:
     for path, kw in ((1, dict(tile_skip=1)), (1, dict(tile_skip=1, step_launch=1)), (4, {}), (4, dict(state16=2)), (1, dict(tile_skip=1, eval_every=3))):
         B.qhap_bsb_solve(g, replicas=264, steps_total=p["T"], steps_run=steps, seed=2, weight_mode=1, path=path, dense_J=J if path == 1 else None, **kw)
         ok(f"solve cfg1-scaled path {path} {kw}")
+    # paired tiles (two boxes per N = 128 accumulator): active from two boxes per CTA on -- 38 boxes x 8 replica tiles
+    fr, p = synth.make_config(1, scale=0.3)
+    g, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    for kw in (dict(), dict(step_launch=1), dict(pair_tiles=2), dict(y_ring=1)):
+        B.qhap_bsb_solve(g, replicas=1024, steps_total=p["T"], steps_run=steps, seed=2, weight_mode=1, path=1, tile_skip=1, dense_J=J, **kw)
+        ok(f"solve cfg1-scaled paired tiles {kw}")
+    B.qhap_cut_eval_static(g, 1, torch.ones((g.n, 300), dtype=torch.int8, device="cuda")); ok("cut_eval_static")
     # SNP graph: build (both depths), block split, batched block path and CSR path, stitch, SNP readout
     fr, p = synth.make_config(3, scale=0.005)
     d3 = B.upload_frags(fr)

@@ -255,6 +255,15 @@ QHAP_API qhap_status qhap_component_merge(int32_t n, int32_t n_kept, const int32
 QHAP_API const char *qhap_last_error(void);
 /* Number of CUDA kernels this library has launched in this process so far (monotonic; bench.py reports the difference
  * over its timed region as "gpu_launches"). */
+/* HOST-only query (no device, nothing launched): the paired-tile plan of the dense tile_skip step for a graph
+ * of n_boxes 64-spin boxes and n_replica_tiles 128-replica tiles on `grid` CTAs.  Slots of a step are numbered pairs first
+ * (pair q of replica tile m: slot q n_replica_tiles + m, boxes 2q and 2q + 1), then the boxes from 2 pairs_per_line on as
+ * singles (box b of replica tile m: slot (b - pairs_per_line) n_replica_tiles + m); slot s runs on CTA s % grid.  Returns the
+ * pairs per replica tile the library would use (0 = no pairs) and the largest / smallest number of boxes any CTA gets per step.
+ * min_boxes: 2 for fused launches (state prefetch distance), 0 for one launch per step. */
+QHAP_API qhap_status qhap_plan_pair_tiles(int32_t n_boxes, int32_t n_replica_tiles, int32_t grid, int32_t min_boxes,
+                                 int32_t *pairs_per_line, int32_t *max_boxes_per_cta, int32_t *min_boxes_per_cta);
+
 QHAP_API uint64_t qhap_launch_count(void);
 /* Library / build identification, e.g. "qhap-b200 0.1 sm_100a". */
 QHAP_API const char *qhap_version(void);

@@ -26,7 +26,7 @@ QHAP_DENSE_NONE, QHAP_DENSE_FP16, QHAP_DENSE_BF16 = 0, 1, 2
 EXPORTS = ["qhap_build_read_graph", "qhap_build_snp_graph", "qhap_build_snp_graph_fill", "qhap_bsb_solve", "qhap_cut_eval", "qhap_cut_eval_static",
            "qhap_phase_readout_reads", "qhap_phase_readout_snps", "qhap_block_split", "qhap_block_stitch",
            "qhap_gauge_transform", "qhap_flip_count_update", "qhap_refine_readout", "qhap_snp_refine",
-           "qhap_component_split", "qhap_component_merge",
+           "qhap_component_split", "qhap_component_merge", "qhap_plan_pair_tiles",
            "qhap_last_error", "qhap_launch_count", "qhap_version"]
 
 
@@ -424,6 +424,14 @@ def qhap_cut_eval_static(graph: Csr, weight_mode: int, spins: torch.Tensor, cut:
     _check(_lib.qhap_cut_eval_static(C.byref(gs), C.c_int32(weight_mode), _ptr(spins), C.c_int32(R), _ptr(cut), _ptr(energy), _stream()),
            "qhap_cut_eval_static")
     return cut, energy
+
+
+def qhap_plan_pair_tiles(n_boxes: int, n_replica_tiles: int, grid: int, min_boxes: int = 2):
+    """Host-only: (pairs per replica tile, max boxes per CTA, min boxes per CTA) of the paired-tile plan."""
+    out = [C.c_int32(0) for _ in range(3)]
+    _check(_lib.qhap_plan_pair_tiles(C.c_int32(n_boxes), C.c_int32(n_replica_tiles), C.c_int32(grid), C.c_int32(min_boxes),
+                                     *[C.byref(o) for o in out]), "qhap_plan_pair_tiles")
+    return tuple(int(o.value) for o in out)
 
 
 def qhap_phase_readout_reads(frags: Frags, spins: torch.Tensor) -> torch.Tensor:

@@ -1461,19 +1461,22 @@ DenseWs carve_dense(Workspace& ws, int32_t n, int32_t R) {
 // the most loaded CTA (in boxes), so: the largest number of pairs that does not raise that maximum above what single boxes
 // give, ceil(boxes / grid) -- or, when min_boxes > 0 (fused launches: state prefetch distance), leaves a CTA with fewer
 // than min_boxes boxes per step.
+void pair_plan_loads(int32_t n_tiles_n, int32_t n_tiles_m, int grid, int32_t P, int64_t& mx, int64_t& mn) {   // boxes per CTA: max, min
+  const int64_t np = int64_t(P) * n_tiles_m, ns = int64_t(n_tiles_n - 2 * P) * n_tiles_m;
+  mx = 0; mn = INT64_MAX;
+  for (int c = 0; c < grid; ++c) {
+    const int64_t pc = np / grid + (c < np % grid ? 1 : 0);
+    const int64_t c0 = ((c - np) % grid + grid) % grid;            // first single i with (np + i) % grid == c
+    const int64_t sc = c0 < ns ? (ns - c0 + grid - 1) / grid : 0;
+    mx = std::max(mx, 2 * pc + sc);
+    mn = std::min(mn, 2 * pc + sc);
+  }
+}
 int32_t choose_pair_lines(int32_t n_tiles_n, int32_t n_tiles_m, int grid, int min_boxes) {
-  const int64_t boxes = int64_t(n_tiles_n) * n_tiles_m;
-  const int64_t target = ceil_div(boxes, grid);
+  const int64_t target = ceil_div(int64_t(n_tiles_n) * n_tiles_m, grid);
   for (int32_t P = n_tiles_n / 2; P > 0; --P) {
-    const int64_t np = int64_t(P) * n_tiles_m, ns = int64_t(n_tiles_n - 2 * P) * n_tiles_m;
-    int64_t mx = 0, mn = INT64_MAX;
-    for (int c = 0; c < grid; ++c) {
-      const int64_t pc = np / grid + (c < np % grid ? 1 : 0);
-      const int64_t c0 = ((c - np) % grid + grid) % grid;            // first single i with (np + i) % grid == c
-      const int64_t sc = c0 < ns ? (ns - c0 + grid - 1) / grid : 0;
-      mx = std::max(mx, 2 * pc + sc);
-      mn = std::min(mn, 2 * pc + sc);
-    }
+    int64_t mx, mn;
+    pair_plan_loads(n_tiles_n, n_tiles_m, grid, P, mx, mn);
     if (mx <= target && mn >= min_boxes) return P;
   }
   return 0;
@@ -1815,3 +1818,19 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
 }
 
 }  // namespace qhap
+
+// Host-only query of the paired-tile plan (no device needed): what dense_solve_steps would choose for this shape.
+extern "C" qhap_status qhap_plan_pair_tiles(int32_t n_boxes, int32_t n_replica_tiles, int32_t grid, int32_t min_boxes,
+                                            int32_t* pairs_per_line, int32_t* max_boxes_per_cta, int32_t* min_boxes_per_cta) {
+  using namespace qhap;
+  QHAP_REQUIRE(n_boxes >= 1 && n_replica_tiles >= 1 && grid >= 1 && min_boxes >= 0, "bad sizes");
+  QHAP_REQUIRE(pairs_per_line && max_boxes_per_cta && min_boxes_per_cta, "output pointers must not be NULL");
+  QHAP_REQUIRE(int64_t(grid) <= int64_t(n_boxes) * n_replica_tiles, "grid larger than the number of boxes");
+  const int32_t P = choose_pair_lines(n_boxes, n_replica_tiles, grid, min_boxes);
+  int64_t mx, mn;
+  pair_plan_loads(n_boxes, n_replica_tiles, grid, P, mx, mn);
+  *pairs_per_line = P;
+  *max_boxes_per_cta = int32_t(mx);
+  *min_boxes_per_cta = int32_t(mn);
+  return QHAP_OK;
+}

@@ -104,3 +104,29 @@ def test_no_oracle_in_product_path():
         assert "oracle" not in re.sub(r"#.*|\"\"\".*?\"\"\"", "", f.read_text(), flags=re.S).replace("the oracle", ""), f
     for f in (ROOT / "paper_2603_25762_b200" / "csrc").glob("*.cu*"):
         assert "orc_" not in f.read_text() and "oracle/" not in f.read_text().replace("used by oracle/", ""), f
+
+
+def test_pair_tile_plan_covers_every_box_once_and_balances(lib):
+    """qhap_plan_pair_tiles (host only): rebuilding the slot list from the documented numbering, every box appears in exactly one
+    slot, the reported per-CTA maxima / minima are those of slot % grid, pairs never raise the most loaded CTA above
+    ceil(boxes / grid), and fused plans leave every CTA at least two boxes.  cfg1's shape gives the plan DESIGN.md 4.4g quotes."""
+    from paper_2603_25762_b200 import binding as B
+    assert B.qhap_plan_pair_tiles(125, 8, 148, 2) == (55, 7, 5)
+    for n_boxes, m, grid, min_boxes in [(125, 8, 148, 2), (63, 16, 148, 2), (38, 8, 148, 2), (36, 16, 148, 2), (36, 16, 148, 0), (13, 3, 39, 0),
+                                        (2, 1, 2, 0), (2, 1, 1, 2), (3672, 2, 148, 0), (9, 5, 22, 2), (40, 1, 7, 2), (41, 4, 148, 2), (1, 1, 1, 0)]:
+        P, mx, mn = B.qhap_plan_pair_tiles(n_boxes, m, grid, min_boxes)
+        assert 0 <= P <= n_boxes // 2
+        slots = [(2 * q, 2, t) for q in range(P) for t in range(m)] + [(b, 1, t) for b in range(2 * P, n_boxes) for t in range(m)]
+        seen = set()
+        load = [0] * grid
+        for s, (b0, w, t) in enumerate(slots):
+            for b in range(b0, b0 + w):
+                assert (b, t) not in seen
+                seen.add((b, t))
+            load[s % grid] += w
+        assert len(seen) == n_boxes * m
+        assert (max(load), min(load)) == (mx, mn), (n_boxes, m, grid, P)
+        if P > 0:
+            assert mx <= -(-n_boxes * m // grid) and mn >= min_boxes
+    with pytest.raises(B.QhapError):
+        B.qhap_plan_pair_tiles(4, 1, 5, 0)                     # more CTAs than boxes

@@ -85,7 +85,9 @@ enum { QHAP_DENSE_NONE = 0, QHAP_DENSE_FP16 = 1, QHAP_DENSE_BF16 = 2 };
  * count pass runs: row_ptr and out->nnz (required) are written and QHAP_ERR_WORKSPACE is returned when col != NULL.
  * Otherwise col/d/c are filled.  Optionally also writes J = -w (Eq. 4) for `weight_mode` as a dense row-major
  * [dense_ld x dense_ld] matrix (dense_ld >= n_frag, multiple of 8; padding rows/cols written as 0) in fp16 or bf16;
- * an entry that is not exactly representable gives QHAP_ERR_RANGE (checked on device, reported after the sync). */
+ * an entry that is not exactly representable gives QHAP_ERR_RANGE (checked on device, reported after the sync).
+ * The call synchronises the stream ONCE, at its end: with col != NULL the fill kernels follow the count and the scan directly
+ * and check on the device that the entries fit (if they do not, col/d/c and dense_J are left untouched). */
 QHAP_API qhap_status qhap_build_read_graph(const qhap_frags *frags, int32_t weight_mode, qhap_csr *out, void *dense_J,
                                   int32_t dense_ld, int32_t dense_dtype, void *workspace, size_t *ws_bytes,
                                   void *stream);

@@ -116,9 +116,12 @@ __global__ void __launch_bounds__(256) read_pairs_kernel(int32_t n, const int64_
                                                          const uint8_t* __restrict__ allele, FragMeta m,
                                                          int32_t* __restrict__ row_ptr /*COUNT: counts out; FILL: offsets in*/,
                                                          int32_t* __restrict__ col, int32_t* __restrict__ dd,
-                                                         int32_t* __restrict__ cc) {
+                                                         int32_t* __restrict__ cc, int64_t capacity) {
   const int32_t a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (a >= n) return;
+  // FILL runs right behind the count and the scan, without a host round trip in between: it looks at their verdict itself
+  // (bad input, 2^31 entries, more entries than the caller's arrays hold) and leaves the arrays alone if there is one
+  if (FILL && (m.flags[0] != 0 || m.flags[1] != 0 || *m.total > capacity)) return;
   const int lane = threadIdx.x & 31;
   const int32_t fa = m.first[a], la = m.last[a];
   // lo = first b with pmax[b] >= fa; hi = last b with first[b] <= la  (both arrays are non-decreasing)
@@ -161,8 +164,10 @@ template <class HT>
 __global__ void __launch_bounds__(256) dense_j_kernel(int32_t n, int32_t ld, const int32_t* __restrict__ row_ptr,
                                                       const int32_t* __restrict__ col, const int32_t* __restrict__ dd,
                                                       const int32_t* __restrict__ cc, int mode, int32_t limit,
-                                                      HT* __restrict__ J, int32_t* __restrict__ flags) {
+                                                      HT* __restrict__ J, int32_t* __restrict__ flags,
+                                                      const int64_t* __restrict__ total, int64_t capacity) {
   __shared__ __align__(16) HT row[kDenseChunk];
+  if (flags[0] != 0 || flags[1] != 0 || *total > capacity) return;      // see read_pairs_kernel<true>
   const int32_t a = blockIdx.x;
   const int32_t e0 = a < n ? row_ptr[a] : 0, e1 = a < n ? row_ptr[a + 1] : 0;
   for (int32_t c0 = 0; c0 < ld; c0 += kDenseChunk) {
@@ -222,10 +227,31 @@ extern "C" qhap_status qhap_build_read_graph(const qhap_frags* fr, int32_t weigh
     prefix_max_kernel<<<1, 1024, 0, stream>>>(n, m.last, m.pmax);
     QHAP_LAUNCH_CHECK();
     read_pairs_kernel<false><<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, fr->frag_ptr, fr->snp_idx, fr->allele,
-                                                                                  m, out->row_ptr, nullptr, nullptr, nullptr);
+                                                                                  m, out->row_ptr, nullptr, nullptr, nullptr, 0);
     QHAP_LAUNCH_CHECK();
   }
   QHAP_TRY(exclusive_scan_i32(out->row_ptr, out->row_ptr, n, m.total, m.flags + 1, stream));
+  // Count-only call, or count + fill in ONE round trip: the fill kernels check the count's verdict on the device, the host
+  // reads it once at the end.
+  const bool fill = out->col != nullptr;
+  if (fill) {
+    QHAP_REQUIRE(out->d && out->c, "out->d and out->c must not be NULL when out->col is given");
+    if (n > 0) {
+      read_pairs_kernel<true><<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, fr->frag_ptr, fr->snp_idx, fr->allele, m,
+                                                                                   out->row_ptr, out->col, out->d, out->c, capacity);
+      QHAP_LAUNCH_CHECK();
+    }
+    if (dense_J && dense_ld > 0) {
+      if (dense_dtype == QHAP_DENSE_FP16)
+        dense_j_kernel<__half><<<dense_ld, 256, 0, stream>>>(n, dense_ld, out->row_ptr, out->col, out->d, out->c, weight_mode,
+                                                            2048, static_cast<__half*>(dense_J), m.flags, m.total, capacity);
+      else
+        dense_j_kernel<__nv_bfloat16><<<dense_ld, 256, 0, stream>>>(n, dense_ld, out->row_ptr, out->col, out->d, out->c,
+                                                                   weight_mode, 256, static_cast<__nv_bfloat16*>(dense_J), m.flags,
+                                                                   m.total, capacity);
+      QHAP_LAUNCH_CHECK();
+    }
+  }
   int64_t total = 0;
   int32_t flags[4] = {0, 0, 0, 0};
   QHAP_CUDA_TRY(cudaMemcpyAsync(&total, m.total, sizeof(total), cudaMemcpyDeviceToHost, stream));
@@ -234,25 +260,8 @@ extern "C" qhap_status qhap_build_read_graph(const qhap_frags* fr, int32_t weigh
   if (flags[0]) { set_error("fragments must be non-empty and sorted by their first SNP index"); return QHAP_ERR_INVALID_ARG; }
   if (flags[1]) { set_error("read graph has >= 2^31 directed entries"); return QHAP_ERR_RANGE; }
   out->nnz = total;
-  if (out->col == nullptr) return QHAP_OK;   // count-only call
+  if (!fill) return QHAP_OK;   // count-only call
   if (capacity < total) { set_error("edge capacity too small: %lld < %lld", (long long)capacity, (long long)total); return QHAP_ERR_WORKSPACE; }
-  QHAP_REQUIRE(out->d && out->c, "out->d and out->c must not be NULL when out->col is given");
-  if (n > 0) {
-    read_pairs_kernel<true><<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, fr->frag_ptr, fr->snp_idx, fr->allele, m,
-                                                                                 out->row_ptr, out->col, out->d, out->c);
-    QHAP_LAUNCH_CHECK();
-  }
-  if (dense_J && dense_ld > 0) {
-    if (dense_dtype == QHAP_DENSE_FP16)
-      dense_j_kernel<__half><<<dense_ld, 256, 0, stream>>>(n, dense_ld, out->row_ptr, out->col, out->d, out->c, weight_mode,
-                                                          2048, static_cast<__half*>(dense_J), m.flags);
-    else
-      dense_j_kernel<__nv_bfloat16><<<dense_ld, 256, 0, stream>>>(n, dense_ld, out->row_ptr, out->col, out->d, out->c,
-                                                                 weight_mode, 256, static_cast<__nv_bfloat16*>(dense_J), m.flags);
-    QHAP_LAUNCH_CHECK();
-    QHAP_CUDA_TRY(cudaMemcpyAsync(flags, m.flags, sizeof(flags), cudaMemcpyDeviceToHost, stream));
-    QHAP_CUDA_TRY(cudaStreamSynchronize(stream));
-    if (flags[2]) { set_error("a weight is not exactly representable in the dense dtype (|w| > %d)", dense_dtype == QHAP_DENSE_FP16 ? 2048 : 256); return QHAP_ERR_RANGE; }
-  }
+  if (flags[2]) { set_error("a weight is not exactly representable in the dense dtype (|w| > %d)", dense_dtype == QHAP_DENSE_FP16 ? 2048 : 256); return QHAP_ERR_RANGE; }
   return QHAP_OK;
 }

@@ -352,11 +352,12 @@ __device__ __forceinline__ void epi_update_x16(const DenseArgs& a, const EpiCons
   }
   uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
   if (interior) {
+    float* yb = a.y + off;
 #pragma unroll
-    for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) {
-      if constexpr (hints) ptx::st_global_f32_hint(a.y + off, yn[j], a.pol_stream);
-      else a.y[off] = yn[j];
-      if constexpr (XW) a.x[off] = xf[j];
+    for (int j = 0; j < kChunk; ++j) {
+      if constexpr (hints) ptx::st_global_f32_hint(yb + uint32_t(j) * uint32_t(a.R), yn[j], a.pol_stream);
+      else yb[uint32_t(j) * uint32_t(a.R)] = yn[j];
+      if constexpr (XW) a.x[off + uint32_t(j) * uint32_t(a.R)] = xf[j];
     }
   } else if (r < a.R) {
 #pragma unroll
@@ -698,7 +699,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
       }
       if (a.stage_out && a.store_warp) {
         ptx::fence_proxy_async();
-        if (RING && a.fused && ++tcount == a.fence_every) { tcount = 0; ptx::fence_proxy_async_global(); }
+        if constexpr (RING && !YLDG) {                  // only the TMA ring re-reads generic stores through the async proxy
+          if (a.fused && ++tcount == a.fence_every) { tcount = 0; ptx::fence_proxy_async_global(); }
+        }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(stg_full(stg_i));
         if (++stg_i == a.stg_bufs) { stg_i = 0; stg_par ^= 1u; }
@@ -761,8 +764,9 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
           const int r = p.tm * kBM + ec.lane_r, i0 = p.tn * a.BN + p.ch * kChunk;
           uint32_t off = uint32_t(i0) * uint32_t(a.R) + uint32_t(r);
           if (r < a.R && i0 + kChunk <= a.n) {
+            const float* yb = a.y + off;               // one wide multiply-add per address: base + j R
 #pragma unroll
-            for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) dst[j] = a.y[off];
+            for (int j = 0; j < kChunk; ++j) dst[j] = yb[uint32_t(j) * uint32_t(a.R)];
           } else {
 #pragma unroll
             for (int j = 0; j < kChunk; ++j, off += uint32_t(a.R)) dst[j] = (r < a.R && i0 + j < a.n) ? a.y[off] : 0.f;

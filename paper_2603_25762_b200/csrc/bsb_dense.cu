@@ -104,6 +104,10 @@ struct DenseArgs {
   // state16 next to a remainder CSR (hybrid block path): the remainder gather reads fp32 x rows of the whole graph between two
   // tile steps, so the epilogue also writes x' = (x_hi' + x_lo') 2^-15 to the fp32 array (write only: 20 B per spin-update)
   int32_t xw32;
+  // fused state16: the staging buffer is reloaded (the pair of the box two ahead) as soon as the store has READ it, before the
+  // store's completion is waited for and signalled.  Safe only if that box is not the one just stored, i.e. every CTA has at
+  // least three boxes per step (its pair was then stored, and waited for, at least one box earlier).
+  int32_t early_reload;
   int32_t pair_lines, n_slots;
   const int32_t* pk_cnt;      // [pair_lines] union of the two boxes' k-block lists
   const int32_t* pk_idx;      // [pair_lines][n_kblocks]
@@ -614,11 +618,12 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         ptx::tma_store_commit();
         ptx::tma_store_wait_read_all();
         if constexpr (!X16) ptx::mbar_arrive(stg_empty(b));
+        if constexpr (X16) { if (a.early_reload) load_next(); }   // into the buffer just read (b_ld == b)
         if (a.fused) {
           ptx::tma_store_wait_all();
           ptx::signal_add_release(a.done + (tn * a.n_tiles_m + tm), 1u);
         }
-        if constexpr (X16) load_next();            // into the buffer just read (b_ld == b)
+        if constexpr (X16) { if (!a.early_reload) load_next(); }
         if (++b == a.stg_bufs) { b = 0; bpar ^= 1u; }
         }
       }
@@ -1319,6 +1324,8 @@ int fused_grid(const DenseArgs& a, const qhap_bsb_params& p, const qhap_bsb_tuni
   return int(grid);
 }
 
+void pair_plan_loads(int32_t n_tiles_n, int32_t n_tiles_m, int grid, int32_t P, int64_t& mx, int64_t& mn);
+
 // All steps of the call in as few launches as the 32-bit virtual tile index allows (one, at every BASELINE size).
 // tm_h / tm_l: the two buffers of split copies; buffer `cur` holds the current x.  Returns the buffer that holds x after.
 qhap_status launch_fused(int grid, cudaStream_t stream, const CUtensorMap& tj, const CUtensorMap& tjl, const CUtensorMap (&tm_h)[2],
@@ -1329,6 +1336,11 @@ qhap_status launch_fused(int grid, cudaStream_t stream, const CUtensorMap& tj, c
   a.store_warp = 1;
   a.tile_stride = int32_t(ceil_div(int64_t(a.n_slots), grid) * grid);
   a.fence_every = uint32_t(std::max<int64_t>(1, int64_t(a.n_slots) / grid - 1));
+  {
+    int64_t mx, mn;                               // boxes per CTA and step
+    pair_plan_loads(a.n_tiles_n, a.n_tiles_m, grid, a.pair_lines, mx, mn);
+    a.early_reload = (a.x16 && mn >= 3) ? 1 : 0;
+  }
   a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0;
   a.c3 = float(p.dt * p.a0);
   a.c2 = 0.f;
@@ -1543,7 +1555,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.kb_idx = skip ? w.kb_idx : nullptr;
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
-  a.xw32 = 0; a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = w.pk_cnt; a.pk_idx = w.pk_idx;
+  a.xw32 = 0; a.early_reload = 0; a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = w.pk_cnt; a.pk_idx = w.pk_idx;
   set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
@@ -1769,6 +1781,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.n_kblocks = n_t;
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
   a.xw32 = (a.x16 && has_rem) ? 1 : 0;
+  a.early_reload = 0;
   a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = nullptr; a.pk_idx = nullptr;
   a.c1 = c1row; a.c1_per_row = 1;
   a.x = x; a.y = y;

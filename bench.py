@@ -455,10 +455,14 @@ def run_ours(args):
         tiles, inv, cnt = np.unique(tile_id, return_inverse=True, return_counts=True)
         j_terms = 2 if (path == 4 and snp) else 1     # fp32 SNP weights are stored as J_hi + J_lo
         thr = 1
+        tile_cost = 8192.0 * j_terms + 32768.0 * ((R + 127) // 128)      # the library's first threshold (tile_threshold)
+        thr0 = 16
+        while thr0 < 4096 and thr0 * 1.4142 < tile_cost / (1.2 * (8.0 + 4.0 * R)):
+            thr0 *= 2
         if path == 4:                                 # the library's rule: keep all tiles if they fit the
-            cap = 16 * g.nnz // 4096 + (g.n + 63) // 64 + 1      # capacity, else only tiles with >= 16, 64, ... entries
+            cap = 16 * g.nnz // 4096 + (g.n + 63) // 64 + 1      # capacity, else only tiles with >= thr0, 2 thr0, ... entries
             while int((cnt >= thr).sum()) > cap:
-                thr = 16 if thr == 1 else thr * 4
+                thr = thr0 if thr == 1 else thr * 2
         nz_blocks = int((cnt >= thr).sum())
         rem = cnt[inv] < thr                          # entries that go through the remainder CSR gather
         rem_rows = int(np.unique(rows[rem]).size)

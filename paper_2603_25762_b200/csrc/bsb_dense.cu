@@ -1633,6 +1633,14 @@ namespace qhap {
 namespace {
 // capacity of the tile arrays: 16x the CSR's own entries, plus one (possibly empty) tile per 64 rows
 int64_t block_capacity(int32_t n, int64_t nnz) { return 16 * nnz / (kBK * kBK) + ceil_div(n, kBK) + 1; }
+// first threshold (entries per tile) tried when not all tiles fit; see block_solve_steps
+int32_t tile_threshold(int32_t R, int32_t j_terms) {
+  const double tile = 8192.0 * j_terms + 32768.0 * double(ceil_div(R, kBM));
+  const double entry = 1.2 * (8.0 + 4.0 * R);
+  int32_t thr = 16;
+  while (thr < kBK * kBK && double(thr) * 1.4142 < tile / entry) thr *= 2;      // nearest power of two on a log scale, at least 16
+  return thr;
+}
 }  // namespace
 
 namespace {
@@ -1712,7 +1720,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   const bool two_terms = weight_mode == QHAP_WEIGHT_FX;      // integer counts are exact in fp16 (|J| <= 2048 checked below)
 
   // tile occupancy -> tile lists -> block offsets.  All tiles are kept if they fit the capacity (banded graphs); otherwise
-  // only tiles with at least thr = 16, 64, ... entries are kept and the rest of the entries (long-range edges) become a
+  // only tiles with at least thr entries (tile_threshold, then doubled) are kept and the rest of the entries (long-range edges) become a
   // remainder CSR that a small gather kernel adds into y before each tile step.  One host synchronisation per attempt.
   QHAP_CUDA_TRY(cudaMemsetAsync(flags, 0, sizeof(int32_t) * size_t(n_t) * n_t, stream));
   QHAP_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(uint32_t) * 4, stream));
@@ -1724,8 +1732,13 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   }
   int64_t total_blocks = 0;
   uint32_t amax_bits = 0;
+  // Which tiles to keep when they do not all fit: a kept tile costs its 8 KB per J term plus a 32 KB x k-block per replica tile,
+  // an entry left to the remainder CSR (8 + 4 R) bytes of latency-bound gather (weighted 1.2) -- break-even entries per tile, as a
+  // power of two.  Measured: cfg4 (R = 128, two J terms) 210.6 us per step at 16, 195.7 at 32 and at 64, 203.8 at 128; cfg1 with
+  // Pore-C fragments (R = 1,024, one term) 285.6 at 32, 262.0 at 64.  Both get 64.  Doubled until the tiles fit.
+  const int32_t thr0 = tile_threshold(R, two_terms ? 2 : 1);
   int32_t thr = 1;
-  for (;; thr = (thr == 1 ? 16 : thr * 4)) {
+  for (;; thr = (thr == 1 ? thr0 : thr * 2)) {
     tile_list_kernel<<<n_t, 32, 0, stream>>>(n_t, flags, thr, kb_cnt, kb_idx);
     QHAP_LAUNCH_CHECK();
     QHAP_TRY(exclusive_scan_i32(kb_cnt, blk_ptr, n_t, totals, reinterpret_cast<int32_t*>(totals + 1), stream));

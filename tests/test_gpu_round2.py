@@ -284,20 +284,24 @@ def test_block_path_at_exact_tile_capacity(B, oracle, guarded, extra_tile):
 
 
 # ------------------------------------------------------------------------------ paired tiles: same bits
-@pytest.mark.parametrize("shape", ["all-pairs-ragged", "pairs-and-singles"])
+@pytest.mark.parametrize("shape", ["all-pairs-ragged", "pairs-and-singles", "three-boxes-per-cta"])
 def test_paired_tiles_are_bit_identical_to_single_boxes(B, oracle, shape):
     """pair_tiles = 1 (two neighbouring 64-spin boxes share one N = 128 accumulator where that keeps the CTAs balanced) against
     pair_tiles = 2 (every box on its own): a k-block that only one box of a pair lists contributes exact zeros to the other, so
     every bit must agree -- fused launch and one launch per step, y through the ring and by plain loads, odd step counts, resume.
     Shapes (148 CTAs): 36 boxes x 16 replica tiles -> every box is in a pair and the ragged last box (10 spins) is the RIGHT
-    half of one; 38 boxes x 8 replica tiles -> 18 pairs + 2 single boxes per replica tile.  Against the CSR path within 1e-3."""
+    half of one; 38 boxes x 8 replica tiles -> 18 pairs + 2 single boxes per replica tile; 38 boxes x 16 replica tiles -> every CTA
+    has at least three boxes per step, so the fused launch reloads its staging buffers early.  Against the CSR
+    path within 1e-3."""
     import torch
-    scale, R = (0.28125, 2048) if shape == "all-pairs-ragged" else (0.3, 1024)
+    scale, R = {"all-pairs-ragged": (0.28125, 2048), "pairs-and-singles": (0.3, 1024), "three-boxes-per-cta": (0.3, 2048)}[shape]
     fr, pp = synth.make_config(1, scale=scale)
     g, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
     n, T = g.n, pp["T"]
     boxes = (n + 63) // 64
     assert (boxes, n % 64 != 0) == ((36, True) if shape == "all-pairs-ragged" else (38, True)), (n, boxes)
+    plan = B.qhap_plan_pair_tiles(boxes, (R + 127) // 128, 148, 2)
+    assert plan[0] > 0 and (plan[2] >= 3) == (shape == "three-boxes-per-cta"), plan
     x0, y0 = synth.bsb_init_state(17, n, R)
 
     def run(path=1, **knobs):

@@ -332,3 +332,23 @@ def test_paired_tiles_are_bit_identical_to_single_boxes(B, oracle, shape):
     print(f"paired tiles {shape}: n {n} R {R}: 9 steps against the CSR path max|dx| {dx:.2e} max|dy| {dy:.2e}; 15 steps against the oracle "
           f"(4 replicas) {ox:.2e} {oy:.2e}")
     assert dx <= 1e-3 and dy <= 1e-3 and ox <= 1e-3 and oy <= 1e-3
+
+
+# ----------------------------------------------- whole solves at full size: same bits whatever the launch mode, run after run
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_full_size_solves_bit_identical_across_launch_modes(B, cfg):
+    """BASELINE configs 1 and 2 at full size, all 2,000 / 3,000 steps: the automatic setting (one fused cooperative launch, paired
+    tiles, y by plain loads, early staging reload) three times in a row, then one launch per step, single boxes, and single boxes
+    with the y ring -- final x, y, best cut and best replica agree bit for bit (a race in the tile-level step boundary of the
+    fused launch would show up here as a run-to-run difference)."""
+    import hashlib
+    import torch
+    fr, p = synth.make_config(cfg)
+    g, J = B.qhap_build_read_graph(B.upload_frags(fr), weight_mode=1, dense_dtype=B.QHAP_DENSE_FP16)
+    seen = []
+    for kw in (dict(), dict(), dict(), dict(step_launch=1), dict(pair_tiles=2), dict(pair_tiles=2, y_ring=1)):
+        r = B.qhap_bsb_solve(g, replicas=p["R"], steps_total=p["T"], seed=p["seed"], weight_mode=1, path=1, dense_J=J, tile_skip=1, **kw)
+        torch.cuda.synchronize()
+        h = hashlib.sha1(r["x"].cpu().numpy().tobytes() + r["y"].cpu().numpy().tobytes()).hexdigest()
+        seen.append((h, int(r["best_cut"][0]), int(r["best_replica"][0])))
+    assert len(set(seen)) == 1, seen

@@ -352,3 +352,22 @@ def test_full_size_solves_bit_identical_across_launch_modes(B, cfg):
         h = hashlib.sha1(r["x"].cpu().numpy().tobytes() + r["y"].cpu().numpy().tobytes()).hexdigest()
         seen.append((h, int(r["best_cut"][0]), int(r["best_replica"][0])))
     assert len(set(seen)) == 1, seen
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_snp_solves_repeat_bit_identically(B, cfg):
+    """BASELINE configs 3 (47 SNP blocks, block path) and 4 (Pore-C SNP graph, hybrid path with state16 next to the remainder
+    CSR) at full size, 300 steps: repeated runs agree bit for bit, and on config 3 so does the y ring against plain loads."""
+    import hashlib
+    import torch
+    fr, p = synth.make_config(cfg)
+    g = B.qhap_build_snp_graph(B.upload_frags(fr), p.get("linkage_tenths", 10), p.get("alpha", 0.1))
+    if "block" in p:
+        g = B.qhap_block_split(g, synth.block_windows(fr.n_snp, p["block"], p["stride"]))
+    seen = []
+    for kw in (dict(), dict()) + ((dict(y_ring=1),) if cfg == 3 else ()):
+        r = B.qhap_bsb_solve(g, replicas=p["R"], steps_total=p["T"], steps_run=300, seed=p["seed"], weight_mode=2, path=4, **kw)
+        torch.cuda.synchronize()
+        seen.append((hashlib.sha1(r["x"].cpu().numpy().tobytes() + r["y"].cpu().numpy().tobytes()).hexdigest(),
+                     tuple(r["best_cut"].cpu().tolist())))
+    assert len(set(seen)) == 1, [s[0] for s in seen]

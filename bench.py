@@ -513,7 +513,7 @@ def run_ours(args):
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if (blocks or (args.scaling == "strong" and world > 1)) else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": workload_name(args.config, fr, p),
-                      "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM)" if tile_skip else " full GEMM"),
+                      "path": {1: "dense-tcgen05" + (" tile_skip (non-zero k-blocks only; bit-identical to the full GEMM; state16, paired tiles, one fused cooperative launch per solve)" if tile_skip else " full GEMM"),
                                2: "sparse-csr", 3: "shared-memory resident (one launch for all steps)", 4: "tcgen05 step on the block-compressed J (64 x 64 tiles built from the CSR)"}[path],
                       "weight_mode": "fixed-point Eq. 14" if snp else "D-C", "replicas_per_gpu": R, "spins_solved": n_solved, "l2": f"flushed between iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                       "parallelism": f"blocks x{world} (strong)" if blocks else f"replicas x{world} ({args.scaling if world > 1 else 'weak'})",

@@ -135,7 +135,7 @@ typedef struct {
                           /*    trajectory drift); 2 = one accumulator.  Changes result bits (documented in DESIGN.md 4.4)       */
   int32_t y_ring;         /* state16: how y reaches the epilogue: automatic = 2 / 1 = per-warp TMA ring in shared memory, 2 = plain   */
                           /*    coalesced loads one work item ahead (frees the ring's 32 KB for another operand stage). Same bits      */
-  int32_t pair_tiles;     /* state16 on the dense tile_skip path: automatic / 1 = two neighbouring 64-spin boxes of a replica tile */
+  int32_t pair_tiles;     /* state16 on the dense tile_skip path and on path 4 with one J term and no remainder: automatic / 1 = two neighbouring 64-spin boxes of a replica tile */
                           /*    share one N = 128 accumulator where that does not unbalance the CTAs (each staged x k-block feeds  */
                           /*    128 output spins; y by plain loads unless y_ring = 1), 2 = every box on its own.  Same bits          */
   int32_t reserved[6];    /* must be 0                                                                                      */

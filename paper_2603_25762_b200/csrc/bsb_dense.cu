@@ -111,6 +111,12 @@ struct DenseArgs {
   int32_t pair_lines, n_slots;
   const int32_t* pk_cnt;      // [pair_lines] union of the two boxes' k-block lists
   const int32_t* pk_idx;      // [pair_lines][n_kblocks]
+  // block path: the union lists are stored back to back (pair q: entries pk_ptr[q] .. pk_ptr[q + 1]) with, per entry, the tile of
+  // the left and of the right box in the block arrays (a box that does not list the k-block points at an all-zero tile)
+  const int32_t* pk_ptr;      // [pair_lines + 1] or nullptr (dense path: pk_cnt / pk_idx)
+  const int32_t* pk_kb;
+  const int32_t* pk_l;
+  const int32_t* pk_r;
 };
 
 struct Slot { int tn0, tm, width, q; };
@@ -141,7 +147,11 @@ __device__ __forceinline__ Slot slot_of(const DenseArgs& a, int slot) {
 template <bool PAIR>
 __device__ __forceinline__ const int32_t* slot_list(const DenseArgs& a, const Slot& sl, int& nkb) {
   if (a.kb_cnt == nullptr) { nkb = a.n_kblocks; return nullptr; }
-  if (PAIR && sl.width == 2) { nkb = a.pk_cnt[sl.q]; return a.pk_idx + size_t(sl.q) * a.n_kblocks; }
+  if (PAIR && sl.width == 2) {
+    if (a.pk_ptr) { const int32_t b = a.pk_ptr[sl.q]; nkb = a.pk_ptr[sl.q + 1] - b; return a.pk_kb + b; }
+    nkb = a.pk_cnt[sl.q];
+    return a.pk_idx + size_t(sl.q) * a.n_kblocks;
+  }
   nkb = a.kb_cnt[sl.tn0];
   return a.kb_idx + size_t(sl.tn0) * a.n_kblocks;
 }
@@ -467,15 +477,29 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
         const CUtensorMap* mh = (s & 1) ? &tm_oh : &tm_xh;               // odd steps of a fused launch read what even steps wrote
         const CUtensorMap* ml = (s & 1) ? &tm_ol : &tm_xl;
         const uint32_t stage_tx = kTileJ * uint32_t(a.j_terms) * uint32_t(sl.width) + 2u * kStageX;
+        // the list entries of k-block j + 1 are requested before k-block j is issued, so that their round trip is not on the
+        // path of every stage
+        const bool bpair = PAIR && sl.width == 2 && a.blk_ptr != nullptr;
+        const int32_t e0 = bpair ? a.pk_ptr[sl.q] : 0;
+        int kb_n = list ? list[0] : 0, tl_n = bpair ? a.pk_l[e0] : 0, tr_n = bpair ? a.pk_r[e0] : 0;
         for (int j = 0; j < nkb; ++j) {
-          const int kb = list ? list[j] : j;
+          const int kb = kb_n, tl = tl_n, tr = tr_n;
+          if (j + 1 < nkb) {
+            kb_n = list ? list[j + 1] : j + 1;
+            if (bpair) { tl_n = a.pk_l[e0 + j + 1]; tr_n = a.pk_r[e0 + j + 1]; }
+          }
           ptx::mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t sj = smem_base + stage * kStageBytes;
           ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx);
           if (a.blk_ptr) {
-            const int brow = (a.blk_ptr[tn] + j) * kBK;
-            ptx::tma_load_2d(sj, &tm_j, full_bar(stage), 0, brow);
-            if (a.j_terms == 2) ptx::tma_load_2d(sj + kTileJ, &tm_jl, full_bar(stage), 0, brow);
+            if (bpair) {                                              // one J term; tiles of the left and the right box
+              ptx::tma_load_2d(sj, &tm_j, full_bar(stage), 0, tl * kBK);
+              ptx::tma_load_2d(sj + kTileJ, &tm_j, full_bar(stage), 0, tr * kBK);
+            } else {
+              const int brow = (a.blk_ptr[tn] + j) * kBK;
+              ptx::tma_load_2d(sj, &tm_j, full_bar(stage), 0, brow);
+              if (a.j_terms == 2) ptx::tma_load_2d(sj + kTileJ, &tm_jl, full_bar(stage), 0, brow);
+            }
           } else {
             ptx::tma_load_2d(sj, &tm_j, full_bar(stage), kb * kBK, tn * a.BN);
             if (PAIR && sl.width == 2) ptx::tma_load_2d(sj + kTileJ, &tm_j, full_bar(stage), kb * kBK, (tn + 1) * a.BN);   // rows 64..127
@@ -803,7 +827,7 @@ dense_step_kernel(const __grid_constant__ CUtensorMap tm_j, const __grid_constan
             for (int j = 0; j < kChunk; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v2[j]));
           }
           if (first) set_step(p.vt);                         // the ramp constant changes between boxes only
-          if constexpr (PAIR) {                              // pairs exist on the dense path only: one c1 for all rows
+          if constexpr (PAIR) {                              // pairs: one instance, one c1 for all rows (dense and block path)
             epi_update_x16<HINTS, false>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
           } else if constexpr (XW) {                         // hybrid block path: per-row c1, fp32 x written next to the pair
             epi_update_x16<HINTS, true, true>(a, ec, p.tn, p.tm, p.ch, v, yc, stg);
@@ -1032,6 +1056,32 @@ __global__ void __launch_bounds__(32) pair_list_kernel(int32_t n_kblocks, const 
     if (cnt == 0) { out[0] = min(n_kblocks - 1, 2 * q); cnt = 1; }
     pk_cnt[q] = cnt;
   }
+}
+
+// Block path pairs: merge of the ascending k-block lists of boxes 2q and 2q + 1.  FILL = false: union sizes; FILL = true: the
+// union (pk_kb) with the tile of each box in the block arrays, `zero_tile` for a box that does not list the k-block.
+template <bool FILL>
+__global__ void __launch_bounds__(128) pair_merge_kernel(int32_t P, int32_t n_kblocks, const int32_t* __restrict__ kb_cnt,
+                                                         const int32_t* __restrict__ kb_idx, const int32_t* __restrict__ blk_ptr,
+                                                         int32_t zero_tile, int32_t* __restrict__ pk_ptr, int32_t* __restrict__ pk_kb,
+                                                         int32_t* __restrict__ pk_l, int32_t* __restrict__ pk_r) {
+  const int32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= P) return;
+  const int32_t *la = kb_idx + size_t(2 * q) * n_kblocks, *lb = la + n_kblocks;
+  const int32_t na = kb_cnt[2 * q], nb = kb_cnt[2 * q + 1], ba = blk_ptr[2 * q], bb = blk_ptr[2 * q + 1];
+  int32_t i = 0, j = 0, out = FILL ? pk_ptr[q] : 0;
+  while (i < na || j < nb) {
+    const int32_t ka = i < na ? la[i] : INT32_MAX, kb = j < nb ? lb[j] : INT32_MAX, k = min(ka, kb);
+    if (FILL) {
+      pk_kb[out] = k;
+      pk_l[out] = ka == k ? ba + i : zero_tile;
+      pk_r[out] = kb == k ? bb + j : zero_tile;
+    }
+    ++out;
+    if (ka == k) ++i;
+    if (kb == k) ++j;
+  }
+  if (!FILL) pk_ptr[q] = out;
 }
 
 // ------------------------------------------------------------------- block-compressed J (64 x 64 fp16 tiles) from a CSR
@@ -1556,6 +1606,7 @@ qhap_status dense_solve_steps(const CsrView& g, const void* dense_J, int32_t ld,
   a.c1 = c1_dev; a.c1_per_row = 0; a.j_terms = 1; a.blk_ptr = nullptr;
   a.x = x; a.y = y;
   a.xw32 = 0; a.early_reload = 0; a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = w.pk_cnt; a.pk_idx = w.pk_idx;
+  a.pk_ptr = nullptr; a.pk_kb = nullptr; a.pk_l = nullptr; a.pk_r = nullptr;
   set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_j, tm_h[2], tm_l[2], tm_sx, tm_sy;
@@ -1649,6 +1700,7 @@ struct BlockWs {
   __half* xh[2];
   __half* xl[2];
   int32_t *kb_cnt, *blk_ptr, *kb_idx, *flags;
+  int32_t *pk_ptr, *pk_kb, *pk_l, *pk_r;      // pairs (single-term J without a remainder): union lists, back to back
   float *c1row, *c1plain;
   int32_t *rem_ptr, *rem_col;
   float* rem_val;
@@ -1679,7 +1731,11 @@ BlockWs carve_block(Workspace& ws, int32_t n, int64_t nnz, int32_t R) {
   w.scan_scratch = ws.take<int64_t>(size_t(ceil_div(int64_t(n), 4096)) + 1);
   w.done = ws.take<uint32_t>(n_t * size_t(ceil_div(R, kBM)));   // fused steps
   w.cap_blocks = block_capacity(n, nnz);
-  const size_t cap = size_t(w.cap_blocks) * kBK * kBK;
+  w.pk_ptr = ws.take<int32_t>(n_t / 2 + 2);
+  w.pk_kb = ws.take<int32_t>(size_t(w.cap_blocks));
+  w.pk_l = ws.take<int32_t>(size_t(w.cap_blocks));
+  w.pk_r = ws.take<int32_t>(size_t(w.cap_blocks));
+  const size_t cap = size_t(w.cap_blocks + 1) * kBK * kBK;          // + one all-zero tile for the pairs
   w.jh = ws.take<__half>(cap);
   w.jl = ws.take<__half>(cap);
   return w;
@@ -1770,7 +1826,7 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   block_scale_kernel<<<int(ceil_div(std::max(n, 1), 256)), 256, 0, stream>>>(n, n_inst, inst_ptr_dev, c1_dev, scal, two_terms ? 0 : 1,
                                                                             scale, c1row, c1plain);
   QHAP_LAUNCH_CHECK();
-  QHAP_CUDA_TRY(cudaMemsetAsync(jh, 0, sizeof(__half) * size_t(total_blocks) * kBK * kBK, stream));
+  QHAP_CUDA_TRY(cudaMemsetAsync(jh, 0, sizeof(__half) * size_t(total_blocks + 1) * kBK * kBK, stream));   // + the zero tile
   if (two_terms) QHAP_CUDA_TRY(cudaMemsetAsync(jl, 0, sizeof(__half) * size_t(total_blocks) * kBK * kBK, stream));
   block_fill_kernel<<<int(ceil_div(int64_t(n) * 32, 256)), 256, 0, stream>>>(n, g.row_ptr, g.col, jval, n_t, kb_cnt, kb_idx, blk_ptr,
                                                                             scale, jh, two_terms ? jl : nullptr);
@@ -1795,15 +1851,19 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
   a.kb_cnt = kb_cnt; a.kb_idx = kb_idx; a.blk_ptr = blk_ptr;
   a.xw32 = (a.x16 && has_rem) ? 1 : 0;
   a.early_reload = 0;
+  a.pk_ptr = nullptr; a.pk_kb = nullptr; a.pk_l = nullptr; a.pk_r = nullptr;
   a.pair_lines = 0; a.n_slots = a.n_tiles_m * a.n_tiles_n; a.pk_cnt = nullptr; a.pk_idx = nullptr;
   a.c1 = c1row; a.c1_per_row = 1;
+  if (n_inst == 1 && !two_terms && !has_rem) {      // one instance, unit scale: every row has the same factor c1 2^-15 -- the dense path's form (the kernel next to a remainder CSR is built for per-row factors)
+    a.c1 = c1plain; a.c1_per_row = 0;   // (bit for bit: c1row[i] = c1 2^-15 / 1), without the per-item loads of the row factors
+  }
   a.x = x; a.y = y;
   set_l2_policies(a, t); a.n_steps = 1; a.fused = 0; a.fence_every = 1; a.k0 = 0; a.steps_total = p.steps_total; a.dt = p.dt; a.a0 = p.a0; a.done = nullptr;
 
   CUtensorMap tm_jh, tm_jl, tm_h[2], tm_l[2], tm_sx, tm_sy;
   QHAP_TRY(make_state_map(&tm_sx, x, n, a.ring ? R : 4));
   QHAP_TRY(make_state_map(&tm_sy, y, n, a.ring ? R : 4));
-  const uint64_t brows = uint64_t(std::max<int64_t>(total_blocks, 1)) * kBK;
+  const uint64_t brows = uint64_t(total_blocks + 1) * kBK;
   QHAP_TRY(make_map(&tm_jh, jh, kBK, brows, kBK, kBK));
   QHAP_TRY(make_map(&tm_jl, two_terms ? jl : jh, kBK, brows, kBK, kBK));
   for (int b = 0; b < 2; ++b) {
@@ -1817,11 +1877,35 @@ qhap_status block_solve_steps(const CsrView& g, const float* jval, int32_t weigh
     merge_x_kernel<<<tgrid, 256, 0, stream>>>(n, R, n_k, xh[0], xl[0], x);
     QHAP_LAUNCH_CHECK();
   }
-  const int grid = int(std::min<int64_t>(int64_t(a.n_tiles_m) * a.n_tiles_n, sm_count()));
-  a.tile_stride = int32_t(ceil_div(int64_t(a.n_tiles_m) * a.n_tiles_n, grid) * grid);
-  int cur = 0;
   // the remainder gather reads the fp32 x of the whole graph between two tile steps: a grid-wide step boundary
-  if (const int gf = has_rem ? 0 : fused_grid(a, p, t)) {
+  const int gf = has_rem ? 0 : fused_grid(a, p, t);
+  // Paired tiles as on the dense path, for one J term (read graphs) without a remainder: the union lists carry,
+  // per k-block, the tile of the left and of the right box; a box that does not list the k-block gets the all-zero tile.
+  if (a.x16 && !has_rem && !two_terms && a.stg_bufs == 2 && t.pair_tiles != 2 && n_inst == 1) {
+    const int g0 = gf ? gf : int(std::min<int64_t>(a.n_slots, sm_count()));
+    const int32_t P = choose_pair_lines(a.n_tiles_n, a.n_tiles_m, g0, gf ? 2 : 0);
+    if (P > 0) {
+      DenseArgs b = a;
+      b.pair_lines = P;
+      b.n_slots = P * a.n_tiles_m + (a.n_tiles_n - 2 * P) * a.n_tiles_m;
+      if (t.y_ring != 1) b.yldg = 1;
+      choose_staging(b, 2 * kBK * kBK * 2 + 2 * kStageX, t);
+      if (b.n_stages >= 2 && b.stg_bufs == 2) {
+        a = b;
+        const int pb = int(ceil_div(P, 128));
+        pair_merge_kernel<false><<<pb, 128, 0, stream>>>(P, n_t, kb_cnt, kb_idx, blk_ptr, int32_t(total_blocks), w.pk_ptr, w.pk_kb, w.pk_l, w.pk_r);
+        QHAP_LAUNCH_CHECK();
+        QHAP_TRY(exclusive_scan_i32(w.pk_ptr, w.pk_ptr, P, totals, reinterpret_cast<int32_t*>(totals + 1), stream, scan_scratch));
+        pair_merge_kernel<true><<<pb, 128, 0, stream>>>(P, n_t, kb_cnt, kb_idx, blk_ptr, int32_t(total_blocks), w.pk_ptr, w.pk_kb, w.pk_l, w.pk_r);
+        QHAP_LAUNCH_CHECK();
+        a.pk_ptr = w.pk_ptr; a.pk_kb = w.pk_kb; a.pk_l = w.pk_l; a.pk_r = w.pk_r;
+      }
+    }
+  }
+  const int grid = int(std::min<int64_t>(a.n_slots, sm_count()));
+  a.tile_stride = int32_t(ceil_div(int64_t(a.n_slots), grid) * grid);
+  int cur = 0;
+  if (gf) {
     QHAP_TRY(launch_fused(gf, stream, tm_jh, tm_jl, tm_h, tm_l, tm_sx, tm_sy, a, p, done, cur));
   } else {
     for (int32_t k = p.step_begin; k < p.step_begin + p.steps_run; ++k) {

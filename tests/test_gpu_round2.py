@@ -315,7 +315,9 @@ def test_paired_tiles_are_bit_identical_to_single_boxes(B, oracle, shape):
 
     ref = run(pair_tiles=2, step_launch=1)
     for knobs in (dict(pair_tiles=1), dict(pair_tiles=1, step_launch=1), dict(pair_tiles=1, y_ring=1), dict(pair_tiles=1, y_ring=1, step_launch=1),
-                  dict(pair_tiles=2), dict()):
+                  dict(pair_tiles=2), dict(),
+                  # the block path on the same read graph (tiles built from the CSR; pairs carry per-box tiles and a zero tile)
+                  dict(path=4), dict(path=4, step_launch=1), dict(path=4, pair_tiles=2), dict(path=4, y_ring=1)):
         got = run(**knobs)
         for a, b in zip(ref, got):
             assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]), (shape, knobs)

@@ -16,6 +16,10 @@
 // TMA stores of the fp16 copies, warps 2..17 = epilogue (TMEM lane quarter = warp % 4, four warps per quarter interleave 8-column chunks; the state of
 // the next chunk is prefetched into registers; at BN = 64 the fp16 copies leave through shared memory and TMA stores).
 // Pipelines: n_stages shared-memory stages (full/empty mbarriers) and 2 TMEM accumulator stages (tmem_full/tmem_empty).
+// Later additions, each described where it lives (DESIGN.md 4.4d-g): fused launches (all steps of a call in one cooperative
+// launch, tile-level step boundary through done[]), state16 (x carried between steps as the fp16 pair; kernels X16), split
+// accumulators, paired tiles (two 64-spin boxes per N = 128 accumulator; kernels PAIR), y by plain loads with its own epilogue
+// loop (kernels YLDG), the fp32 x written next to the pair for the remainder gather of the hybrid block path (kernels XW).
 #include <cuda.h>
 #include <cuda_fp16.h>
 
